@@ -1,0 +1,676 @@
+"""Pins of the CPU oracle to what the paper and the mathematics fix (no GPU, no CUDA library).
+
+Each test cites the PAPER.md passage (line + equation) whose content it pins and is chosen so that a
+plausible mistake in oracle/ref_lbm.cpp (a dropped term, a wrong sign or index, a transposed
+operand, a wrong weight) fails at least one of them.  Nothing here calls paper_2502_12955_b200.
+"""
+import fractions
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+from oracle.ref_lbm import RefLBM, lattice_table
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def make(cfg):
+    return RefLBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+
+
+def rest_populations(w, rho):
+    """f_i = w_i rho: the u = 0 equilibrium of Eq. 6; an input, not the method."""
+    return np.stack([wi * rho for wi in w])
+
+
+# ----------------------------------------------------------------------------------------------
+# lattice tables: Tables 1-3
+# ----------------------------------------------------------------------------------------------
+def parse_golden():
+    out, cur = {}, None
+    for line in open(os.path.join(GOLDEN, "lattice_tables.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        if line.startswith("["):
+            cur = line.strip("[]")
+            out[cur] = {}
+            continue
+        key, *vals = line.split()
+        out[cur][key] = [float(fractions.Fraction(v)) for v in vals]
+    return out
+
+
+@pytest.mark.parametrize("name,lattice,kind", [("D3Q19", "D3Q19", 0), ("D2Q9", "D2Q9", 0), ("D2Q5", "D2Q9", 1)])
+def test_lattice_tables_match_paper(name, lattice, kind):
+    g = parse_golden()[name]
+    c, w = lattice_table(lattice, kind)
+    assert np.allclose(w, g["w"], rtol=0, atol=1e-16)
+    assert np.array_equal(c[:, 0], np.array(g["cx"], int))
+    assert np.array_equal(c[:, 1], np.array(g["cy"], int))
+    if "cz" in g:
+        assert np.array_equal(c[:, 2], np.array(g["cz"], int))
+    else:
+        assert not c[:, 2].any()
+
+
+@pytest.mark.parametrize("lattice,kind,cs2", [("D3Q19", 0, 1 / 3), ("D2Q9", 0, 1 / 3), ("D2Q9", 1, 0.3), ("D3Q19", 1, 0.25)])
+def test_lattice_isotropy(lattice, kind, cs2):
+    """weights sum to one, sum w c = 0, sum w c_a c_b = c_s^2 delta_ab; every c has its opposite."""
+    c, w = lattice_table(lattice, kind)
+    d = 3 if lattice == "D3Q19" else 2
+    assert abs(w.sum() - 1) < 1e-15
+    assert np.abs((w[:, None] * c).sum(0)).max() < 1e-16
+    M = np.einsum("i,ia,ib->ab", w, c, c)[:d, :d]
+    assert np.abs(M - cs2 * np.eye(d)).max() < 1e-15
+    vecs = {tuple(v) for v in c.tolist()}
+    assert len(vecs) == len(c) and all(tuple(-np.array(v)) in vecs for v in vecs)
+    if kind == 0:  # fourth-order isotropy needed by Eq. 6: sum w c_a c_b c_g c_d = c_s^4 (dd + dd + dd)
+        T = np.einsum("i,ia,ib,ic,id->abcd", w, c, c, c, c)[:d, :d, :d, :d]
+        e = np.eye(d)
+        iso = cs2 ** 2 * (np.einsum("ab,cd->abcd", e, e) + np.einsum("ac,bd->abcd", e, e) + np.einsum("ad,bc->abcd", e, e))
+        assert np.abs(T - iso).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# equilibrium, Eq. 6-8: moments of the initial (equilibrium) populations
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lattice,grid", [("D2Q9", (16, 12, 1)), ("D3Q19", (8, 8, 8))])
+def test_equilibrium_moments(lattice, grid):
+    r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(0.8, 0.8), rho_init=(1.3, 1.0), u0=0.07, init_kind="TAYLOR_GREEN")
+    r.init_from_seed(0)
+    c, w = lattice_table(lattice)
+    f, _ = r.split_populations(r.get_populations())
+    f = f[0]
+    m = r.get_macros()
+    rho, u = m["rho"][0], m["u"]
+    d = r.d
+    assert np.abs(f.sum(0) - rho).max() < 1e-15
+    for a in range(d):
+        assert np.abs((c[:, a, None] * f).sum(0) - rho * u[a]).max() < 1e-16
+    assert np.abs(u).max() > 0.05  # the velocity field is not trivially zero
+    for a in range(d):
+        for b in range(d):
+            Pi = (c[:, a, None] * c[:, b, None] * f).sum(0)
+            expect = rho * u[a] * u[b] + (rho / 3.0 if a == b else 0.0)
+            assert np.abs(Pi - expect).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# config 1: Taylor-Green decay, nu = (tau - 1/2)/3 ; pins BGK collision + periodic streaming
+# Eq. 3-6
+# ----------------------------------------------------------------------------------------------
+def test_taylor_green_decay_cfg1():
+    cfg = workloads.config("cfg1")
+    r = make(cfg)
+    r.init_from_seed(1)
+    nx, ny, _ = cfg["grid"]
+    k = 2 * np.pi / nx
+    X, Y = np.meshgrid(np.arange(nx), np.arange(ny), indexing="xy")
+    mode_x = (-np.cos(k * X) * np.sin(k * Y)).ravel()
+    mode_y = (np.sin(k * X) * np.cos(k * Y)).ravel()
+    nu = (0.8 - 0.5) / 3.0
+    amps, times = [], []
+    mass0 = r.get_macros()["rho"].sum()
+    t = 0
+    for _ in range(10):
+        r.step(100)
+        t += 100
+        m = r.get_macros()
+        ax = (m["u"][0] * mode_x).sum() / (mode_x ** 2).sum()
+        ay = (m["u"][1] * mode_y).sum() / (mode_y ** 2).sum()
+        assert abs(ax - ay) < 1e-12  # the vortex stays symmetric
+        # the field stays a pure mode
+        assert np.abs(m["u"][0] - ax * mode_x).max() < 2e-4 * 0.01
+        amps.append(ax)
+        times.append(t)
+    amps, times = np.array(amps), np.array(times)
+    exact = 0.01 * np.exp(-2 * nu * k * k * times)
+    assert abs(amps[-1] / exact[-1] - 1) < 5e-3          # amplitude at t = 1000 (0.145489 u0)
+    rate = -np.polyfit(times[1:], np.log(amps[1:]), 1)[0]
+    assert abs(rate / (2 * nu * k * k) - 1) < 1e-3       # decay rate pins nu = (tau-1/2)/3
+    assert abs(r.get_macros()["rho"].sum() - mass0) < 1e-9
+
+
+def test_taylor_green_viscosity_depends_on_tau():
+    """the rate changes with tau as (tau - 1/2)/3: pins the 1/tau in Eq. 3 against e.g. tau vs 1/tau mix-ups"""
+    rates = []
+    for tau in (0.6, 1.0, 1.4):
+        r = RefLBM(32, 32, 1, "D2Q9", "BGK", precision=64, tau=(tau, tau), u0=0.01, init_kind="TAYLOR_GREEN")
+        r.init_from_seed(0)
+        k = 2 * np.pi / 32
+        X, Y = np.meshgrid(np.arange(32), np.arange(32), indexing="xy")
+        mode = (-np.cos(k * X) * np.sin(k * Y)).ravel()
+        r.step(100)
+        a1 = (r.get_macros()["u"][0] * mode).sum() / (mode ** 2).sum()
+        r.step(200)
+        a2 = (r.get_macros()["u"][0] * mode).sum() / (mode ** 2).sum()
+        rates.append(-np.log(a2 / a1) / 200 / (2 * k * k))
+    assert np.allclose(rates, [(t - 0.5) / 3 for t in (0.6, 1.0, 1.4)], rtol=1.5e-2)
+
+
+def test_taylor_green_3d_short_time():
+    """Eq. 45 on D3Q19: at t -> 0 the kinetic energy decays at 2 nu |k|^2 with |k|^2 = 3 k^2."""
+    n, tau = 24, 0.8
+    r = RefLBM(n, n, n, "D3Q19", "BGK", precision=64, tau=(tau, tau), u0=0.002, init_kind="TAYLOR_GREEN")
+    r.init_from_seed(0)
+    k = 2 * np.pi / n
+
+    def energy():
+        m = r.get_macros()
+        return float((m["u"] ** 2).sum())
+
+    r.step(20)
+    e1 = energy()
+    r.step(40)
+    e2 = energy()
+    rate = -np.log(e2 / e1) / 40
+    nu = (tau - 0.5) / 3
+    assert abs(rate / (2 * nu * 3 * k * k * 2 / 2) - 1) < 0.02  # energy ~ amplitude^2: 2 * (nu * 3 k^2)
+
+
+# ----------------------------------------------------------------------------------------------
+# config 4: Guo body force + halfway bounce-back walls -> Poiseuille parabola (PAPER.md:504-531,
+# Eq. 43-44 with the missing 1/2 restored; Eq. 20-23; bounce-back PAPER.md:446, 525)
+# ----------------------------------------------------------------------------------------------
+def poiseuille_exact(nz, tau, g):
+    nu = (tau - 0.5) / 3
+    z = np.arange(nz)
+    return (g / (2 * nu)) * (z + 0.5) * (nz - z - 0.5) + (g / (8 * nu)) * (16 * (tau - 0.5) ** 2 / 3 - 1)
+
+
+@pytest.mark.parametrize("tau", [0.6, 0.9, 0.5 + np.sqrt(3.0 / 16.0), 1.2])
+def test_poiseuille_profile(tau):
+    nz, g = 16, 1e-6
+    cfg = workloads.config("cfg4", grid=(1, 1, nz), tau=(tau, tau))
+    r = make(cfg)
+    r.init_from_seed(0)
+    r.step(int(30 * nz * nz / ((tau - 0.5) / 3)))
+    m = r.get_macros()
+    ex = poiseuille_exact(nz, tau, g)
+    assert np.abs(m["u"][0] - ex).max() / ex.max() < 1e-8
+    assert np.abs(m["u"][1]).max() == 0 and np.abs(m["u"][2]).max() < 1e-12   # round-off only
+    assert np.abs(m["rho"] - 1).max() < 1e-10                 # round-off accumulated over ~1e5 steps
+    # discrete second difference = -g/nu exactly (independent of the wall slip)
+    d2 = m["u"][0][2:] - 2 * m["u"][0][1:-1] + m["u"][0][:-2]
+    assert np.allclose(d2, -g / ((tau - 0.5) / 3), rtol=1e-6)
+
+
+def test_poiseuille_xy_invariance_is_bit_exact():
+    """a 3x2xnz channel equals the 1x1xnz one bit for bit (used by the 256^3 GPU parity test)"""
+    nz = 12
+    a = make(workloads.config("cfg4", grid=(1, 1, nz)))
+    b = make(workloads.config("cfg4", grid=(3, 2, nz)))
+    for r in (a, b):
+        r.init_from_seed(0)
+        r.step(57)
+    ua, ub = a.get_macros()["u"], b.get_macros()["u"].reshape(3, nz, 2, 3)
+    for x in range(3):
+        for y in range(2):
+            assert np.array_equal(ub[:, :, y, x], ua)
+    fa = a.get_populations().reshape(19, nz)
+    fb = b.get_populations().reshape(19, nz, 6)
+    assert np.array_equal(fb[:, :, 4], fa)
+
+
+def test_walls_on_other_axes_and_2d():
+    """the same channel with walls on x (3D) and on y (2D): pins the bounce-back index logic per axis"""
+    n, tau, g = 12, 0.9, 1e-6
+    ex = poiseuille_exact(n, tau, g)
+    r = RefLBM(n, 1, 1, "D3Q19", "BGK", precision=64, tau=(tau, tau), force=(0, g, 0), bc=(1, 0, 0))
+    r.init_from_seed(0)
+    r.step(40000)
+    assert np.abs(r.get_macros()["u"][1] - ex).max() / ex.max() < 1e-8
+    r = RefLBM(1, n, 1, "D2Q9", "BGK", precision=64, tau=(tau, tau), force=(g, 0, 0), bc=(0, 1, 0))
+    r.init_from_seed(0)
+    r.step(40000)
+    assert np.abs(r.get_macros()["u"][0] - ex).max() / ex.max() < 1e-8
+
+
+def test_poiseuille_fp32_close_to_closed_form():
+    nz, tau, g = 16, 0.9, 1e-5
+    r = make(workloads.config("cfg4", grid=(1, 1, nz), precision=32, force=(g, 0, 0)))
+    r.init_from_seed(0)
+    r.step(60000)
+    ex = poiseuille_exact(nz, tau, g)
+    assert np.abs(r.get_macros()["u"][0] - ex).max() / ex.max() < 2e-3
+
+
+# ----------------------------------------------------------------------------------------------
+# Guo forcing bookkeeping, Eq. 15, 20, 22
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lattice,grid,force", [("D2Q9", (6, 5, 1), (3e-5, -2e-5, 0.0)), ("D3Q19", (4, 5, 3), (1e-5, 2e-5, -3e-5))])
+def test_uniform_force_momentum_growth(lattice, grid, force):
+    """periodic box, uniform force density F: every step adds exactly F to the momentum of each cell, and the
+    physical velocity carries the half-force shift: u(t) = F (t + 1/2) / rho.  Pins (1 - 1/2tau) F_i and F/2."""
+    tau = 0.77
+    r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(tau, tau), force=force, rho_init=(1.25, 1.0))
+    r.init_from_seed(0)
+    c, _ = lattice_table(lattice)
+    for t in (0, 1, 7, 40):
+        if t:
+            r.step(t - r_t)
+        r_t = t
+        m = r.get_macros()
+        f, _ = r.split_populations(r.get_populations())
+        for a in range(r.d):
+            assert np.allclose(m["u"][a], force[a] * (t + 0.5) / 1.25, rtol=1e-11, atol=1e-19)
+            mom = (c[:, a, None] * f[0]).sum(0)
+            assert np.allclose(mom, force[a] * t, rtol=1e-10, atol=1e-18)
+        assert np.abs(m["rho"] - 1.25).max() < 1e-13
+
+
+def noise_cfg(model, lattice, grid, precision=64, **kw):
+    base = dict(precision=precision, tau=(1.0, 0.9), tau_c=0.8, psi_kind=1, G=workloads.G12, k_react=0.0,
+                init_kind="UNIFORM_NOISE", rho_init=(1.0, 0.8), noise_amp=0.05, c_init=0.7)
+    if model == "SC1":
+        base.update(psi_kind=0, G=((-5.0, 0), (0, 0)), rho_init=(0.7, 1.0))
+    base.update(kw)
+    return RefLBM(*grid, lattice, model, **base)
+
+
+@pytest.mark.parametrize("model,lattice,grid", [
+    ("BGK", "D2Q9", (9, 7, 1)), ("SC1", "D2Q9", (16, 16, 1)), ("SC2", "D2Q9", (16, 12, 1)), ("SC2_ADE", "D2Q9", (12, 12, 1)),
+    ("SC1", "D3Q19", (8, 6, 7)), ("SC2_ADE", "D3Q19", (8, 8, 6))])
+def test_mass_and_momentum_conservation(model, lattice, grid):
+    """sum_x rho^sigma is invariant (sum_i F_i = 0, sum_i f^eq = rho); the Shan-Chen force sums to zero over a
+    periodic box, so the total momentum sum_x sum_sigma j^sigma is invariant too; k = 0 conserves sum C."""
+    # total momentum is conserved by the multi-component Guo scheme only for equal relaxation times:
+    # sum_sigma omega^sigma (j^sigma - rho^sigma u^b) = -omega sum F / 2 needs a common omega (Eq. 15, 20)
+    r = noise_cfg(model, lattice, grid, tau=(0.9, 0.9))
+    r.init_from_seed(11)
+    c, _ = lattice_table(lattice)
+
+    def totals():
+        f, h = r.split_populations(r.get_populations())
+        mass = f.sum(axis=(1, 2))
+        mom = np.array([(c[:, a, None] * f.sum(0)).sum() for a in range(r.d)])
+        return mass, mom, (h.sum() if h is not None else 0.0)
+
+    m0, p0, c0 = totals()
+    r.step(200)
+    m1, p1, c1 = totals()
+    assert np.abs(m1 - m0).max() / m0.max() < 1e-13
+    assert np.abs(p1 - p0).max() / m0.sum() < 1e-13
+    assert abs(c1 - c0) <= 1e-13 * max(abs(c0), 1)
+    if model != "BGK":
+        F = r.get_force()
+        assert np.abs(F.sum(axis=(0, 2))).max() < 1e-12          # Newton's third law over the box
+        assert np.abs(F).max() > 1e-5                            # ... of a force that is not trivially zero
+
+
+# ----------------------------------------------------------------------------------------------
+# Shan-Chen force against the literal pair sum of Eq. 9, discretised as stated
+# at PAPER.md:126: G(x~ - x) = w_i G if x~ - x = c_i, else 0.   Eq. 11 / 13
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("model,lattice,grid", [("SC1", "D2Q9", (8, 8, 1)), ("SC2", "D2Q9", (8, 8, 1)), ("SC2_ADE", "D3Q19", (6, 6, 6))])
+def test_shan_chen_force_equals_pair_sum(model, lattice, grid):
+    G = ((-5.0, 0.0), (0.0, 0.0)) if model == "SC1" else ((0.3, 1.2), (1.2, -0.4))
+    r = noise_cfg(model, lattice, grid, G=G)
+    r.init_from_seed(5)
+    r.step(3)  # a state with non-trivial velocity
+    m = r.get_macros()
+    F = r.get_force()
+    nx, ny, nz = grid
+    c, w = lattice_table(lattice)
+    S, d, N = r.S, r.d, r.N
+    rho = m["rho"]
+    psi = rho if model != "SC1" else 1.0 - np.exp(-rho)
+    wmap = {tuple(ci): wi for ci, wi in zip(c.tolist(), w)}
+    coords = [(x, y, z) for z in range(nz) for y in range(ny) for x in range(nx)]
+    Fb = np.zeros((S, d, N))
+    for a_idx, xa in enumerate(coords):
+        for b_idx, xb in enumerate(coords):
+            if a_idx == b_idx:
+                continue
+            # every periodic image of xb that is a lattice neighbour of xa
+            for sx in (-nx, 0, nx):
+                for sy in (-ny, 0, ny):
+                    for sz in ((-nz, 0, nz) if nz > 1 else (0,)):
+                        dv = (xb[0] + sx - xa[0], xb[1] + sy - xa[1], xb[2] + sz - xa[2])
+                        wi = wmap.get(dv)
+                        if wi is None:
+                            continue
+                        for s in range(S):
+                            for t in range(S):
+                                for a in range(d):
+                                    Fb[s, a, a_idx] -= dv[a] * wi * G[s][t] * psi[s, a_idx] * psi[t, b_idx]
+    assert np.abs(F - Fb).max() < 1e-14
+    assert np.abs(Fb).max() > 1e-3
+
+
+def test_shan_chen_force_uniform_and_linear_psi():
+    """uniform psi -> F = 0; psi linear in x -> F_x = -G psi c_s^2 dpsi/dx (continuum limit of Eq. 11)"""
+    nx, ny = 16, 6
+    c, w = lattice_table("D2Q9")
+    r = RefLBM(nx, ny, 1, "D2Q9", "SC1", precision=64, tau=(1, 1), psi_kind=1, G=((-3.0, 0), (0, 0)))
+    x = np.arange(nx)
+    for slope in (0.0, 0.01):
+        rho = np.tile(1.0 + slope * x, ny)
+        r.set_populations(rest_populations(w, rho).ravel())
+        F = r.get_force()[0].reshape(2, ny, nx)
+        inner = slice(1, nx - 1)
+        expect = -(-3.0) * (1.0 + slope * x[inner]) * (1.0 / 3.0) * slope
+        assert np.abs(F[0][:, inner] - expect).max() < 1e-15
+        assert np.abs(F[1][:, inner]).max() < 1e-16
+
+
+def test_shan_chen_3d_gradient_each_axis():
+    c, w = lattice_table("D3Q19")
+    n = 8
+    r = RefLBM(n, n, n, "D3Q19", "SC1", precision=64, tau=(1, 1), psi_kind=1, G=((2.0, 0), (0, 0)))
+    idx = np.indices((n, n, n))  # [z, y, x] order of axes -> map axis a to array
+    for a in range(3):
+        coord = idx[2 - a].ravel().astype(float)
+        rho = 1.0 + 0.02 * coord
+        r.set_populations(rest_populations(w, rho).ravel())
+        F = r.get_force()[0]
+        inner = (coord > 0) & (coord < n - 1)
+        for b in range(3):
+            expect = -2.0 * rho * (1 / 3) * 0.02 if a == b else 0.0 * rho
+            assert np.abs((F[b] - expect)[inner]).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# config 2: Laplace law, Eq. 47, with the single-component EOS p = rho/3 + G psi^2/6
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.slow
+def test_laplace_law_reduced_cfg2():
+    n = 96
+    res = []
+    for R in (12, 17, 22):
+        cfg = workloads.config("cfg2", grid=(n, n, 1), radius=float(R))
+        r = make(cfg)
+        r.init_from_seed(7)
+        mass0 = r.get_macros()["rho"].sum()
+        r.step(5000)
+        m = r.get_macros()
+        rho = m["rho"][0].reshape(n, n)
+        assert abs(rho.sum() - mass0) / mass0 < 1e-11           # mass conservation
+        psi = 1 - np.exp(-rho)
+        p = rho / 3 + (-5.0 / 6) * psi ** 2
+        rin, rout = rho[n // 2, n // 2], rho[0, 0]
+        assert rin > 1.8 and rout < 0.2                          # liquid inside, vapour outside
+        reff = np.sqrt(((rho - rout) / (rin - rout)).sum() / np.pi)
+        res.append((1 / reff, p[n // 2, n // 2] - p[0, 0]))
+        assert np.abs(m["u"]).max() < 0.02                       # spurious currents stay small
+    inv_r, dp = np.array(res).T
+    gamma = dp / inv_r
+    assert (dp > 0).all() and (np.diff(dp) < 0).all()            # larger droplet, smaller jump
+    assert gamma.max() / gamma.min() - 1 < 0.05                  # dp * R constant
+    slope = (inv_r * dp).sum() / (inv_r ** 2).sum()              # line through the origin
+    assert np.abs(dp - slope * inv_r).max() / dp.max() < 0.03
+
+
+# ----------------------------------------------------------------------------------------------
+# two components: EOS Eq. 46 and the critical coupling G_c > 1/(rho1+rho2)...
+# ----------------------------------------------------------------------------------------------
+def test_two_component_flat_interface_pressure_balance():
+    """an asymmetric A-rich / B-rich slab relaxes until P = (rhoA+rhoB)/3 + G12 rhoA rhoB / 3 is equal in both
+    bulks although the ideal part (rhoA+rhoB)/3 differs by several per cent: pins the magnitude of Eq. 13."""
+    nx, ny = 2, 128
+    _, w = lattice_table("D2Q9")
+    y = np.arange(ny)
+    I = 0.5 * (1 + np.tanh((y - 32) / 2.0)) * 0.5 * (1 - np.tanh((y - 96) / 2.0))
+    rA, rB = np.repeat(0.05 + 1.85 * I, nx), np.repeat(1.4 - 1.35 * I, nx)
+    r = RefLBM(nx, ny, 1, "D2Q9", "SC2", precision=64, tau=(1.0, 1.0), psi_kind=1, G=workloads.G12)
+    r.set_populations(np.concatenate([rest_populations(w, rA).ravel(), rest_populations(w, rB).ravel()]))
+    r.step(15000)
+    rho = r.get_macros()["rho"].reshape(2, ny, nx)[:, :, 0]
+    P = (rho[0] + rho[1]) / 3 + 1.2 * rho[0] * rho[1] / 3
+    ideal = (rho[0] + rho[1]) / 3
+    assert abs(P[64] - P[0]) / P[0] < 1e-3
+    assert abs(ideal[64] - ideal[0]) / ideal[0] > 0.03
+    assert rho[0, 64] > 1.2 and rho[1, 0] > 1.0                  # still demixed
+
+
+def test_two_component_demixing_threshold():
+    """psi = rho, rhoA = rhoB = 1: noise grows iff G12 sqrt(rhoA rhoB) > 1 (config 3 is above it; reading R3)"""
+    out = {}
+    for G12 in (0.8, 1.2):
+        cfg = workloads.config("cfg3", grid=(48, 48, 1), G=((0, G12), (G12, 0)))
+        r = make(cfg)
+        r.init_from_seed(3)
+        d0 = np.abs(np.diff(r.get_macros()["rho"], axis=0)).max()
+        r.step(600)
+        out[G12] = np.abs(np.diff(r.get_macros()["rho"], axis=0)).max() / d0
+    assert out[0.8] < 0.5 and out[1.2] > 5.0
+
+
+# ----------------------------------------------------------------------------------------------
+# scalar lattice, Eq. 34-36: diffusion, advection, first-order source
+# ----------------------------------------------------------------------------------------------
+def scalar_setup(lattice, grid, u, Cfield, rhoA=1.0, rhoB=1.0, **kw):
+    """SC2_ADE context with G = 0 (the flow is a uniform fixed point) moving at velocity u; inputs are built from
+    the lattice tables only."""
+    c, w = lattice_table(lattice, 0)
+    cs, ws = lattice_table(lattice, 1)
+    d = 3 if lattice == "D3Q19" else 2
+    cs2g = (1 - ws[0]) / d
+    par = dict(precision=64, tau=(1.0, 1.0), tau_c=0.8, psi_kind=1, G=((0, 0), (0, 0)), k_react=0.0)
+    par.update(kw)
+    r = RefLBM(*grid, lattice, "SC2_ADE", **par)
+    N = r.N
+    u = np.asarray(u, float)
+    cu = c[:, :d] @ u[:d]
+    feq = w * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u[:d] @ u[:d]))
+    fA = np.outer(feq, np.full(N, rhoA))
+    fB = np.outer(feq, np.full(N, rhoB))
+    heq = ws[:, None] * Cfield[None, :] * (1 + (cs[:, :d] @ u[:d])[:, None] / cs2g)
+    r.set_populations(np.concatenate([fA.ravel(), fB.ravel(), heq.ravel()]))
+    return r
+
+
+@pytest.mark.parametrize("lattice,grid,axis", [("D2Q9", (64, 2, 1), 0), ("D2Q9", (2, 64, 1), 1),
+                                               ("D3Q19", (64, 2, 2), 0), ("D3Q19", (2, 64, 2), 1), ("D3Q19", (2, 2, 64), 2)])
+def test_scalar_diffusion_and_advection(lattice, grid, axis):
+    """a sine mode of C decays as exp(-D k^2 t), D = c_sg^2 (tau_c - 1/2) [tau_d = D/c_sg^2 + 1/2 is the paper's
+    (10/3) D + 0.5 for D2Q5, PAPER.md:336] and translates at the fluid velocity u (Eq. 35)."""
+    d = 3 if lattice == "D3Q19" else 2
+    n = 64
+    idx = np.indices(grid[::-1])[2 - axis].ravel().astype(float)  # coordinate along `axis` per cell
+    k = 2 * np.pi / n
+    cs2g = 0.3 if d == 2 else 0.25
+    D = cs2g * (0.8 - 0.5)
+    for speed in (0.0, 0.05):
+        u = np.zeros(3)
+        u[axis] = speed
+        r = scalar_setup(lattice, grid, u, 1.0 + 0.1 * np.sin(k * idx))
+        T = 400
+        r.step(T)
+        m = r.get_macros()
+        C = m["C"]
+        assert np.allclose(m["u"][axis], speed, atol=1e-14)
+        a_s = 2 * ((C - 1) * np.sin(k * idx)).mean()
+        a_c = 2 * ((C - 1) * np.cos(k * idx)).mean()
+        amp = np.hypot(a_s, a_c)
+        # second-order advection correction of the LBGK scheme: D_eff = D - (tau_c - 1/2) u^2
+        d_eff = D - (0.8 - 0.5) * speed ** 2
+        assert abs(amp / (0.1 * np.exp(-d_eff * k * k * T)) - 1) < 3e-3
+        shift = np.arctan2(-a_c, a_s) / k
+        assert abs(shift - speed * T) < 0.02
+        assert abs(C.mean() - 1) < 1e-13                          # k_react = 0 conserves sum C
+
+
+@pytest.mark.parametrize("lattice,grid", [("D2Q9", (5, 4, 1)), ("D3Q19", (4, 3, 5))])
+def test_scalar_first_order_reaction_uniform_state(lattice, grid):
+    """uniform state: C(t) = C0 (1 - k chi)^t exactly, chi = 4 rhoA rhoB / (rhoA + rhoB)^2 (BASELINE.json config 5)"""
+    N = int(np.prod(grid))
+    kr, rA, rB, C0 = 1e-3, 1.5, 0.5, 0.8
+    r = scalar_setup(lattice, grid, (0, 0, 0), np.full(N, C0), rhoA=rA, rhoB=rB, k_react=kr)
+    chi = 4 * rA * rB / (rA + rB) ** 2
+    for T in (1, 10, 300):
+        r.step(T if T == 1 else (9 if T == 10 else 290))
+        C = r.get_macros()["C"]
+        assert np.abs(C / (C0 * (1 - kr * chi) ** T) - 1).max() < 1e-13
+    # a pure component (chi = 0) does not react
+    r = scalar_setup(lattice, grid, (0, 0, 0), np.full(N, C0), rhoA=1.0, rhoB=0.0, k_react=kr)
+    r.step(50)
+    assert np.abs(r.get_macros()["C"] - C0).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# fixed points and symmetry
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("model,lattice,grid", [("BGK", "D2Q9", (5, 4, 1)), ("SC1", "D2Q9", (5, 4, 1)),
+                                                ("SC2_ADE", "D2Q9", (5, 4, 1)), ("SC2_ADE", "D3Q19", (4, 3, 3))])
+def test_uniform_rest_state_is_stationary(model, lattice, grid):
+    r = noise_cfg(model, lattice, grid, noise_amp=0.0, init_kind="REST", k_react=0.0)
+    r.init_from_seed(0)
+    f0 = r.get_populations()
+    r.step(25)
+    assert np.abs(r.get_populations() - f0).max() < 1e-15
+    assert np.abs(r.get_macros()["u"]).max() < 1e-16
+
+
+def rotation_maps(lattice, grid):
+    """90-degree rotation about z: (x, y) -> (-y, x).  Returns the rotated grid, the cell map and the
+    direction permutations of the flow and scalar lattices (built from the tables)."""
+    nx, ny, nz = grid
+    gx, gy = ny, nx
+    cell_map = np.empty(nx * ny * nz, int)
+    for z in range(nz):
+        for y in range(ny):
+            for x in range(nx):
+                xr, yr = (gx - 1 - y), x
+                cell_map[x + nx * (y + ny * z)] = xr + gx * (yr + gy * z)
+    perms = []
+    for kind in (0, 1):
+        c, _ = lattice_table(lattice, kind)
+        lut = {tuple(v): i for i, v in enumerate(c.tolist())}
+        perms.append(np.array([lut[(-v[1], v[0], v[2])] for v in c.tolist()]))
+    return (gx, gy, nz), cell_map, perms
+
+
+@pytest.mark.parametrize("model,lattice,grid", [("SC2_ADE", "D2Q9", (8, 6, 1)), ("SC1", "D2Q9", (7, 5, 1)), ("SC2_ADE", "D3Q19", (6, 4, 5))])
+def test_rotation_equivariance(model, lattice, grid):
+    """rotating the input by 90 degrees (cells and lattice directions) rotates the output: catches any
+    inconsistency between the velocity table, the streaming offsets and the force / equilibrium terms."""
+    a = noise_cfg(model, lattice, grid, k_react=1e-3, force=(0.0, 0.0, 0.0))
+    a.init_from_seed(9)
+    a.step(2)
+    fa, ha = a.split_populations(a.get_populations())
+    g2, cmap, (pf, ph) = rotation_maps(lattice, grid)
+    b = noise_cfg(model, lattice, g2, k_react=1e-3)
+    fb = np.empty_like(fa)
+    fb[:, pf[:, None], cmap[None, :]] = fa
+    parts = [fb.ravel()]
+    if ha is not None:
+        hb = np.empty_like(ha)
+        hb[ph[:, None], cmap[None, :]] = ha
+        parts.append(hb.ravel())
+    b.set_populations(np.concatenate(parts))
+    a.step(20)
+    b.step(20)
+    fa2, ha2 = a.split_populations(a.get_populations())
+    fb2, hb2 = b.split_populations(b.get_populations())
+    assert np.abs(fb2[:, pf[:, None], cmap[None, :]] - fa2).max() < 1e-14
+    if ha2 is not None:
+        assert np.abs(hb2[ph[:, None], cmap[None, :]] - ha2).max() < 1e-14
+    assert np.abs(fa2 - fa).max() > 1e-4                         # the state did evolve
+
+
+def test_streaming_moves_each_population_along_its_velocity():
+    """tau = 1 and u = 0 equilibrium everywhere except one marked population: after one step the excess of f_i
+    sits at x + c_i (Eq. 5); pins the direction table against the streaming offsets."""
+    for lattice, grid in (("D2Q9", (5, 6, 1)), ("D3Q19", (5, 6, 4))):
+        c, w = lattice_table(lattice)
+        nx, ny, nz = grid
+        N = nx * ny * nz
+        for i in range(len(w)):
+            r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(1e9, 1e9))  # omega ~ 0: no relaxation
+            f = rest_populations(w, np.ones(N))
+            x0 = (2, 3, 1 if nz > 1 else 0)
+            cell0 = x0[0] + nx * (x0[1] + ny * x0[2])
+            f[i, cell0] += 0.5
+            r.set_populations(f.ravel())
+            r.step(1)
+            f1, _ = r.split_populations(r.get_populations())
+            x1 = ((x0[0] + c[i, 0]) % nx, (x0[1] + c[i, 1]) % ny, (x0[2] + c[i, 2]) % nz)
+            cell1 = x1[0] + nx * (x1[1] + ny * x1[2])
+            excess = f1[0] - rest_populations(w, np.ones(N))
+            assert abs(excess[i, cell1] - 0.5) < 1e-9
+            excess[i, cell1] = 0
+            assert np.abs(excess).max() < 1e-9
+
+
+def test_bounce_back_reverses_population_at_wall():
+    """halfway bounce-back: a population leaving through a wall is back in the same cell, in the
+    opposite direction, at t + 1; wall-parallel motion and the periodic axes are untouched."""
+    c, w = lattice_table("D3Q19")
+    nx, ny, nz = 4, 3, 4
+    N = nx * ny * nz
+    for i in range(19):
+        r = RefLBM(nx, ny, nz, "D3Q19", "BGK", precision=64, tau=(1e9, 1e9), bc=(0, 0, 1))
+        f = rest_populations(w, np.ones(N))
+        x0 = (1, 1, 0)  # bottom layer
+        cell0 = x0[0] + nx * (x0[1] + ny * x0[2])
+        f[i, cell0] += 0.5
+        r.set_populations(f.ravel())
+        r.step(1)
+        f1, _ = r.split_populations(r.get_populations())
+        excess = f1[0] - rest_populations(w, np.ones(N))
+        if c[i, 2] < 0:
+            opp = [j for j in range(19) if (c[j] == -c[i]).all()][0]
+            assert abs(excess[opp, cell0] - 0.5) < 1e-9
+        else:
+            x1 = ((x0[0] + c[i, 0]) % nx, (x0[1] + c[i, 1]) % ny, x0[2] + c[i, 2])
+            assert abs(excess[i, x1[0] + nx * (x1[1] + ny * x1[2])] - 0.5) < 1e-9
+        assert abs(excess.sum() - 0.5) < 1e-9
+
+
+# ----------------------------------------------------------------------------------------------
+# precision variants and the seeded inputs
+# ----------------------------------------------------------------------------------------------
+def test_fp32_oracle_tracks_fp64_oracle():
+    a = noise_cfg("SC2_ADE", "D3Q19", (8, 8, 8), precision=64, k_react=1e-3)
+    b = noise_cfg("SC2_ADE", "D3Q19", (8, 8, 8), precision=32, k_react=1e-3)
+    for r in (a, b):
+        r.init_from_seed(4)
+        r.step(50)
+    ma, mb = a.get_macros(), b.get_macros()
+    assert mb["rho"].dtype == np.float32
+    for key in ("rho", "C"):
+        assert np.abs(ma[key] - mb[key]).max() / np.abs(ma[key]).max() < 2e-6
+    assert np.abs(ma["u"] - mb["u"]).max() < 1e-6
+
+
+def test_seeded_noise_statistics_and_reproducibility():
+    cfg = workloads.config("cfg3", grid=(64, 64, 1))
+    a, b, c3 = make(cfg), make(cfg), make(cfg)
+    a.init_from_seed(1)
+    b.init_from_seed(1)
+    c3.init_from_seed(2)
+    ra, rb, rc = (r.get_macros()["rho"] for r in (a, b, c3))
+    assert np.array_equal(ra, rb) and not np.array_equal(ra, rc)
+    dev = (ra - 1.0) / 0.01                                          # uniform in [-1, 1)
+    assert dev.min() >= -1 - 1e-12 and dev.max() < 1 + 1e-12
+    assert abs(dev.mean()) < 0.03 and abs(dev.std() - 1 / np.sqrt(3)) < 0.02
+    assert abs(np.corrcoef(ra[0], ra[1])[0, 1]) < 0.05             # components use different streams
+
+
+def test_random_droplets_volume_fraction():
+    cfg = workloads.config("cfg5", grid=(64, 64, 64), rmin=5.0, rmax=10.0)
+    r = make(cfg)
+    r.init_from_seed(12)
+    m = r.get_macros()
+    rhoA, rhoB, Cc = m["rho"][0], m["rho"][1], m["C"]
+    assert abs(rhoA.min() - 0.1) < 1e-6 and abs(rhoA.max() - 1.9) < 1e-6
+    assert np.abs(rhoA + rhoB - 2.0).max() < 1e-6                   # total density 2 everywhere
+    frac = (Cc > 0.5).mean()
+    assert 0.03 < frac < 0.09                                       # about the 5 % requested (overlaps allowed)
+    assert np.abs(Cc - (rhoA - 0.1) / 1.8).max() < 1e-6             # C = 1 inside A, 0 outside
+
+
+def test_errors():
+    with pytest.raises(ValueError):
+        RefLBM(4, 4, 2, "D2Q9", "BGK")                             # 2D lattice with nz != 1
+    with pytest.raises(ValueError):
+        RefLBM(4, 4, 1, "D2Q9", "BGK", tau=(0.5, 1.0))
+    with pytest.raises(ValueError):
+        RefLBM(4, 4, 1, "D2Q9", "SC1", bc=(0, 1, 0))               # Shan-Chen with walls: not implemented
+    r = RefLBM(4, 4, 1, "D2Q9", "BGK")
+    with pytest.raises(RuntimeError):
+        r.step(1)                                                    # step before init
