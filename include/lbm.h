@@ -1,0 +1,144 @@
+/*
+ * include/lbm.h -- C ABI of the B200 (sm_100a) lattice Boltzmann hot path.
+ *
+ * What the library computes: the per-time-step, per-cell collide-and-stream update of the
+ * lattice Boltzmann method as stated in CooLBM (arXiv 2502.12955; citations below are
+ * "PAPER.md:<line>" + equation):
+ *   - LBGK collision with Guo forcing on D2Q9 / D3Q19 populations
+ *         Eq. 3-8, Eq. 15, Eq. 20-23
+ *   - Shan-Chen pseudopotential interaction force, one or two components
+ *         Eq. 10-11, Eq. 13, Eq. 24
+ *   - an advection-diffusion scalar lattice D2Q5 / D3Q7 with a first-order interface reaction
+ *     source, Eq. 34-36; source term and D3Q7: DESIGN.md readings R6, R8
+ *   - periodic boundaries and halfway bounce-back walls
+ * Every step of that path runs in CUDA kernels; there is no CPU fallback.  If no CUDA device
+ * is usable, lbm_create returns NULL and lbm_last_error() says why.
+ *
+ * Conventions
+ *   - 2D <=> lattice LBM_D2Q9 and nz == 1.  Cell index = x + nx*(y + ny*z), x fastest.
+ *   - "ctx precision" R is float (precision 32) or double (precision 64).  All field buffers
+ *     are arrays of R, structure-of-arrays.  N = nx*ny*nz, S = components (1 or 2),
+ *     d = 2 or 3, Q = 9 or 19, Qs = 5 or 7.
+ *   - Unless a function name ends in _host, every buffer pointer is a DEVICE pointer owned by
+ *     the caller and must be valid on the context's stream.  _host functions take HOST
+ *     pointers (pageable or pinned), copy inside the call and synchronise the stream.
+ *   - All kernels are enqueued on the context's stream (lbm_params.stream, a cudaStream_t, or
+ *     the legacy default stream when NULL).  lbm_step and lbm_get_* do not synchronise.
+ *   - Return value: 0 on success, a negative LBM_E* code on error; the message is available
+ *     from lbm_last_error() (thread-local).  No exception crosses this boundary.
+ *   - The context owns only the memory it allocated itself; it never frees lbm_params.workspace.
+ */
+#ifndef LBM_H
+#define LBM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* flow lattice; the scalar lattice is D2Q5 for D2Q9 and D3Q7 for D3Q19.  PAPER.md:217-240 Tables 1-3.
+ * Direction order:
+ *   D3Q19: Table 1 as printed: 0 rest; 1..6 = +x,-x,+y,-y,+z,-z; 7..18 = (+,+,0)(-,-,0)(+,0,+)(-,0,-)
+ *          (0,+,+)(0,-,-)(+,-,0)(-,+,0)(+,0,-)(-,0,+)(0,+,-)(0,-,+); opposite of 2k-1 is 2k.
+ *   D2Q9 : 0 rest; 1 +x; 2 +y; 3 -x; 4 -y; 5 (+,+); 6 (-,+); 7 (-,-); 8 (+,-)   (Table 2, w_4 = 1/9: R1)
+ *   D2Q5 : 0 rest; 1 +x; 2 +y; 3 -x; 4 -y (Table 3).   D3Q7: 0 rest; 1..6 = +x,-x,+y,-y,+z,-z (R6). */
+enum { LBM_D2Q9 = 0, LBM_D3Q19 = 1 };
+
+/* model: BGK single phase; Shan-Chen one component (Eq. 11); Shan-Chen two components (Eq. 13);
+ * two components + scalar lattice with reaction source (Eq. 34-36) */
+enum { LBM_BGK = 0, LBM_SC1 = 1, LBM_SC2 = 2, LBM_SC2_ADE = 3 };
+
+/* initial condition kinds of lbm_init_from_seed */
+enum { LBM_INIT_REST = 0, LBM_INIT_TAYLOR_GREEN = 1, LBM_INIT_DROPLET = 2,
+       LBM_INIT_UNIFORM_NOISE = 3, LBM_INIT_RANDOM_DROPLETS = 4 };
+
+/* error codes */
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE = -4 };
+
+typedef struct lbm_params {
+    uint32_t struct_size;   /* must be sizeof(lbm_params) */
+    int32_t  precision;     /* 32 or 64: storage and arithmetic type of the whole path */
+    double   tau[2];        /* relaxation time of each component, > 0.5; Eq. 15 */
+    double   tau_c;         /* scalar-lattice relaxation time, > 0.5; Eq. 34 */
+    double   G[2][2];       /* Shan-Chen coupling G_{sigma sigma~}; SC1 uses G[0][0]; Eq. 11/13 */
+    int32_t  psi_kind;      /* 0: psi = rho0 (1 - exp(-rho/rho0)), Eq. 10/24 ; 1: psi = rho (R3) */
+    int32_t  forcing;       /* 0: Guo, Eq. 20-23 (the only accepted value) */
+    double   rho0_psi;      /* rho0 of Eq. 10 */
+    double   force[3];      /* constant body-force density; S = 2: split by mass fraction (R5) */
+    int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls on both faces;
+                               walls are accepted for LBM_BGK only */
+    int32_t  init_kind;     /* LBM_INIT_* */
+    double   k_react;       /* k of the source R = -k C 4 rhoA rhoB/(rhoA+rhoB)^2 (R8) */
+    double   w0_scalar;     /* rest weight of the scalar lattice; 0 -> 0.4 (D2Q5) / 0.25 (D3Q7) */
+    double   rho_init[2];   /* REST / TAYLOR_GREEN / UNIFORM_NOISE: density per component */
+    double   c_init;        /* scalar value (REST...) or value inside droplets (DROPLET, RANDOM_DROPLETS) */
+    double   rho_in, rho_out;   /* DROPLET / RANDOM_DROPLETS: component-A density inside / outside */
+    double   radius, width;     /* DROPLET radius; interface width W */
+    double   noise_amp;         /* relative amplitude of the seeded uniform noise */
+    double   u0;                /* TAYLOR_GREEN velocity amplitude */
+    double   rmin, rmax, vol_frac;  /* RANDOM_DROPLETS: radius range and target volume fraction */
+    void*    workspace;     /* DEVICE memory of >= lbm_workspace_bytes() bytes, 256-byte aligned (e.g. from
+                               torch), or NULL: the library allocates (cudaMalloc) and frees it */
+    void*    stream;        /* cudaStream_t, or NULL for the legacy default stream */
+} lbm_params;
+
+typedef struct lbm_ctx lbm_ctx;   /* opaque */
+
+/* Bytes of device workspace a context of this shape needs: the in-place population array
+ * (S*Q + Qs values per cell, ONE copy: AA-pattern streaming), the psi field (S values per cell,
+ * Shan-Chen models only) and padding.  0 on invalid arguments. */
+size_t lbm_workspace_bytes(int nx, int ny, int nz, int lattice, int model, const lbm_params* p);
+
+/* Validate, bind to the current CUDA device, allocate.  NULL on error (see lbm_last_error). */
+lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_params* p);
+
+/* Fill the populations with the equilibrium (Eq. 6) of the seeded initial fields (init_kind),
+ * time level t = 0.  Runs on the device. */
+int lbm_init_from_seed(lbm_ctx* ctx, uint64_t seed);
+
+/* Advance n >= 0 time steps (asynchronous).  One step = steps a1..a8 of DESIGN.md: moments, psi,
+ * Shan-Chen force, barycentric velocity (Eq. 20), BGK + Guo collision (Eq. 15, 22), scalar
+ * lattice + source, in-place streaming (Eq. 5), boundaries.  LBM_ESTATE before init / set. */
+int lbm_step(lbm_ctx* ctx, int n);
+
+/* Macroscopic fields at the current time level into caller-owned DEVICE buffers (NULL = skip):
+ *   rho[sigma][cell] (S*N)   density per component, Eq. 7/18
+ *   u[a][cell]       (d*N)   barycentric velocity incl. F/2, Eq. 20
+ *   phi[cell]        (N)     S = 2: (rhoA-rhoB)/(rhoA+rhoB);  S = 1: psi(rho)
+ *   C[cell]          (N)     scalar concentration, Eq. 36; LBM_EINVAL if the model has no scalar lattice */
+int lbm_get_macros(lbm_ctx* ctx, void* rho, void* u, void* phi, void* C);
+
+/* Total force density per component (Shan-Chen + body), F[sigma][a][cell] (S*d*N), device buffer. */
+int lbm_get_force(lbm_ctx* ctx, void* F);
+
+/* Canonical populations at the current time level, independent of the in-place slot permutation:
+ * f[sigma][i][cell] (S*Q*N) followed by h[i][cell] (Qs*N, scalar models only).  Device buffers.
+ * lbm_set_populations also marks the context initialised and resets the time level parity. */
+size_t lbm_population_count(const lbm_ctx* ctx);
+int lbm_get_populations(lbm_ctx* ctx, void* f);
+int lbm_set_populations(lbm_ctx* ctx, const void* f);
+
+/* End-to-end call with HOST buffers: (optional) upload canonical populations from f_in_host
+ * (NULL = keep the current state), run n steps, compute the macros and copy them to the host
+ * buffers (NULL = skip), then synchronise.  Layouts as in lbm_set_populations / lbm_get_macros. */
+int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
+                 void* rho_host, void* u_host, void* phi_host, void* C_host);
+
+/* number of time steps taken since init / set_populations */
+int64_t lbm_time(const lbm_ctx* ctx);
+
+/* number of kernel launches this context has enqueued so far (for benchmarks) */
+int64_t lbm_launch_count(const lbm_ctx* ctx);
+
+/* Lattice tables as the kernels use them: kind 0 = flow lattice, 1 = scalar lattice (default w0).
+ * c receives Q*3 ints, w receives Q doubles, opp receives Q ints.  Host pointers. */
+int lbm_lattice_table(int lattice, int kind, int* Q, int* c, double* w, int* opp);
+
+void lbm_destroy(lbm_ctx* ctx);            /* NULL-safe; synchronises the stream first */
+const char* lbm_last_error(void);          /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,108 @@
+// Launchers: runtime (model, parity, walls, forced) -> kernel template instance.
+#pragma once
+#include "dispatch.h"
+#include "kernels.cuh"
+
+namespace lbm {
+
+inline unsigned grid_for(int N) { return (unsigned)(((long long)N + BLOCK - 1) / BLOCK); }
+
+template <class R, class L>
+struct Launch {
+    template <int MODEL, int PARITY>
+    static void psi2(const KP<R>& p, cudaStream_t st) {
+        k_psi<R, L, MODEL, PARITY><<<grid_for(p.N), BLOCK, 0, st>>>(p);
+    }
+    static cudaError_t psi(const void* kp, int model, int parity, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+#define LBM_PSI(M) case M: parity ? psi2<M, 1>(p, st) : psi2<M, 0>(p, st); break;
+        switch (model) { LBM_PSI(M_SC1) LBM_PSI(M_SC2) LBM_PSI(M_SC2_ADE) default: return cudaErrorInvalidValue; }
+#undef LBM_PSI
+        return cudaGetLastError();
+    }
+
+    template <int MODEL, bool WALLS, bool FORCED>
+    static void step3(const KP<R>& p, int parity, cudaStream_t st) {
+        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p.N), BLOCK, 0, st>>>(p);
+        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p.N), BLOCK, 0, st>>>(p);
+    }
+    static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        switch (model) {
+        case M_BGK:
+            if (walls) { if (forced) step3<M_BGK, true, true>(p, parity, st); else step3<M_BGK, true, false>(p, parity, st); }
+            else { if (forced) step3<M_BGK, false, true>(p, parity, st); else step3<M_BGK, false, false>(p, parity, st); }
+            break;
+        case M_SC1: step3<M_SC1, false, true>(p, parity, st); break;
+        case M_SC2: step3<M_SC2, false, true>(p, parity, st); break;
+        case M_SC2_ADE: step3<M_SC2_ADE, false, true>(p, parity, st); break;
+        default: return cudaErrorInvalidValue;
+        }
+        return cudaGetLastError();
+    }
+
+    template <int MODEL, bool WALLS>
+    static void macros2(const KP<R>& p, int parity, R* rho, R* u, R* phi, R* C, R* F, cudaStream_t st) {
+        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p.N), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
+        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p.N), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
+    }
+    static cudaError_t macros(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
+                              void* F, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        R *r = (R*)rho, *uu = (R*)u, *ph = (R*)phi, *c = (R*)C, *f = (R*)F;
+        switch (model) {
+        case M_BGK: if (walls) macros2<M_BGK, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_BGK, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC1: macros2<M_SC1, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC2: macros2<M_SC2, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC2_ADE: macros2<M_SC2_ADE, false>(p, parity, r, uu, ph, c, f, st); break;
+        default: return cudaErrorInvalidValue;
+        }
+        return cudaGetLastError();
+    }
+
+    template <class LL, bool TOC>
+    static void permute2(const KP<R>& p, int parity, int walls, R* slots, R* canon, int nl, cudaStream_t st) {
+        const unsigned g = grid_for(p.N);
+        if (parity) {
+            if (walls) k_permute<R, LL, 1, true, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
+            else k_permute<R, LL, 1, false, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
+        } else {
+            k_permute<R, LL, 0, false, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
+        }
+    }
+    static cudaError_t permute(const void* kp, int model, int parity, int walls, void* canon, int to_canonical,
+                               cudaStream_t st) {
+        using LS = typename ScalarOf<L>::type;
+        const KP<R>& p = *(const KP<R>*)kp;
+        const int S = (model == M_SC2 || model == M_SC2_ADE) ? 2 : 1;
+        R* cf = (R*)canon;
+        if (to_canonical) permute2<L, true>(p, parity, walls, p.f, cf, S, st);
+        else permute2<L, false>(p, parity, walls, p.f, cf, S, st);
+        if (model == M_SC2_ADE) {
+            R* ch = cf + (size_t)S * L::Q * (size_t)p.N;
+            if (to_canonical) permute2<LS, true>(p, parity, walls, p.h, ch, 1, st);
+            else permute2<LS, false>(p, parity, walls, p.h, ch, 1, st);
+        }
+        return cudaGetLastError();
+    }
+
+    static cudaError_t init(const void* kp, int model, const InitArgs* ia, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        const unsigned g = grid_for(p.N);
+        switch (model) {
+        case M_BGK: k_init<R, L, M_BGK><<<g, BLOCK, 0, st>>>(p, *ia); break;
+        case M_SC1: k_init<R, L, M_SC1><<<g, BLOCK, 0, st>>>(p, *ia); break;
+        case M_SC2: k_init<R, L, M_SC2><<<g, BLOCK, 0, st>>>(p, *ia); break;
+        case M_SC2_ADE: k_init<R, L, M_SC2_ADE><<<g, BLOCK, 0, st>>>(p, *ia); break;
+        default: return cudaErrorInvalidValue;
+        }
+        return cudaGetLastError();
+    }
+
+    static const Ops* ops() {
+        static const Ops o = {&psi, &step, &macros, &permute, &init};
+        return &o;
+    }
+};
+
+}  // namespace lbm

@@ -1,0 +1,585 @@
+// CUDA kernels of the lattice Boltzmann hot path (sm_100a).  See DESIGN.md for the data layout,
+// the AA-pattern in-place streaming and the arithmetic specification.
+//
+// Layout (structure of arrays, ONE copy of the populations):
+//   f[(sigma*Q + slot)*N + cell], h[slot*N + cell], psi[sigma*N + cell], cell = x + nx*(y + ny*z).
+//
+// AA-pattern in-place streaming: at time level t
+//   t even: f_i(x,t) lives in slot i of cell x;
+//   t odd : f_i(x,t) lives in slot opp(i) of cell x - c_i (periodic wrap), or, if x - c_i lies
+//           beyond a bounce-back wall, in slot i of cell x itself.
+// Call that location P_i(x).  One time step reads f_i from P_i(x), collides, and writes the
+// post-collision f*_{opp(i)} back to the same P_i(x): every thread overwrites exactly the slots it
+// read, slot sets of different cells are disjoint, so a step needs no barrier and no second copy.
+// Eq. 5 and halfway bounce-back are both encoded in P_i.
+//
+// Arithmetic: every floating-point operation is a single IEEE-754 add/sub/mul/div in the context
+// precision R, in the order written (the files are compiled with --fmad=false, default
+// -prec-div=true); DESIGN.md "Arithmetic" lists the expression tree.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "lattice.cuh"
+
+namespace lbm {
+
+enum { M_BGK = 0, M_SC1 = 1, M_SC2 = 2, M_SC2_ADE = 3 };
+enum { I_REST = 0, I_TAYLOR_GREEN = 1, I_DROPLET = 2, I_UNIFORM_NOISE = 3, I_RANDOM_DROPLETS = 4 };
+
+constexpr int BLOCK = 128;
+
+template <class R>
+struct KP {
+    R* f;
+    R* h;
+    R* psi;
+    int nx, ny, nz, N;
+    int bc[3];
+    int psi_kind;
+    R omega[2], cf[2];        // 1/tau, 1 - 1/(2 tau): Eq. 15
+    R omega_c, inv_cs2g;      // 1/tau_c (Eq. 34), 1/c_{s,g}^2 = d/(1-w0) (Eq. 35, R6)
+    R ws0, ws1;               // scalar-lattice weights
+    R G[2][2];
+    R rho0_psi;
+    R force[3];
+    R k_react;
+};
+
+struct InitArgs {
+    int kind;
+    uint64_t seed;
+    double rho_init[2], c_init, rho_in, rho_out, radius, width, noise_amp, u0;
+    const double4* droplets;  // (cx, cy, cz, r), device
+    int n_droplets;
+};
+
+template <int MODEL> struct ModelTraits {
+    static constexpr int S = (MODEL == M_SC2 || MODEL == M_SC2_ADE) ? 2 : 1;
+    static constexpr bool SC = MODEL != M_BGK;
+    static constexpr bool SCALAR = MODEL == M_SC2_ADE;
+};
+
+// ------------------------------------------------------------------------------------------
+// neighbourhood of one cell: signed index offsets to coordinate -1 / 0 / +1 on each axis
+// (periodic wrap folded in) and the wall flags
+// ------------------------------------------------------------------------------------------
+template <int D, bool WALLS>
+struct Nbr {
+    int cell;
+    int dx[3], dy[3], dz[3];
+    bool lo[3], hi[3];
+
+    template <class R>
+    __device__ __forceinline__ Nbr(const KP<R>& p, int cell_) : cell(cell_) {
+        const int nx = p.nx, ny = p.ny;
+        const int x = cell % nx, t = cell / nx;
+        int y, z;
+        if constexpr (D == 3) { y = t % ny; z = t / ny; } else { y = t; z = 0; }
+        dx[0] = (x == 0) ? nx - 1 : -1;          dx[1] = 0; dx[2] = (x == nx - 1) ? -(nx - 1) : 1;
+        dy[0] = ((y == 0) ? ny - 1 : -1) * nx;   dy[1] = 0; dy[2] = ((y == ny - 1) ? -(ny - 1) : 1) * nx;
+        if constexpr (D == 3) {
+            const int nz = p.nz, sxy = nx * ny;
+            dz[0] = ((z == 0) ? nz - 1 : -1) * sxy; dz[1] = 0; dz[2] = ((z == nz - 1) ? -(nz - 1) : 1) * sxy;
+        } else {
+            dz[0] = dz[1] = dz[2] = 0;
+        }
+        if constexpr (WALLS) {
+            lo[0] = p.bc[0] && x == 0; hi[0] = p.bc[0] && x == nx - 1;
+            lo[1] = p.bc[1] && y == 0; hi[1] = p.bc[1] && y == ny - 1;
+            lo[2] = D == 3 && p.bc[2] && z == 0; hi[2] = D == 3 && p.bc[2] && z == p.nz - 1;
+        } else {
+            lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
+        }
+    }
+    // index of the cell at offset (cx,cy,cz), components in {-1,0,1}
+    template <int CX, int CY, int CZ>
+    __device__ __forceinline__ int at() const { return cell + dx[CX + 1] + dy[CY + 1] + dz[CZ + 1]; }
+    // does the offset cross a bounce-back wall?
+    template <int CX, int CY, int CZ>
+    __device__ __forceinline__ bool outside() const {
+        if constexpr (!WALLS) return false;
+        bool o = false;
+        if constexpr (CX < 0) o = o || lo[0];
+        if constexpr (CX > 0) o = o || hi[0];
+        if constexpr (CY < 0) o = o || lo[1];
+        if constexpr (CY > 0) o = o || hi[1];
+        if constexpr (CZ < 0) o = o || lo[2];
+        if constexpr (CZ > 0) o = o || hi[2];
+        return o;
+    }
+};
+
+// element index (relative to the lattice base) of P_I(x): where f_I(x,t) is read and
+// f*_{opp(I)}(x,t) is written
+template <class L, int PARITY, bool WALLS, int I, class NB>
+__device__ __forceinline__ size_t slot_of(const NB& nb, size_t N) {
+    if constexpr (PARITY == 0 || I == 0) {
+        return (size_t)I * N + (size_t)nb.cell;
+    } else {
+        constexpr int CX = -L::c(I, 0), CY = -L::c(I, 1), CZ = -L::c(I, 2);
+        const int src = nb.template at<CX, CY, CZ>();
+        if constexpr (WALLS) {
+            return nb.template outside<CX, CY, CZ>() ? (size_t)I * N + (size_t)nb.cell
+                                                     : (size_t)L::opp(I) * N + (size_t)src;
+        } else {
+            return (size_t)L::opp(I) * N + (size_t)src;
+        }
+    }
+}
+
+// sum_a c_{I,a} v_a in axis order, skipping the zero components (adding +-0 changes nothing)
+template <class L, int I, class R>
+__device__ __forceinline__ R dotc(const R* v) {
+    constexpr int c0 = L::c(I, 0), c1 = L::c(I, 1), c2 = L::c(I, 2);
+    R r = (R)0;
+    if constexpr (c0 != 0) r = c0 > 0 ? v[0] : -v[0];
+    if constexpr (c1 != 0) {
+        if constexpr (c0 == 0) r = c1 > 0 ? v[1] : -v[1];
+        else r = c1 > 0 ? r + v[1] : r - v[1];
+    }
+    if constexpr (L::D == 3 && c2 != 0) {
+        if constexpr (c0 == 0 && c1 == 0) r = c2 > 0 ? v[2] : -v[2];
+        else r = c2 > 0 ? r + v[2] : r - v[2];
+    }
+    return r;
+}
+
+template <class L>
+__host__ __device__ constexpr bool first_nonzero(int i, int a) {
+    for (int k = 0; k < i; ++k)
+        if (L::c(k, a) != 0) return false;
+    return true;
+}
+
+// rho = sum_i f_i, j = sum_i c_i f_i, both in index order: Eq. 7-8 / 18
+template <class L, class R>
+__device__ __forceinline__ void moments(const R* fl, R& rho, R* j) {
+    static_for<0, L::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        if constexpr (i == 0) rho = fl[0]; else rho = rho + fl[i];
+        static_for<0, L::D>([&](auto ac) {
+            constexpr int a = decltype(ac)::value;
+            constexpr int c = L::c(i, a);
+            if constexpr (c != 0) {
+                if constexpr (first_nonzero<L>(i, a)) j[a] = c > 0 ? fl[i] : -fl[i];
+                else j[a] = c > 0 ? j[a] + fl[i] : j[a] - fl[i];
+            }
+        });
+    });
+}
+
+// Eq. 10 / 24 or psi = rho (R3)
+template <class R>
+__device__ __forceinline__ R psi_of(R rho, int kind, R rho0) {
+    if (kind == 1) return rho;
+    return rho0 * ((R)1 - exp(-(rho / rho0)));
+}
+
+template <class L, int PARITY, bool WALLS, class R, class NB>
+__device__ __forceinline__ void load_pops(const R* __restrict__ base, const NB& nb, size_t N, R* fl) {
+    static_for<0, L::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        fl[i] = base[slot_of<L, PARITY, WALLS, i>(nb, N)];
+    });
+}
+// writes fl[opp(i)] (post-collision) to P_i
+template <class L, int PARITY, bool WALLS, class R, class NB>
+__device__ __forceinline__ void store_pops(R* __restrict__ base, const NB& nb, size_t N, const R* fl) {
+    static_for<0, L::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        base[slot_of<L, PARITY, WALLS, i>(nb, N)] = fl[L::opp(i)];
+    });
+}
+
+// Shan-Chen stencil sums acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a}: Eq. 11 / 13
+template <class L, int S, class R, class NB>
+__device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& nb, size_t N, R (*acc)[3]) {
+    static_for<0, S>([&](auto tc) {
+        constexpr int t = decltype(tc)::value;
+        const R* __restrict__ ps = psi + (size_t)t * N;
+        acc[t][0] = acc[t][1] = acc[t][2] = (R)0;
+        static_for<1, L::Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
+            const R wp = (R)L::w(i) * __ldg(ps + nb.template at<CX, CY, CZ>());
+            static_for<0, L::D>([&](auto ac) {
+                constexpr int a = decltype(ac)::value;
+                constexpr int c = L::c(i, a);
+                if constexpr (c != 0) {
+                    if constexpr (first_nonzero<L>(i, a)) acc[t][a] = c > 0 ? wp : -wp;
+                    else acc[t][a] = c > 0 ? acc[t][a] + wp : acc[t][a] - wp;
+                }
+            });
+        });
+    });
+}
+
+// ------------------------------------------------------------------------------------------
+// per-cell state after steps a1-a4 (moments, force, barycentric velocity)
+// ------------------------------------------------------------------------------------------
+template <class R, class L, int MODEL>
+struct CellMacro {
+    static constexpr int S = ModelTraits<MODEL>::S;
+    R rho[S];
+    R F[S][3];
+    R u[3];
+    R inv_rho;
+};
+
+// steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field
+template <class R, class L, int MODEL, bool FORCED, class NB>
+__device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const R (*fl)[L::Q], CellMacro<R, L, MODEL>& m) {
+    constexpr int S = ModelTraits<MODEL>::S, D = L::D;
+    constexpr bool SC = ModelTraits<MODEL>::SC;
+    const size_t N = (size_t)p.N;
+    R j[S][3];
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        j[s][0] = j[s][1] = j[s][2] = (R)0;
+        moments<L>(fl[s], m.rho[s], j[s]);
+    });
+    R rho_t = m.rho[0];
+    if constexpr (S == 2) rho_t = rho_t + m.rho[1];
+    m.inv_rho = (R)1 / rho_t;
+    if constexpr (FORCED) {
+        R acc[S][3];
+        if constexpr (SC) sc_stencil<L, S>(p.psi, nb, N, acc);
+        static_for<0, S>([&](auto sc) {
+            constexpr int s = decltype(sc)::value;
+            R psi_s = (R)0;
+            if constexpr (SC) psi_s = p.psi[(size_t)s * N + nb.cell];
+            static_for<0, D>([&](auto ac) {
+                constexpr int a = decltype(ac)::value;
+                R Fa = (R)0;
+                if constexpr (SC) {
+                    R t = p.G[s][0] * acc[0][a];
+                    if constexpr (S == 2) t = t + p.G[s][1] * acc[1][a];
+                    Fa = -(psi_s * t);
+                }
+                // constant body-force density, split by mass fraction for S = 2 (R5)
+                R Fext;
+                if constexpr (S == 1) Fext = p.force[a]; else Fext = p.force[a] * (m.rho[s] * m.inv_rho);
+                m.F[s][a] = Fa + Fext;
+            });
+        });
+    }
+    // u^b = (1/rho) sum_sigma [ j^sigma + F^sigma / 2 ]: Eq. 20-21
+    static_for<0, D>([&](auto ac) {
+        constexpr int a = decltype(ac)::value;
+        R jt = j[0][a];
+        if constexpr (S == 2) jt = jt + j[1][a];
+        if constexpr (FORCED) {
+            R Ft = m.F[0][a];
+            if constexpr (S == 2) Ft = Ft + m.F[1][a];
+            m.u[a] = (jt + (R)0.5 * Ft) * m.inv_rho;
+        } else {
+            m.u[a] = jt * m.inv_rho;
+        }
+    });
+}
+
+// step a5 for one component: f* = f - (f - f^eq)/tau + (1 - 1/(2 tau)) F_i
+// Eq. 15, Eq. 6 with c_s^2 = 1/3, Eq. 22.
+// Opposite directions share c.u, c.F and the even terms (exactly: negation is exact).
+template <class R, class L, bool FORCED>
+__device__ __forceinline__ void collide(R* fl, R rho_s, const R* u, const R* Fs, R omega, R cfs) {
+    constexpr int D = L::D;
+    R usq = u[0] * u[0];
+    usq = usq + u[1] * u[1];
+    if constexpr (D == 3) usq = usq + u[2] * u[2];
+    const R base = (R)1 - (R)1.5 * usq;
+    R uF = (R)0;
+    if constexpr (FORCED) {
+        uF = u[0] * Fs[0];
+        uF = uF + u[1] * Fs[1];
+        if constexpr (D == 3) uF = uF + u[2] * Fs[2];
+    }
+    const R W[3] = {(R)L::w(0), (R)L::w(1), (R)L::w(L::Q - 1)};
+    const R wr[3] = {W[0] * rho_s, W[1] * rho_s, W[2] * rho_s};
+    {   // rest population: c = 0
+        const R fe = wr[0] * base;
+        R fs = fl[0] - omega * (fl[0] - fe);
+        if constexpr (FORCED) fs = fs + cfs * (W[0] * ((R)3 * (-uF)));
+        fl[0] = fs;
+    }
+    static_for<1, L::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int o = L::opp(i);
+        if constexpr (i < o) {
+            constexpr int k = L::wclass(i);
+            const R cu = dotc<L, i>(u);
+            const R t3 = (R)3 * cu;
+            const R q = ((R)4.5 * cu) * cu;
+            const R fe_i = wr[k] * ((base + t3) + q);
+            const R fe_o = wr[k] * ((base - t3) + q);
+            R fs_i = fl[i] - omega * (fl[i] - fe_i);
+            R fs_o = fl[o] - omega * (fl[o] - fe_o);
+            if constexpr (FORCED) {
+                const R cF = dotc<L, i>(Fs);
+                const R g = ((R)9 * cu) * cF;
+                const R Fi_i = W[k] * ((R)3 * (cF - uF) + g);
+                const R Fi_o = W[k] * ((R)3 * ((-cF) - uF) + g);
+                fs_i = fs_i + cfs * Fi_i;
+                fs_o = fs_o + cfs * Fi_o;
+            }
+            fl[i] = fs_i;
+            fl[o] = fs_o;
+        }
+    });
+}
+
+// step a6: scalar lattice, Eq. 34-36 + source w_i R, R = -k C 4 rhoA rhoB/(rhoA+rhoB)^2 (R8)
+template <class R, class LS>
+__device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB, R inv_rho, const R* u) {
+    R C = hl[0];
+    static_for<1, LS::Q>([&](auto ic) { C = C + hl[decltype(ic)::value]; });
+    const R chi = ((R)4 * (rA * inv_rho)) * (rB * inv_rho);
+    const R Rsrc = -((p.k_react * C) * chi);
+    const R wC0 = p.ws0 * C, wC1 = p.ws1 * C;
+    const R s0 = p.ws0 * Rsrc, s1 = p.ws1 * Rsrc;
+    hl[0] = (hl[0] - p.omega_c * (hl[0] - wC0)) + s0;
+    static_for<1, LS::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int o = LS::opp(i);
+        if constexpr (i < o) {
+            const R m = p.inv_cs2g * dotc<LS, i>(u);
+            const R he_i = wC1 * ((R)1 + m);
+            const R he_o = wC1 * ((R)1 - m);
+            hl[i] = (hl[i] - p.omega_c * (hl[i] - he_i)) + s1;
+            hl[o] = (hl[o] - p.omega_c * (hl[o] - he_o)) + s1;
+        }
+    });
+}
+
+// ------------------------------------------------------------------------------------------
+// psi pass (step a2): rho^sigma from the populations at the current parity, psi^sigma to HBM
+// ------------------------------------------------------------------------------------------
+template <class R, class L, int MODEL, int PARITY>
+__global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
+    constexpr int S = ModelTraits<MODEL>::S, Q = L::Q;
+    const int cell = blockIdx.x * BLOCK + threadIdx.x;
+    if (cell >= p.N) return;
+    const size_t N = (size_t)p.N;
+    const Nbr<L::D, false> nb(p, cell);
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        R fl[Q];
+        load_pops<L, PARITY, false>(p.f + (size_t)s * Q * N, nb, N, fl);
+        R rho, j[3];
+        moments<L>(fl, rho, j);
+        p.psi[(size_t)s * N + cell] = psi_of(rho, p.psi_kind, p.rho0_psi);
+    });
+}
+
+// ------------------------------------------------------------------------------------------
+// fused step (a1, a3-a8): one thread per cell
+// ------------------------------------------------------------------------------------------
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED>
+__global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p) {
+    using MT = ModelTraits<MODEL>;
+    using LS = typename ScalarOf<L>::type;
+    constexpr int S = MT::S, Q = L::Q;
+    const int cell = blockIdx.x * BLOCK + threadIdx.x;
+    if (cell >= p.N) return;
+    const size_t N = (size_t)p.N;
+    const Nbr<L::D, WALLS> nb(p, cell);
+
+    R fl[S][Q];
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
+    });
+    R hl[LS::Q];
+    if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+
+    CellMacro<R, L, MODEL> m;
+    cell_macros<R, L, MODEL, FORCED>(p, nb, fl, m);
+
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+        store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
+    });
+    if constexpr (MT::SCALAR) {
+        collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
+        store_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// macros out (step a9) and force diagnostic; psi must be current
+// ------------------------------------------------------------------------------------------
+template <class R, class L, int MODEL, int PARITY, bool WALLS>
+__global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> p, R* __restrict__ rho_o,
+                                                  R* __restrict__ u_o, R* __restrict__ phi_o, R* __restrict__ C_o,
+                                                  R* __restrict__ F_o) {
+    using MT = ModelTraits<MODEL>;
+    using LS = typename ScalarOf<L>::type;
+    constexpr int S = MT::S, Q = L::Q, D = L::D;
+    const int cell = blockIdx.x * BLOCK + threadIdx.x;
+    if (cell >= p.N) return;
+    const size_t N = (size_t)p.N;
+    const Nbr<D, WALLS> nb(p, cell);
+    R fl[S][Q];
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
+    });
+    CellMacro<R, L, MODEL> m;
+    cell_macros<R, L, MODEL, true>(p, nb, fl, m);
+    if (rho_o) static_for<0, S>([&](auto sc) { rho_o[(size_t)decltype(sc)::value * N + cell] = m.rho[decltype(sc)::value]; });
+    if (u_o) static_for<0, D>([&](auto ac) { u_o[(size_t)decltype(ac)::value * N + cell] = m.u[decltype(ac)::value]; });
+    if (phi_o) {
+        if constexpr (S == 2) phi_o[cell] = (m.rho[0] - m.rho[1]) * m.inv_rho;
+        else if constexpr (MT::SC) phi_o[cell] = p.psi[cell];
+        else phi_o[cell] = psi_of(m.rho[0], p.psi_kind, p.rho0_psi);
+    }
+    if constexpr (MT::SCALAR) {
+        if (C_o) {
+            R hl[LS::Q];
+            load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+            R C = hl[0];
+            static_for<1, LS::Q>([&](auto ic) { C = C + hl[decltype(ic)::value]; });
+            C_o[cell] = C;
+        }
+    }
+    if (F_o)
+        static_for<0, S>([&](auto sc) {
+            constexpr int s = decltype(sc)::value;
+            static_for<0, D>([&](auto ac) {
+                constexpr int a = decltype(ac)::value;
+                F_o[((size_t)s * D + a) * N + cell] = m.F[s][a];
+            });
+        });
+}
+
+// canonical populations f_i(x,t) out of the slot array at the current parity (and back)
+template <class R, class L, int PARITY, bool WALLS, bool TO_CANONICAL>
+__global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R> p, R* __restrict__ slots,
+                                                   R* __restrict__ canon, int n_lattices) {
+    const int cell = blockIdx.x * BLOCK + threadIdx.x;
+    if (cell >= p.N) return;
+    const size_t N = (size_t)p.N;
+    const Nbr<L::D, WALLS> nb(p, cell);
+    for (int s = 0; s < n_lattices; ++s) {
+        R* sb = slots + (size_t)s * L::Q * N;
+        R* cb = canon + (size_t)s * L::Q * N;
+        static_for<0, L::Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const size_t P = slot_of<L, PARITY, WALLS, i>(nb, N);
+            if constexpr (TO_CANONICAL) cb[(size_t)i * N + cell] = sb[P];
+            else sb[P] = cb[(size_t)i * N + cell];
+        });
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// seeded initial condition: macroscopic fields in double, then
+// equilibrium populations (Eq. 6) in R, written at even parity
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {   // splitmix64 finaliser
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ double uniform01(uint64_t seed, uint64_t index) {
+    const uint64_t hsh = mix64(seed + 0x9E3779B97F4A7C15ULL * (index + 1ULL));
+    return (double)(hsh >> 11) * (1.0 / 9007199254740992.0);
+}
+__device__ __forceinline__ double min_image(double a, double b, int n, int bc) {
+    double dd = fabs(a - b);
+    if (bc == 0 && (double)n - dd < dd) dd = (double)n - dd;
+    return dd;
+}
+
+template <class R, class L, int MODEL>
+__global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p, const __grid_constant__ InitArgs ia) {
+    using MT = ModelTraits<MODEL>;
+    using LS = typename ScalarOf<L>::type;
+    constexpr int S = MT::S, Q = L::Q, D = L::D;
+    const int cell = blockIdx.x * BLOCK + threadIdx.x;
+    if (cell >= p.N) return;
+    const size_t N = (size_t)p.N;
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const int x = cell % nx, t = cell / nx, y = t % ny, z = t / ny;
+    const double PI = 3.14159265358979323846;
+    double r0[2] = {ia.rho_init[0], ia.rho_init[1]};
+    double u0[3] = {0.0, 0.0, 0.0};
+    double c0 = ia.c_init;
+    if (ia.kind == I_TAYLOR_GREEN) {
+        if constexpr (D == 2) {
+            // planar Taylor-Green vortex (R19), the 2D analogue of Eq. 45
+            const double kx = 2.0 * PI / (double)nx, ky = 2.0 * PI / (double)ny;
+            const double A = ia.u0, B = ia.u0 * (kx / ky);
+            u0[0] = -A * cos(kx * x) * sin(ky * y);
+            u0[1] = B * sin(kx * x) * cos(ky * y);
+            r0[0] = ia.rho_init[0] * (1.0 - 0.75 * (A * A * cos(2.0 * kx * x) + B * B * cos(2.0 * ky * y)));
+        } else {
+            // Eq. 45a-c; pressure: textbook form (R21); rho = rho0 + 3 (P - P0)
+            const double kx = 2.0 * PI / (double)nx, ky = 2.0 * PI / (double)ny, kz = 2.0 * PI / (double)nz;
+            u0[0] = ia.u0 * cos(kx * x) * sin(ky * y) * sin(kz * z);
+            u0[1] = -ia.u0 * sin(kx * x) * cos(ky * y) * sin(kz * z);
+            u0[2] = 0.0;
+            r0[0] = ia.rho_init[0] * (1.0 + 3.0 * (ia.u0 * ia.u0 / 16.0) * (cos(2.0 * kz * z) + 2.0) *
+                                                (cos(2.0 * kx * x) + cos(2.0 * ky * y)));
+        }
+    } else if (ia.kind == I_DROPLET) {
+        // centred droplet with a tanh profile of width W (R17), then seeded noise (R16)
+        const double ddx = min_image((double)x, 0.5 * (nx - 1), nx, p.bc[0]);
+        const double ddy = min_image((double)y, 0.5 * (ny - 1), ny, p.bc[1]);
+        const double ddz = (D == 3) ? min_image((double)z, 0.5 * (nz - 1), nz, p.bc[2]) : 0.0;
+        const double dist = sqrt(ddx * ddx + ddy * ddy + ddz * ddz);
+        const double th = tanh(2.0 * (dist - ia.radius) / ia.width);
+        const double mean = 0.5 * (ia.rho_in + ia.rho_out), half = 0.5 * (ia.rho_in - ia.rho_out);
+        r0[0] = mean - half * th;
+        r0[1] = mean + half * th;
+        c0 = ia.c_init * (0.5 * (1.0 - th));
+        for (int s = 0; s < S; ++s)
+            r0[s] = r0[s] * (1.0 + ia.noise_amp * (2.0 * uniform01(ia.seed, (uint64_t)cell + (uint64_t)N * s) - 1.0));
+    } else if (ia.kind == I_UNIFORM_NOISE) {
+        for (int s = 0; s < S; ++s)
+            r0[s] = ia.rho_init[s] * (1.0 + ia.noise_amp * (2.0 * uniform01(ia.seed, (uint64_t)cell + (uint64_t)N * s) - 1.0));
+    } else if (ia.kind == I_RANDOM_DROPLETS) {
+        // indicator I = max_k prof((dist_k - r_k)/W), prof = cubic smoothstep (R18)
+        double I = 0.0;
+        for (int k = 0; k < ia.n_droplets; ++k) {
+            const double4 dr = ia.droplets[k];
+            const double ddx = min_image((double)x, dr.x, nx, p.bc[0]);
+            const double ddy = min_image((double)y, dr.y, ny, p.bc[1]);
+            const double ddz = (D == 3) ? min_image((double)z, dr.z, nz, p.bc[2]) : 0.0;
+            const double s = (sqrt(ddx * ddx + ddy * ddy + ddz * ddz) - dr.w) / ia.width;
+            const double v = (s <= -1.0) ? 1.0 : (s >= 1.0 ? 0.0 : (0.5 - 0.75 * s) + (0.25 * s) * (s * s));
+            if (v > I) I = v;
+        }
+        r0[0] = ia.rho_out + (ia.rho_in - ia.rho_out) * I;
+        r0[1] = ia.rho_in - (ia.rho_in - ia.rho_out) * I;
+        c0 = ia.c_init * I;
+    }
+    // populations = equilibrium at (rho, u), no non-equilibrium part (R10)
+    const R u[3] = {(R)u0[0], (R)u0[1], (R)u0[2]};
+    R usq = u[0] * u[0];
+    usq = usq + u[1] * u[1];
+    if constexpr (D == 3) usq = usq + u[2] * u[2];
+    const R base = (R)1 - (R)1.5 * usq;
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        const R rho_s = (R)r0[s];
+        R* fb = p.f + (size_t)s * Q * N;
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const R cu = dotc<L, i>(u);
+            fb[(size_t)i * N + cell] = ((R)L::w(i) * rho_s) * ((base + (R)3 * cu) + ((R)4.5 * cu) * cu);
+        });
+    });
+    if constexpr (MT::SCALAR) {
+        static_for<0, LS::Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const R cu = dotc<LS, i>(u);
+            const R wsi = i == 0 ? p.ws0 : p.ws1;
+            p.h[(size_t)i * N + cell] = (wsi * (R)c0) * ((R)1 + p.inv_cs2g * cu);
+        });
+    }
+}
+
+}  // namespace lbm

@@ -1,0 +1,417 @@
+// C ABI of the B200 lattice Boltzmann library (include/lbm.h): context, validation, launch logic.
+// All compute runs in the kernels of kernels.cuh; there is no CPU path.
+#include "../../include/lbm.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "dispatch.h"
+#include "kernels.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return LBM_ECUDA;
+}
+#define CK(call)                                              \
+    do {                                                      \
+        cudaError_t e_ = (call);                              \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Shape {
+    int S, Q, Qs, d;
+    bool sc, scalar;
+    size_t N, B;
+    size_t f_bytes, h_bytes, psi_bytes, total;
+};
+
+// returns empty string if valid
+std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_params* p, Shape* sh) {
+    if (!p) return "params is NULL";
+    if (p->struct_size != sizeof(lbm_params)) return "params.struct_size != sizeof(lbm_params)";
+    if (nx < 1 || ny < 1 || nz < 1) return "grid extents must be >= 1";
+    if (lattice != LBM_D2Q9 && lattice != LBM_D3Q19) return "unknown lattice";
+    if (lattice == LBM_D2Q9 && nz != 1) return "D2Q9 needs nz == 1";
+    if (model < LBM_BGK || model > LBM_SC2_ADE) return "unknown model";
+    if (p->precision != 32 && p->precision != 64) return "precision must be 32 or 64";
+    if (p->forcing != 0) return "only Guo forcing (forcing = 0) is implemented";
+    if (p->psi_kind != 0 && p->psi_kind != 1) return "psi_kind must be 0 or 1";
+    if ((double)nx * (double)ny * (double)nz > 2147483647.0) return "grid has more than 2^31-1 cells";
+    const int S = (model == LBM_SC2 || model == LBM_SC2_ADE) ? 2 : 1;
+    for (int s = 0; s < S; ++s)
+        if (!(p->tau[s] > 0.5)) return "tau must exceed 0.5";
+    if (model == LBM_SC2_ADE && !(p->tau_c > 0.5)) return "tau_c must exceed 0.5";
+    for (int a = 0; a < 3; ++a) {
+        if (p->bc[a] != 0 && p->bc[a] != 1) return "bc must be 0 (periodic) or 1 (bounce-back walls)";
+        if (p->bc[a] == 1 && model != LBM_BGK) return "Shan-Chen models with walls are not implemented";
+    }
+    if (lattice == LBM_D2Q9 && p->bc[2] != 0) return "2D: bc[2] must be 0";
+    if (model != LBM_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) return "rho0_psi must be > 0";
+    if (p->w0_scalar < 0.0 || p->w0_scalar >= 1.0) return "w0_scalar must lie in [0, 1)";
+    if (p->init_kind < LBM_INIT_REST || p->init_kind > LBM_INIT_RANDOM_DROPLETS) return "unknown init_kind";
+    if (sh) {
+        sh->S = S;
+        sh->d = lattice == LBM_D3Q19 ? 3 : 2;
+        sh->Q = lattice == LBM_D3Q19 ? 19 : 9;
+        sh->Qs = lattice == LBM_D3Q19 ? 7 : 5;
+        sh->sc = model != LBM_BGK;
+        sh->scalar = model == LBM_SC2_ADE;
+        sh->N = (size_t)nx * ny * nz;
+        sh->B = p->precision == 64 ? 8 : 4;
+        sh->f_bytes = align_up((size_t)S * sh->Q * sh->N * sh->B, 256);
+        sh->h_bytes = sh->scalar ? align_up((size_t)sh->Qs * sh->N * sh->B, 256) : 0;
+        sh->psi_bytes = sh->sc ? align_up((size_t)S * sh->N * sh->B, 256) : 0;
+        sh->total = sh->f_bytes + sh->h_bytes + sh->psi_bytes;
+    }
+    return "";
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+struct lbm_ctx {
+    int nx, ny, nz, lattice, model;
+    lbm_params p;
+    Shape sh;
+    int device;
+    cudaStream_t stream;
+    char* ws;
+    bool owns_ws;
+    void *f, *h, *psi;
+    const lbm::Ops* ops;
+    lbm::KP<double> kp64;
+    lbm::KP<float> kp32;
+    bool walls, forced;
+    bool inited;
+    int64_t t;
+    int64_t launches;
+    double4* droplets_dev;
+    void* scratch;        // device staging for lbm_run_host outputs
+    size_t scratch_bytes;
+
+    const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
+};
+
+namespace {
+
+template <class R>
+void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
+    const lbm_params& p = c->p;
+    k.f = (R*)c->f; k.h = (R*)c->h; k.psi = (R*)c->psi;
+    k.nx = c->nx; k.ny = c->ny; k.nz = c->nz; k.N = (int)c->sh.N;
+    for (int a = 0; a < 3; ++a) { k.bc[a] = p.bc[a]; k.force[a] = (R)p.force[a]; }
+    k.psi_kind = p.psi_kind;
+    // constants are formed in double and rounded once to R
+    for (int s = 0; s < 2; ++s) {
+        k.omega[s] = (R)(1.0 / p.tau[s]);
+        k.cf[s] = (R)(1.0 - 0.5 / p.tau[s]);
+        for (int t = 0; t < 2; ++t) k.G[s][t] = (R)p.G[s][t];
+    }
+    const double w0s = p.w0_scalar > 0.0 ? p.w0_scalar : (c->lattice == LBM_D3Q19 ? 0.25 : 0.4);
+    k.omega_c = (R)(1.0 / p.tau_c);
+    k.inv_cs2g = (R)((double)c->sh.d / (1.0 - w0s));
+    k.ws0 = (R)w0s;
+    k.ws1 = (R)((1.0 - w0s) / (double)(c->sh.Qs - 1));
+    k.rho0_psi = (R)p.rho0_psi;
+    k.k_react = (R)p.k_react;
+}
+
+// host copy of the counter-based generator (integer arithmetic, bit-identical to the device one)
+uint64_t h_mix64(uint64_t z) {
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+double h_uniform01(uint64_t seed, uint64_t index) {
+    return (double)(h_mix64(seed + 0x9E3779B97F4A7C15ULL * (index + 1ULL)) >> 11) * (1.0 / 9007199254740992.0);
+}
+
+// RANDOM_DROPLETS (R18): sequential draws (cx, cy, cz, r) from stream 2 until the volume fraction is reached
+std::vector<double4> droplet_list(const lbm_ctx* c, uint64_t seed) {
+    std::vector<double4> v;
+    const double PI = 3.14159265358979323846;
+    const double N = (double)c->sh.N;
+    const double target = c->p.vol_frac * N;
+    double vol = 0.0;
+    const uint64_t base = 2ULL * (uint64_t)c->sh.N;
+    for (uint64_t k = 0; vol < target && k < 100000; ++k) {
+        double4 dr;
+        dr.x = (double)c->nx * h_uniform01(seed, base + 4 * k + 0);
+        dr.y = (double)c->ny * h_uniform01(seed, base + 4 * k + 1);
+        dr.z = (c->sh.d == 3) ? (double)c->nz * h_uniform01(seed, base + 4 * k + 2) : 0.0;
+        dr.w = c->p.rmin + (c->p.rmax - c->p.rmin) * h_uniform01(seed, base + 4 * k + 3);
+        vol += (c->sh.d == 3) ? (4.0 / 3.0) * PI * dr.w * dr.w * dr.w : PI * dr.w * dr.w;
+        v.push_back(dr);
+    }
+    return v;
+}
+
+int run_psi(lbm_ctx* c) {
+    CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->stream));
+    c->launches++;
+    return 0;
+}
+
+int ensure_scratch(lbm_ctx* c, size_t bytes) {
+    if (c->scratch_bytes >= bytes) return 0;
+    if (c->scratch) { cudaFree(c->scratch); c->scratch = nullptr; c->scratch_bytes = 0; }
+    cudaError_t e = cudaMalloc(&c->scratch, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(LBM_ENOMEM, "cudaMalloc of the host-transfer staging buffer failed"); }
+    c->scratch_bytes = bytes;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lbm_last_error(void) { return g_err.c_str(); }
+
+size_t lbm_workspace_bytes(int nx, int ny, int nz, int lattice, int model, const lbm_params* p) {
+    Shape sh;
+    std::string e = validate(nx, ny, nz, lattice, model, p, &sh);
+    if (!e.empty()) { g_err = e; return 0; }
+    return sh.total;
+}
+
+lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_params* p) {
+    Shape sh;
+    std::string e = validate(nx, ny, nz, lattice, model, p, &sh);
+    if (!e.empty()) { g_err = "lbm_create: " + e; return nullptr; }
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        g_err = std::string("lbm_create: no usable CUDA device (") + (ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0") +
+                "); this library has no CPU path";
+        return nullptr;
+    }
+    lbm_ctx* c = new (std::nothrow) lbm_ctx();
+    if (!c) { g_err = "lbm_create: out of host memory"; return nullptr; }
+    c->nx = nx; c->ny = ny; c->nz = nz; c->lattice = lattice; c->model = model;
+    c->p = *p; c->sh = sh;
+    c->stream = (cudaStream_t)p->stream;
+    c->inited = false; c->t = 0; c->launches = 0;
+    c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
+    if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
+    if (p->workspace) {
+        if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
+        c->ws = (char*)p->workspace; c->owns_ws = false;
+    } else {
+        void* w = nullptr;
+        ce = cudaMalloc(&w, sh.total);
+        if (ce != cudaSuccess) {
+            cudaGetLastError();
+            g_err = std::string("lbm_create: cudaMalloc of the workspace failed: ") + cudaGetErrorString(ce);
+            delete c;
+            return nullptr;
+        }
+        c->ws = (char*)w; c->owns_ws = true;
+    }
+    c->f = c->ws;
+    c->h = sh.scalar ? c->ws + sh.f_bytes : nullptr;
+    c->psi = sh.sc ? c->ws + sh.f_bytes + sh.h_bytes : nullptr;
+    c->walls = p->bc[0] || p->bc[1] || p->bc[2];
+    c->forced = sh.sc || p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0;
+    if (p->precision == 64) c->ops = lattice == LBM_D3Q19 ? lbm::ops_f64_d3q19() : lbm::ops_f64_d2q9();
+    else c->ops = lattice == LBM_D3Q19 ? lbm::ops_f32_d3q19() : lbm::ops_f32_d2q9();
+    fill_kp(c->kp64, c);
+    fill_kp(c->kp32, c);
+    return c;
+}
+
+void lbm_destroy(lbm_ctx* c) {
+    if (!c) return;
+    DeviceGuard g(c->device);
+    cudaStreamSynchronize(c->stream);
+    if (c->droplets_dev) cudaFree(c->droplets_dev);
+    if (c->scratch) cudaFree(c->scratch);
+    if (c->owns_ws && c->ws) cudaFree(c->ws);
+    cudaGetLastError();
+    delete c;
+}
+
+int lbm_init_from_seed(lbm_ctx* c, uint64_t seed) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    DeviceGuard g(c->device);
+    lbm::InitArgs ia;
+    std::memset(&ia, 0, sizeof(ia));
+    ia.kind = c->p.init_kind; ia.seed = seed;
+    ia.rho_init[0] = c->p.rho_init[0]; ia.rho_init[1] = c->p.rho_init[1];
+    ia.c_init = c->p.c_init; ia.rho_in = c->p.rho_in; ia.rho_out = c->p.rho_out;
+    ia.radius = c->p.radius; ia.width = c->p.width; ia.noise_amp = c->p.noise_amp; ia.u0 = c->p.u0;
+    ia.droplets = nullptr; ia.n_droplets = 0;
+    if (c->p.init_kind == LBM_INIT_RANDOM_DROPLETS) {
+        std::vector<double4> v = droplet_list(c, seed);
+        if (c->droplets_dev) { cudaStreamSynchronize(c->stream); cudaFree(c->droplets_dev); c->droplets_dev = nullptr; }
+        if (!v.empty()) {
+            CK(cudaMalloc((void**)&c->droplets_dev, v.size() * sizeof(double4)));
+            CK(cudaMemcpyAsync(c->droplets_dev, v.data(), v.size() * sizeof(double4), cudaMemcpyHostToDevice, c->stream));
+            CK(cudaStreamSynchronize(c->stream));   // v goes out of scope
+        }
+        ia.droplets = c->droplets_dev; ia.n_droplets = (int)v.size();
+    }
+    CK(c->ops->init(c->kp(), c->model, &ia, c->stream));
+    c->launches++;
+    c->inited = true;
+    c->t = 0;
+    return 0;
+}
+
+int lbm_step(lbm_ctx* c, int n) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (!c->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init_from_seed / lbm_set_populations");
+    if (n < 0) return fail(LBM_EINVAL, "n < 0");
+    DeviceGuard g(c->device);
+    for (int k = 0; k < n; ++k) {
+        const int parity = (int)(c->t & 1);
+        if (c->sh.sc) {   // a2: psi of every cell at this time level (full-field barrier, R9)
+            CK(c->ops->psi(c->kp(), c->model, parity, c->stream));
+            c->launches++;
+        }
+        CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, c->stream));
+        c->launches++;
+        c->t++;
+    }
+    return 0;
+}
+
+int lbm_get_macros(lbm_ctx* c, void* rho, void* u, void* phi, void* C) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (!c->inited) return fail(LBM_ESTATE, "lbm_get_macros before init");
+    if (C && !c->sh.scalar) return fail(LBM_EINVAL, "model has no scalar lattice");
+    DeviceGuard g(c->device);
+    if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
+    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->walls, rho, u, phi, C, nullptr, c->stream));
+    c->launches++;
+    return 0;
+}
+
+int lbm_get_force(lbm_ctx* c, void* F) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (!c->inited) return fail(LBM_ESTATE, "lbm_get_force before init");
+    if (!F) return fail(LBM_EINVAL, "F is NULL");
+    DeviceGuard g(c->device);
+    if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
+    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->walls, nullptr, nullptr, nullptr, nullptr, F, c->stream));
+    c->launches++;
+    return 0;
+}
+
+size_t lbm_population_count(const lbm_ctx* c) {
+    if (!c) return 0;
+    return (size_t)c->sh.S * c->sh.Q * c->sh.N + (c->sh.scalar ? (size_t)c->sh.Qs * c->sh.N : 0);
+}
+
+int lbm_get_populations(lbm_ctx* c, void* f) {
+    if (!c || !f) return fail(LBM_EINVAL, "NULL argument");
+    if (!c->inited) return fail(LBM_ESTATE, "lbm_get_populations before init");
+    DeviceGuard g(c->device);
+    const size_t nf = (size_t)c->sh.S * c->sh.Q * c->sh.N * c->sh.B, nh = (size_t)c->sh.Qs * c->sh.N * c->sh.B;
+    if ((c->t & 1) == 0) {
+        CK(cudaMemcpyAsync(f, c->f, nf, cudaMemcpyDeviceToDevice, c->stream));
+        if (c->sh.scalar) CK(cudaMemcpyAsync((char*)f + nf, c->h, nh, cudaMemcpyDeviceToDevice, c->stream));
+    } else {
+        CK(c->ops->permute(c->kp(), c->model, 1, c->walls, f, 1, c->stream));
+        c->launches += c->sh.scalar ? 2 : 1;
+    }
+    return 0;
+}
+
+int lbm_set_populations(lbm_ctx* c, const void* f) {
+    if (!c || !f) return fail(LBM_EINVAL, "NULL argument");
+    DeviceGuard g(c->device);
+    const size_t nf = (size_t)c->sh.S * c->sh.Q * c->sh.N * c->sh.B, nh = (size_t)c->sh.Qs * c->sh.N * c->sh.B;
+    CK(cudaMemcpyAsync(c->f, f, nf, cudaMemcpyDeviceToDevice, c->stream));
+    if (c->sh.scalar) CK(cudaMemcpyAsync(c->h, (const char*)f + nf, nh, cudaMemcpyDeviceToDevice, c->stream));
+    c->inited = true;
+    c->t = 0;
+    return 0;
+}
+
+int lbm_run_host(lbm_ctx* c, const void* f_in_host, int n, void* rho_h, void* u_h, void* phi_h, void* C_h) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (C_h && !c->sh.scalar) return fail(LBM_EINVAL, "model has no scalar lattice");
+    if (n < 0) return fail(LBM_EINVAL, "n < 0");
+    DeviceGuard g(c->device);
+    const Shape& sh = c->sh;
+    if (f_in_host) {
+        const size_t nf = (size_t)sh.S * sh.Q * sh.N * sh.B, nh = (size_t)sh.Qs * sh.N * sh.B;
+        CK(cudaMemcpyAsync(c->f, f_in_host, nf, cudaMemcpyHostToDevice, c->stream));
+        if (sh.scalar) CK(cudaMemcpyAsync(c->h, (const char*)f_in_host + nf, nh, cudaMemcpyHostToDevice, c->stream));
+        c->inited = true;
+        c->t = 0;
+    }
+    if (!c->inited) return fail(LBM_ESTATE, "lbm_run_host without populations");
+    int rc = lbm_step(c, n);
+    if (rc) return rc;
+    if (rho_h || u_h || phi_h || C_h) {
+        const size_t fb = sh.N * sh.B;
+        const size_t need = (size_t)(sh.S + sh.d + 2) * fb;
+        rc = ensure_scratch(c, need);
+        if (rc) return rc;
+        char* s = (char*)c->scratch;
+        void* rho_d = rho_h ? s : nullptr;
+        void* u_d = u_h ? s + (size_t)sh.S * fb : nullptr;
+        void* phi_d = phi_h ? s + (size_t)(sh.S + sh.d) * fb : nullptr;
+        void* C_d = C_h ? s + (size_t)(sh.S + sh.d + 1) * fb : nullptr;
+        rc = lbm_get_macros(c, rho_d, u_d, phi_d, C_d);
+        if (rc) return rc;
+        if (rho_h) CK(cudaMemcpyAsync(rho_h, rho_d, (size_t)sh.S * fb, cudaMemcpyDeviceToHost, c->stream));
+        if (u_h) CK(cudaMemcpyAsync(u_h, u_d, (size_t)sh.d * fb, cudaMemcpyDeviceToHost, c->stream));
+        if (phi_h) CK(cudaMemcpyAsync(phi_h, phi_d, fb, cudaMemcpyDeviceToHost, c->stream));
+        if (C_h) CK(cudaMemcpyAsync(C_h, C_d, fb, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+int64_t lbm_time(const lbm_ctx* c) { return c ? c->t : -1; }
+int64_t lbm_launch_count(const lbm_ctx* c) { return c ? c->launches : -1; }
+
+int lbm_lattice_table(int lattice, int kind, int* Q, int* cc, double* w, int* opp) {
+    if (!Q || !cc || !w || !opp) return fail(LBM_EINVAL, "NULL argument");
+    if (lattice != LBM_D2Q9 && lattice != LBM_D3Q19) return fail(LBM_EINVAL, "unknown lattice");
+    auto fill = [&](auto L, bool flow, double w0) {
+        using LL = decltype(L);
+        *Q = LL::Q;
+        for (int i = 0; i < LL::Q; ++i) {
+            for (int a = 0; a < 3; ++a) cc[3 * i + a] = LL::c(i, a);
+            opp[i] = LL::opp(i);
+            if (!flow) w[i] = i == 0 ? w0 : (1.0 - w0) / (double)(LL::Q - 1);
+        }
+    };
+    if (kind == 0) {
+        if (lattice == LBM_D3Q19) { fill(lbm::D3Q19{}, true, 0); for (int i = 0; i < 19; ++i) w[i] = lbm::D3Q19::w(i); }
+        else { fill(lbm::D2Q9{}, true, 0); for (int i = 0; i < 9; ++i) w[i] = lbm::D2Q9::w(i); }
+    } else {
+        if (lattice == LBM_D3Q19) fill(lbm::D3Q7{}, false, 0.25); else fill(lbm::D2Q5{}, false, 0.4);
+    }
+    return 0;
+}
+
+}  // extern "C"

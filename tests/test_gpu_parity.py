@@ -1,0 +1,359 @@
+"""Parity of the CUDA library (through the C ABI of include/lbm.h) with the CPU oracle.  `-m gpu`.
+
+Same seeded inputs on both sides (workloads.py); the oracle never sees a value produced by the
+CUDA path.  Bars:
+  * populations, models without a transcendental (BGK, psi = rho): BIT-EXACT, fp64 and fp32 --
+    both sides evaluate the same IEEE expression tree without FMA contraction;
+  * SC1 (psi = 1 - exp(-rho), Eq. 10): CUDA's and glibc's exp differ by <= 1 ulp, so <= 1e-13
+    per field over 16 steps and the north-star bar <= 1e-12 (fp64) after 1000 steps;
+  * fields after 1000 steps: max|a-b| / max|b| <= 1e-12 (fp64), <= 1e-5 (fp32 vs fp32 oracle),
+    vector fields with the Euclidean norm per cell (BASELINE.json north_star; R14).
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests need a B200")
+    import paper_2502_12955_b200 as lbm
+    lbm.lib()
+    return lbm
+
+
+def make_pair(lbm, cfg):
+    from oracle.ref_lbm import RefLBM
+    ref = RefLBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev = lbm.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    return ref, dev
+
+
+def field_err(a, b):
+    """max_x |a - b| / max_x |b|; a, b shaped (components, N) or (N,): Euclidean norm over components."""
+    a = np.asarray(a, np.float64)
+    b = np.asarray(b, np.float64)
+    if a.ndim == 1:
+        a, b = a[None], b[None]
+    num = np.sqrt(((a - b) ** 2).sum(0)).max()
+    den = np.sqrt((b ** 2).sum(0)).max()
+    return num / den if den > 0 else num
+
+
+def macro_errs(ref, dev):
+    mr = ref.get_macros()
+    md = dev.get_macros()
+    out = {}
+    for s in range(ref.S):
+        out["rho%d" % s] = field_err(md["rho"][s].cpu().numpy(), mr["rho"][s])
+    out["u"] = field_err(md["u"].cpu().numpy(), mr["u"])
+    out["phi"] = field_err(md["phi"].cpu().numpy(), mr["phi"])
+    if mr["C"] is not None:
+        out["C"] = field_err(md["C"].cpu().numpy(), mr["C"])
+    return out
+
+
+SMALL = [
+    # (config, grid, overrides)
+    ("cfg1", (8, 8, 1), {}),
+    ("cfg1", (7, 5, 1), {}),
+    ("cfg1", (33, 17, 1), {}),
+    ("cfg1", (9, 6, 1), dict(bc=(0, 1, 0), force=(2e-5, 0.0, 0.0))),
+    ("cfg1", (6, 9, 1), dict(bc=(1, 1, 0), force=(1e-5, -2e-5, 0.0))),
+    ("cfg2", (8, 8, 1), dict(radius=2.5)),
+    ("cfg2", (33, 17, 1), dict(radius=5.0)),
+    ("cfg3", (8, 8, 1), {}),
+    ("cfg3", (33, 17, 1), dict(force=(1e-5, 2e-5, 0.0), tau=(0.8, 1.3))),
+    ("cfg4", (8, 8, 8), {}),
+    ("cfg4", (33, 17, 9), {}),
+    ("cfg4", (5, 4, 7), dict(bc=(1, 0, 1))),
+    ("cfg4", (4, 6, 5), dict(bc=(1, 1, 1), force=(1e-6, 2e-6, -1e-6))),
+    ("cfg4", (8, 6, 5), dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.03)),
+    ("cfg4", (8, 8, 8), dict(precision=32)),
+    ("cfg4", (33, 17, 9), dict(precision=32)),
+    ("cfg5", (8, 8, 8), dict(rmin=2.0, rmax=3.0, vol_frac=0.2)),
+    ("cfg5", (33, 17, 9), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
+    ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
+    ("cfg3", (16, 8, 1), dict(precision=32)),
+]
+
+
+@pytest.mark.parametrize("name,grid,over", SMALL, ids=lambda v: str(v).replace(" ", ""))
+def test_populations_exact_steps_1_to_16(gpu, name, grid, over):
+    """Population-exact comparison at every step 1..16 (odd and even AA parity), small and awkward
+    grids that are not multiples of the block size, every model, walls on/off."""
+    cfg = workloads.config(name, grid=grid, **over)
+    ref, dev = make_pair(gpu, cfg)
+    ref.init_from_seed(7)
+    f0 = ref.get_populations()
+    dev.set_populations(torch.from_numpy(f0))     # identical inputs: the oracle's seeded state
+    exact = not (cfg["model"] == "SC1" and cfg["params"].get("psi_kind", 0) == 0)
+    for step in range(1, 17):
+        ref.step(1)
+        dev.step(1)
+        fr = ref.get_populations()
+        fd = dev.get_populations().cpu().numpy()
+        if exact:
+            bad = np.flatnonzero(fr != fd)
+            assert bad.size == 0, "step %d: %d of %d populations differ, first at %d: %r vs %r" % (
+                step, bad.size, fr.size, bad[0], fd[bad[0]], fr[bad[0]])
+        else:
+            err = np.abs(fr - fd).max() / np.abs(fr).max()
+            assert err <= 1e-13, "step %d: population error %.3e" % (step, err)
+    errs = macro_errs(ref, dev)
+    tol = 0.0 if exact else 1e-13
+    assert max(errs.values()) <= tol, errs
+    Fr = ref.get_force()
+    Fd = dev.get_force().cpu().numpy()
+    if exact:
+        assert np.array_equal(Fr, Fd)
+    else:
+        assert np.abs(Fr - Fd).max() <= 1e-13 * max(np.abs(Fr).max(), 1e-300)
+
+
+@pytest.mark.parametrize("name,grid,over", [
+    ("cfg1", (64, 64, 1), {}),
+    ("cfg2", (40, 24, 1), dict(radius=8.0)),
+    ("cfg3", (24, 40, 1), {}),
+    ("cfg4", (6, 5, 16), {}),
+    ("cfg4", (12, 10, 8), dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.05)),
+    ("cfg5", (24, 20, 16), dict(rmin=3.0, rmax=6.0, vol_frac=0.1)),
+    ("cfg5", (24, 20, 1), dict(rmin=3.0, rmax=6.0, vol_frac=0.1)),
+], ids=lambda v: str(v).replace(" ", ""))
+def test_init_from_seed_matches_oracle(gpu, name, grid, over):
+    """lbm_init_from_seed against ref_init_from_seed: the counter-based noise is integer-exact; the
+    macroscopic fields go through cos/sin/tanh/sqrt in double (<= few ulp between libm and CUDA)."""
+    if name == "cfg5" and grid[2] == 1:
+        cfg = workloads.config(name, grid=grid, **over)
+        cfg["lattice"] = "D2Q9"
+    else:
+        cfg = workloads.config(name, grid=grid, **over)
+    ref, dev = make_pair(gpu, cfg)
+    ref.init_from_seed(1234)
+    dev.init_from_seed(1234)
+    fr = ref.get_populations()
+    fd = dev.get_populations().cpu().numpy()
+    tol = 1e-14 if cfg["params"]["precision"] == 64 else 3e-7
+    assert np.abs(fr - fd).max() <= tol * np.abs(fr).max()
+    if cfg["params"]["init_kind"] in ("REST", "UNIFORM_NOISE"):
+        assert np.array_equal(fr, fd)      # no transcendental on the way: bit-exact
+
+
+def run_1000(gpu, cfg, seed, nsteps=1000):
+    ref, dev = make_pair(gpu, cfg)
+    ref.init_from_seed(seed)
+    dev.set_populations(torch.from_numpy(ref.get_populations()))
+    ref.step(nsteps)
+    dev.step(nsteps)
+    return ref, dev
+
+
+def test_cfg1_taylor_green_1000_steps(gpu):
+    """configs[0]: D2Q9 BGK fp64 64x64, 1000 steps, fields <= 1e-12 and the closed-form decay
+    exp(-2 nu k^2 t), nu = (tau - 1/2)/3 (Eq. 3-6; 533-545)."""
+    cfg = workloads.config("cfg1")
+    ref, dev = run_1000(gpu, cfg, 1)
+    errs = macro_errs(ref, dev)
+    assert max(errs.values()) <= 1e-12, errs
+    # the GPU path's own init + closed form, independent of the oracle
+    dev.init_from_seed(1)
+    dev.step(1000)
+    u = dev.get_macros()["u"].cpu().numpy().reshape(2, 64, 64)
+    k = 2 * np.pi / 64
+    x = np.arange(64)
+    mode = -np.cos(k * x)[None, :] * np.sin(k * x)[:, None]
+    amp = (u[0] * mode).sum() / (mode ** 2).sum()
+    exact = 0.01 * np.exp(-2 * 0.1 * k * k * 1000)
+    assert abs(amp / exact - 1) <= 5e-3
+
+
+def test_cfg2_shan_chen_droplet_1000_steps(gpu):
+    """configs[1] at full size 256x256, R = 30, 1000 steps: fields <= 1e-12; mass conserved."""
+    cfg = workloads.config("cfg2")
+    ref, dev = run_1000(gpu, cfg, 2)
+    errs = macro_errs(ref, dev)
+    assert max(errs.values()) <= 1e-12, errs
+    m0 = ref.get_macros()["rho"].sum()
+    dev.step(1000)
+    m1 = dev.get_macros()["rho"].double().sum().item()
+    assert abs(m1 / m0 - 1) <= 1e-10
+
+
+def test_cfg3_two_component_1000_steps(gpu):
+    """configs[2] on a reduced 192x160 grid (the oracle needs ~3 min for 512x512), 1000 steps of
+    spinodal decomposition: fields <= 1e-12 (bit-exact by construction); per-component mass."""
+    cfg = workloads.config("cfg3", grid=(192, 160, 1))
+    ref, dev = run_1000(gpu, cfg, 3)
+    errs = macro_errs(ref, dev)
+    assert max(errs.values()) <= 1e-12, errs
+    rho = dev.get_macros()["rho"].cpu().numpy()
+    assert np.ptp(rho[0]) > 0.05           # demixing has started (psi = rho, G12 = 1.2 > 1: R3)
+    N = rho.shape[1]
+    for s in range(2):
+        assert abs(rho[s].sum() / N - 1.0) <= 1e-3    # +-1 % noise averages out
+    m0 = rho.sum(1)
+    dev.step(1000)
+    m1 = dev.get_macros()["rho"].cpu().numpy().sum(1)
+    assert np.abs(m1 / m0 - 1).max() <= 1e-10
+
+
+@pytest.mark.parametrize("precision,tol", [(64, 1e-12), (32, 1e-5)])
+def test_cfg4_poiseuille_full_size_vs_column_oracle(gpu, precision, tol):
+    """configs[3] at the full 256^3 in the launch configuration bench.py times, 1000 steps, against
+    the oracle run on a 1x1x256 column: the flow is x/y-invariant, which the oracle reproduces
+    bit for bit (tests/test_oracle_pins.py::test_poiseuille_xy_invariance_is_bit_exact)."""
+    from oracle.ref_lbm import RefLBM
+    cfg = workloads.config("cfg4", precision=precision)
+    col = workloads.config("cfg4", grid=(1, 1, 256), precision=precision)
+    ref = RefLBM(*col["grid"], col["lattice"], col["model"], **col["params"])
+    ref.init_from_seed(0)
+    ref.step(1000)
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(0)
+    dev.step(1000)
+    mr = ref.get_macros()
+    md = dev.get_macros(phi=False)
+    rho = md["rho"].reshape(256, 256 * 256)
+    u = md["u"].reshape(3, 256, 256 * 256)
+    rr = torch.from_numpy(mr["rho"].reshape(256, 1)).to(rho.device)
+    ur = torch.from_numpy(mr["u"].reshape(3, 256, 1)).to(rho.device)
+    e_rho = ((rho - rr).abs().max() / rr.abs().max()).item()
+    e_u = (((u - ur) ** 2).sum(0).sqrt().max() / (ur ** 2).sum(0).sqrt().max()).item()
+    assert e_rho <= tol and e_u <= tol, (e_rho, e_u)
+    assert e_rho == 0.0 and e_u == 0.0      # same expression tree, no transcendental: bit-exact
+
+
+def test_cfg4_steady_poiseuille_closed_form(gpu):
+    """Guo force + halfway bounce-back on the GPU path alone against the closed form
+    u_x(z) = g/(2 nu) (z+1/2)(H-z-1/2) + g/(8 nu) (16 (tau-1/2)^2/3 - 1), H = nz (DESIGN.md pins;
+    PAPER.md:504-531 Eq. 43-44 with the textbook 1/2)."""
+    nz, tau, g = 32, 0.9, 1e-6
+    cfg = workloads.config("cfg4", grid=(16, 12, nz))
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(0)
+    nu = (tau - 0.5) / 3
+    dev.step(int(30 * nz * nz / nu / 9.87))
+    u = dev.get_macros()["u"].cpu().numpy().reshape(3, nz, 12 * 16)
+    z = np.arange(nz)
+    exact = g / (2 * nu) * (z + 0.5) * (nz - z - 0.5) + g / (8 * nu) * (16 * (tau - 0.5) ** 2 / 3 - 1)
+    assert np.abs(u[0] - exact[:, None]).max() <= 1e-6 * exact.max()
+    assert np.abs(u[1:]).max() <= 1e-15
+
+
+def test_cfg5_reduced_1000_steps_fp32(gpu):
+    """configs[4] on a reduced 28x24x20 grid (the oracle runs ~0.5 MLUPS), fp32 against the fp32
+    oracle, 1000 steps: fields <= 1e-5 (north_star); bit-exact by construction (psi = rho)."""
+    cfg = workloads.config("cfg5", grid=(28, 24, 20), rmin=4.0, rmax=8.0, vol_frac=0.1)
+    ref, dev = run_1000(gpu, cfg, 5)
+    errs = macro_errs(ref, dev)
+    assert max(errs.values()) <= 1e-5, errs
+    assert np.array_equal(ref.get_populations(), dev.get_populations().cpu().numpy())
+
+
+def tile_populations(f_small, nvals, small, full, device):
+    """(nvals, nz, ny, nx) periodic tile of a small canonical population array to the full grid."""
+    sx, sy, sz = small
+    fx, fy, fz = full
+    t = torch.from_numpy(f_small.reshape(nvals, sz, sy, sx)).to(device)
+    return t.repeat(1, fz // sz, fy // sy, fx // sx).reshape(-1)
+
+
+def check_tiled(out, ref_small, nvals, small, full):
+    sx, sy, sz = small
+    fx, fy, fz = full
+    o = out.reshape(nvals, fz // sz, sz, fy // sy, sy, fx // sx, sx)
+    r = torch.from_numpy(ref_small.reshape(nvals, 1, sz, 1, sy, 1, sx)).to(out.device)
+    return bool((o == r).all().item())
+
+
+@pytest.mark.parametrize("name,small,over,nsteps", [
+    ("cfg3", (32, 16, 1), {}, 5),
+    ("cfg4", (8, 4, 256), dict(init_kind="UNIFORM_NOISE", noise_amp=0.05), 5),
+    ("cfg4", (8, 4, 256), dict(init_kind="UNIFORM_NOISE", noise_amp=0.05, precision=32), 4),
+    ("cfg5", (16, 8, 8), dict(rmin=2.0, rmax=4.0, vol_frac=0.1), 3),
+], ids=lambda v: str(v).replace(" ", ""))
+def test_full_size_equals_tiled_small_oracle(gpu, name, small, over, nsteps):
+    """Full BASELINE.json sizes (512^2, 256^3, 512^3) in the launch configuration bench.py times:
+    a periodic tiling of a small seeded state stays a periodic tiling, so every cell of the full
+    grid must equal, bit for bit, the oracle's result on the small grid."""
+    from oracle.ref_lbm import RefLBM
+    full = workloads.CONFIGS[name]["grid"]
+    cs = workloads.config(name, grid=small, **over)
+    cf = workloads.config(name, **over)
+    ref = RefLBM(*cs["grid"], cs["lattice"], cs["model"], **cs["params"])
+    ref.init_from_seed(11)
+    nvals = ref.population_count() // ref.N
+    dev = gpu.LBM(*cf["grid"], cf["lattice"], cf["model"], **cf["params"])
+    big = tile_populations(ref.get_populations(), nvals, small, full, dev.device)
+    dev.set_populations(big)
+    del big
+    ref.step(nsteps)
+    dev.step(nsteps)
+    out = dev.get_populations()
+    assert check_tiled(out, ref.get_populations(), nvals, small, full)
+    del out
+    torch.cuda.empty_cache()
+
+
+def test_cfg5_full_size_invariants(gpu):
+    """configs[4] at 512^3 from its own seeded init: masses of A and B conserved, total C
+    non-increasing and bounded below by C0 (1-k)^t (reaction sink, R8), no NaN."""
+    cfg = workloads.config("cfg5")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(42)
+    m = dev.get_macros(u=False, phi=False)
+    m0 = m["rho"].double().sum(1).cpu().numpy()
+    c0 = m["C"].double().sum().item()
+    vol = (m["rho"][0] > 1.0).double().mean().item()
+    assert 0.03 <= vol <= 0.07            # ~5 % volume fraction of component A (overlaps allowed)
+    del m
+    nsteps = 20
+    dev.step(nsteps)
+    m = dev.get_macros(phi=False)
+    assert bool(torch.isfinite(m["u"]).all().item())
+    m1 = m["rho"].double().sum(1).cpu().numpy()
+    c1 = m["C"].double().sum().item()
+    assert np.abs(m1 / m0 - 1).max() <= 1e-4        # fp32 populations, fp64 sum
+    assert c0 * (1 - 1e-3) ** nsteps * (1 - 1e-5) <= c1 <= c0 * (1 + 1e-6)
+    del m, dev
+    torch.cuda.empty_cache()
+
+
+def test_run_host_matches_device_path(gpu):
+    """lbm_run_host (host buffers in and out, copies inside) gives the same bits as the device calls."""
+    cfg = workloads.config("cfg4", grid=(16, 12, 10))
+    ref, dev = make_pair(gpu, cfg)
+    ref.init_from_seed(3)
+    f0 = ref.get_populations()
+    rho = np.empty((1, dev.N))
+    u = np.empty((3, dev.N))
+    dev.run_host(f0, 7, rho=rho, u=u)
+    ref.step(7)
+    mr = ref.get_macros()
+    assert np.array_equal(rho, mr["rho"]) and np.array_equal(u, mr["u"])
+    assert dev.time() == 7 and dev.launch_count() > 0
+
+
+def test_errors_and_state(gpu):
+    cfg = workloads.config("cfg1", grid=(8, 8, 1))
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    with pytest.raises(gpu.LbmError) as e:
+        dev.step(1)                                   # before init
+    assert e.value.code == -4
+    dev.init_from_seed(0)
+    dev.step(0)
+    with pytest.raises(gpu.LbmError):
+        dev.step(-1)
+    buf = dev._new(dev.N)
+    assert dev.L.lbm_get_macros(dev.h, None, None, None, buf.data_ptr()) == -1   # BGK has no scalar lattice
+    assert "scalar" in gpu.lbm.last_error()
+    with pytest.raises(gpu.LbmError):
+        gpu.LBM(8, 8, 2, "D2Q9", "BGK")               # D2Q9 needs nz == 1
+    with pytest.raises(gpu.LbmError):
+        gpu.LBM(8, 8, 1, "D2Q9", "SC1", bc=(1, 0, 0))  # Shan-Chen + walls: not implemented
