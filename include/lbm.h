@@ -131,6 +131,14 @@ int64_t lbm_time(const lbm_ctx* ctx);
 /* number of kernel launches this context has enqueued so far (for benchmarks) */
 int64_t lbm_launch_count(const lbm_ctx* ctx);
 
+/* Per-kernel timing for benchmarks.  lbm_kernel_timing(ctx, 1) synchronises the stream, discards
+ * earlier records and from then on brackets every launch of the fused step kernel (kind 0) and of
+ * the psi pass (kind 1) with a pair of CUDA events on the context's stream; (ctx, 0) switches it
+ * off.  lbm_kernel_time_ms synchronises the stream and returns the summed device time (ms) and
+ * the number of launches of that kind recorded since timing was switched on.  Host pointers. */
+int lbm_kernel_timing(lbm_ctx* ctx, int enable);
+int lbm_kernel_time_ms(lbm_ctx* ctx, int kind, double* total_ms, int64_t* launches);
+
 /* Lattice tables as the kernels use them: kind 0 = flow lattice, 1 = scalar lattice (default w0).
  * c receives Q*3 ints, w receives Q doubles, opp receives Q ints.  Host pointers. */
 int lbm_lattice_table(int lattice, int kind, int* Q, int* c, double* w, int* opp);

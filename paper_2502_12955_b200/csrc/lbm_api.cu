@@ -112,6 +112,9 @@ struct lbm_ctx {
     double4* droplets_dev;
     void* scratch;        // device staging for lbm_run_host outputs
     size_t scratch_bytes;
+    // per-kernel timing (lbm_kernel_timing): event pairs around every launch of kind 0 (fused step) / 1 (psi pass)
+    bool timing;
+    std::vector<cudaEvent_t> ev[2];
 
     const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
 };
@@ -170,10 +173,29 @@ std::vector<double4> droplet_list(const lbm_ctx* c, uint64_t seed) {
     return v;
 }
 
+// event before / after a launch of the given kind while kernel timing is on
+int mark(lbm_ctx* c, int kind) {
+    if (!c->timing) return 0;
+    cudaEvent_t e;
+    CK(cudaEventCreate(&e));
+    c->ev[kind].push_back(e);
+    CK(cudaEventRecord(e, c->stream));
+    return 0;
+}
+
+void drop_events(lbm_ctx* c) {
+    for (int k = 0; k < 2; ++k) {
+        for (cudaEvent_t e : c->ev[k]) cudaEventDestroy(e);
+        c->ev[k].clear();
+    }
+}
+
 int run_psi(lbm_ctx* c) {
+    int rc = mark(c, 1);
+    if (rc) return rc;
     CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->stream));
     c->launches++;
-    return 0;
+    return mark(c, 1);
 }
 
 int ensure_scratch(lbm_ctx* c, size_t bytes) {
@@ -217,6 +239,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->stream = (cudaStream_t)p->stream;
     c->inited = false; c->t = 0; c->launches = 0;
     c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
+    c->timing = false;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
         if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
@@ -248,6 +271,7 @@ void lbm_destroy(lbm_ctx* c) {
     if (!c) return;
     DeviceGuard g(c->device);
     cudaStreamSynchronize(c->stream);
+    drop_events(c);
     if (c->droplets_dev) cudaFree(c->droplets_dev);
     if (c->scratch) cudaFree(c->scratch);
     if (c->owns_ws && c->ws) cudaFree(c->ws);
@@ -289,12 +313,15 @@ int lbm_step(lbm_ctx* c, int n) {
     DeviceGuard g(c->device);
     for (int k = 0; k < n; ++k) {
         const int parity = (int)(c->t & 1);
+        int rc;
         if (c->sh.sc) {   // a2: psi of every cell at this time level (full-field barrier, R9)
-            CK(c->ops->psi(c->kp(), c->model, parity, c->stream));
-            c->launches++;
+            rc = run_psi(c);
+            if (rc) return rc;
         }
+        if ((rc = mark(c, 0))) return rc;
         CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, c->stream));
         c->launches++;
+        if ((rc = mark(c, 0))) return rc;
         c->t++;
     }
     return 0;
@@ -387,6 +414,32 @@ int lbm_run_host(lbm_ctx* c, const void* f_in_host, int n, void* rho_h, void* u_
         if (C_h) CK(cudaMemcpyAsync(C_h, C_d, fb, cudaMemcpyDeviceToHost, c->stream));
     }
     CK(cudaStreamSynchronize(c->stream));
+    return 0;
+}
+
+int lbm_kernel_timing(lbm_ctx* c, int enable) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    DeviceGuard g(c->device);
+    CK(cudaStreamSynchronize(c->stream));
+    drop_events(c);
+    c->timing = enable != 0;
+    return 0;
+}
+
+int lbm_kernel_time_ms(lbm_ctx* c, int kind, double* total_ms, int64_t* launches) {
+    if (!c || !total_ms || !launches) return fail(LBM_EINVAL, "NULL argument");
+    if (kind != 0 && kind != 1) return fail(LBM_EINVAL, "kind must be 0 (fused step) or 1 (psi pass)");
+    DeviceGuard g(c->device);
+    CK(cudaStreamSynchronize(c->stream));
+    double sum = 0.0;
+    const std::vector<cudaEvent_t>& v = c->ev[kind];
+    for (size_t k = 0; k + 1 < v.size(); k += 2) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, v[k], v[k + 1]));
+        sum += (double)ms;
+    }
+    *total_ms = sum;
+    *launches = (int64_t)(v.size() / 2);
     return 0;
 }
 

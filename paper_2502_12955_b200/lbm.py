@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_time", "lbm_launch_count", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -79,6 +79,8 @@ def lib():
     L.lbm_time.argtypes = [C.c_void_p]
     L.lbm_launch_count.restype = C.c_int64
     L.lbm_launch_count.argtypes = [C.c_void_p]
+    L.lbm_kernel_timing.argtypes = [C.c_void_p, C.c_int]
+    L.lbm_kernel_time_ms.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.lbm_lattice_table.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int), C.c_void_p, C.c_void_p, C.c_void_p]
     L.lbm_destroy.argtypes = [C.c_void_p]
     L.lbm_last_error.restype = C.c_char_p
@@ -238,6 +240,15 @@ class LBM:
 
     def launch_count(self):
         return int(self.L.lbm_launch_count(self.h))
+
+    def kernel_timing(self, enable):
+        self._chk(self.L.lbm_kernel_timing(self.h, 1 if enable else 0))
+
+    def kernel_time_ms(self, kind):
+        """(summed device ms, launches) of kind 0 = fused step kernel, 1 = psi pass"""
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        self._chk(self.L.lbm_kernel_time_ms(self.h, int(kind), C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def synchronize(self):
         self.stream.synchronize()
