@@ -1,0 +1,449 @@
+"""Benchmark of the lattice Boltzmann hot path (BASELINE.json metric: MLUPS and achieved HBM GB/s as a
+fraction of the B200 peak, per lattice/model, one GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--precision 64|32]
+                    [--impl ours|reference] [--no-extras]
+
+A "step" is ONE time step of the whole hot path (moments, psi, Shan-Chen force, velocity, BGK + Guo
+collision, scalar lattice, in-place streaming, boundaries: DESIGN.md rows a1-a8) over the whole grid.
+The headline workload is BASELINE.json configs[3]: D3Q19 BGK + Guo force, 256^3, halfway bounce-back
+walls in z, fp64 ("throughput timed over 1000 steps"); the other configs are reported in "per_model"
+with the same kernels and timing method.  Inputs are seeded and synthetic (workloads.py), resident in
+HBM before the timed region; the population array (2.55 GB) is far larger than the 126 MB L2, so no
+explicit L2 flush is needed between steps (config.l2 says so).
+
+Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard (north_star: one GPU, one domain),
+so --gpus N runs N independent replicas ("replicas only", weak scaling, no data-path collective).
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
+workload on the host cores; it is the only other place this file executes oracle/.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+HBM_NOMINAL_GBS = 8000.0      # north_star: "the B200's ~8 TB/s"
+HBM_FALLBACK_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def measured_peak():
+    """(GB/s, 'measured'|'fallback')"""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback"
+
+
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, copied by hand from
+    the newest `ncu --set full` capture into profiles/r*_traffic.csv (None when there is no capture)."""
+    import csv
+    import glob
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv"))):
+        try:
+            with open(path) as fh:
+                for row in csv.DictReader(fh):
+                    if row["workload"] == workload:
+                        best = float(row["traffic_bytes_per_launch"])
+        except Exception:
+            pass
+    return best
+
+
+def shape_of(cfg):
+    S = 2 if cfg["model"] in ("SC2", "SC2_ADE") else 1
+    Q = 19 if cfg["lattice"] == "D3Q19" else 9
+    Qs = (7 if cfg["lattice"] == "D3Q19" else 5) if cfg["model"] == "SC2_ADE" else 0
+    B = 8 if cfg["params"]["precision"] == 64 else 4
+    N = cfg["grid"][0] * cfg["grid"][1] * cfg["grid"][2]
+    sc = cfg["model"] != "BGK"
+    return dict(S=S, Q=Q, Qs=Qs, B=B, N=N, sc=sc)
+
+
+def algorithmic_bytes(cfg):
+    """Algorithmic bytes per lattice update:
+    step kernel: every population read once and written once (+ one compulsory psi read per component);
+    psi pass: psi written once per component (its re-read of the flow populations is NOT algorithmic:
+    it is this design's overhead and shows up as a lower fraction)."""
+    s = shape_of(cfg)
+    step = (2 * (s["S"] * s["Q"] + s["Qs"]) + (s["S"] if s["sc"] else 0)) * s["B"]
+    psi = (s["S"] if s["sc"] else 0) * s["B"]
+    return step, psi
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (NVML; B200_PROFILING.md clocks line)."""
+
+    def __init__(self, index=0, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+# --------------------------------------------------------------------------------------------
+# GPU arm
+# --------------------------------------------------------------------------------------------
+def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None):
+    """Times `steps` time steps with populations resident in HBM.  Returns a dict with the elapsed
+    ms (CUDA events on the context's stream), the per-kernel device times measured with event pairs
+    around every launch in a second pass of the same length, and the launch count."""
+    import torch
+    import paper_2502_12955_b200 as lbm
+    sim = lbm.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], device=device, **cfg["params"])
+    sim.init_from_seed(seed)
+    sim.step(warmup)
+    sim.synchronize()
+    if barrier is not None:
+        barrier()
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx = sampler if sampler is not None else _Null()
+    with ctx:
+        e0.record(sim.stream)
+        sim.step(steps)
+        e1.record(sim.stream)
+        e1.synchronize()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    if barrier is not None:
+        barrier()
+    # second pass: the dominant kernel's own average duration (event pair around every launch)
+    nk = min(steps, 200)
+    sim.kernel_timing(True)
+    sim.step(nk)
+    step_ms, step_n = sim.kernel_time_ms(0)
+    psi_ms, psi_n = sim.kernel_time_ms(1)
+    sim.kernel_timing(False)
+    # sanity: the state is finite (a NaN-producing run is not a benchmark)
+    m = sim.get_macros(u=False, phi=False, C_=False)
+    finite = bool(torch.isfinite(m["rho"]).all().item())
+    del m
+    sim.close()
+    torch.cuda.empty_cache()
+    return dict(ms=ms, launches=launches, step_ms=step_ms, step_n=step_n, psi_ms=psi_ms, psi_n=psi_n, finite=finite)
+
+
+class _Null:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        pass
+
+
+def time_e2e(cfg, steps, device, seed):
+    """The same metric through lbm_run_host: pinned HOST buffers in and out, the host->device copy of
+    the canonical populations and the device->host copy of rho and u inside the timed region."""
+    import torch
+    import paper_2502_12955_b200 as lbm
+    s = shape_of(cfg)
+    sim = lbm.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], device=device, **cfg["params"])
+    sim.init_from_seed(seed)
+    f_dev = sim.get_populations()
+    f_host = torch.empty(f_dev.numel(), dtype=f_dev.dtype, pin_memory=True)
+    f_host.copy_(f_dev)
+    del f_dev
+    d = 3 if cfg["lattice"] == "D3Q19" else 2
+    rho = torch.empty(s["S"] * s["N"], dtype=f_host.dtype, pin_memory=True)
+    u = torch.empty(d * s["N"], dtype=f_host.dtype, pin_memory=True)
+    sim.run_host(f_host, min(steps, 3), rho=rho, u=u)       # warm-up call (same path)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(sim.stream)
+    sim.run_host(f_host, steps, rho=rho, u=u)
+    e1.record(sim.stream)
+    e1.synchronize()
+    ms = e0.elapsed_time(e1)
+    ok = bool(torch.isfinite(rho).all().item())
+    h2d = f_host.numel() * f_host.element_size()
+    d2h = (rho.numel() + u.numel()) * rho.element_size()
+    sim.close()
+    del f_host, rho, u
+    torch.cuda.empty_cache()
+    return dict(ms=ms, h2d=h2d, d2h=d2h, finite=ok)
+
+
+def model_line(name, cfg, r, steps, peak):
+    """per-model entry: MLUPS, achieved algorithmic GB/s of the whole step and of each kernel"""
+    s = shape_of(cfg)
+    step_b, psi_b = algorithmic_bytes(cfg)
+    mlups = s["N"] * steps / (r["ms"] * 1e-3) / 1e6
+    gbs = (step_b + psi_b) * s["N"] * steps / (r["ms"] * 1e-3) / 1e9
+    out = {"workload": name, "lattice": cfg["lattice"], "model": cfg["model"], "grid": list(cfg["grid"]),
+           "dtype": "f64" if s["B"] == 8 else "f32", "steps": steps, "ms_per_step": r["ms"] / steps,
+           "mlups": round(mlups, 1), "algorithmic_bytes_per_update": step_b + psi_b,
+           "hbm_gbs": round(gbs, 1), "frac_of_measured": round(gbs / peak, 4),
+           "frac_of_nominal_8TBs": round(gbs / HBM_NOMINAL_GBS, 4),
+           "population_mb": round((s["S"] * s["Q"] + s["Qs"]) * s["N"] * s["B"] / 1e6, 1),
+           "finite": r["finite"]}
+    if r["step_n"]:
+        t = r["step_ms"] / r["step_n"]
+        out["step_kernel_ms"] = round(t, 5)
+        out["step_kernel_gbs"] = round(step_b * s["N"] / (t * 1e-3) / 1e9, 1)
+    if r["psi_n"]:
+        t = r["psi_ms"] / r["psi_n"]
+        out["psi_kernel_ms"] = round(t, 5)
+    return out
+
+
+# --------------------------------------------------------------------------------------------
+# CPU arm: the oracle as it stands (single-threaded), on a bounded sample of the workload
+# --------------------------------------------------------------------------------------------
+def oracle_sample_grid(cfg, budget_cells):
+    """A sub-grid of the workload with about budget_cells cells: the wall axis (z for cfg4) keeps its
+    full extent, the periodic axes shrink by powers of two."""
+    g = list(cfg["grid"])
+    bc = cfg["params"].get("bc", (0, 0, 0))
+    axes = [a for a in range(3) if not bc[a] and g[a] > 1]
+    while g[0] * g[1] * g[2] > budget_cells and axes:
+        a = max(axes, key=lambda k: g[k])
+        if g[a] <= 8:
+            break
+        g[a] //= 2
+    return tuple(g)
+
+
+def time_oracle(cfg, steps, warmup, seconds):
+    """(MLUPS, sample description, seconds spent).  The sample grid is chosen from a one-step probe so
+    that warmup + steps oracle steps take about `seconds`."""
+    from oracle.ref_lbm import RefLBM
+    over = {}
+    if cfg["params"].get("init_kind") == "RANDOM_DROPLETS":
+        over = dict(rmin=4.0, rmax=8.0, vol_frac=0.05)       # droplets that fit the sample grid
+    probe_grid = oracle_sample_grid(cfg, 1 << 18)           # larger than the host L2: an honest rate
+    pc = dict(cfg, grid=probe_grid, params=dict(cfg["params"], **over))
+    ref = RefLBM(*pc["grid"], pc["lattice"], pc["model"], **pc["params"])
+    ref.init_from_seed(1)
+    ref.step(1)
+    t0 = time.perf_counter()
+    ref.step(2)
+    rate = 2 * ref.N / (time.perf_counter() - t0)            # cell updates / s
+    ref.close()
+    budget = int(0.7 * rate * seconds / max(1, steps + warmup))
+    grid = oracle_sample_grid(cfg, max(budget, 1 << 12))
+    sc = dict(cfg, grid=grid, params=dict(cfg["params"], **over))
+    ref = RefLBM(*sc["grid"], sc["lattice"], sc["model"], **sc["params"])
+    ref.init_from_seed(1)
+    ref.step(warmup)
+    t0 = time.perf_counter()
+    ref.step(steps)
+    dt = time.perf_counter() - t0
+    n = ref.N
+    ref.close()
+    desc = "%s %s %s grid %dx%dx%d (sub-grid of %dx%dx%d), %d steps, single thread" % (
+        cfg["lattice"], cfg["model"], "f64" if cfg["params"]["precision"] == 64 else "f32",
+        grid[0], grid[1], grid[2], cfg["grid"][0], cfg["grid"][1], cfg["grid"][2], steps)
+    return n * steps / dt / 1e6, desc, dt
+
+
+def workload_name(key, cfg):
+    s = shape_of(cfg)
+    return "%s: %s %s %s %dx%dx%d" % (key, cfg["lattice"], cfg["model"], "fp64" if s["B"] == 8 else "fp32",
+                                      cfg["grid"][0], cfg["grid"][1], cfg["grid"][2])
+
+
+def run_reference(args, cfg, key):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    mlups, desc, dt = time_oracle(cfg, args.steps, args.warmup, seconds=90.0)
+    line = {"impl": "reference", "metric": "MLUPS", "value": round(mlups, 3), "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if cfg["params"]["precision"] == 64 else "f32", "data": "synthetic",
+            "config": {"workload": workload_name(key, cfg), "sample": desc},
+            "cpu_baseline": {"value": round(mlups, 3), "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": round(mlups, 3), "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# per-model lines of the default run: (key, config overrides, steps, warmup).  BASELINE.json configs
+# 1-3 at paper size are L2-resident (0.3 / 4.7 / 38 MB): their rate is launch/L2-bound and their "HBM
+# fraction" is flagged l2_resident; the 8192^2 rows run the same D2Q9 kernels HBM-bound.
+EXTRAS = [
+    ("cfg4", dict(precision=32), None, 1000, 50),
+    ("cfg5", dict(), None, 100, 10),
+    ("cfg1", dict(), None, 2000, 100),
+    ("cfg2", dict(), None, 2000, 100),
+    ("cfg3", dict(), None, 1000, 50),
+    ("cfg1", dict(), (8192, 8192, 1), 100, 10),
+    ("cfg2", dict(radius=2000.0), (8192, 8192, 1), 100, 10),
+    ("cfg3", dict(), (8192, 8192, 1), 50, 5),
+    ("cfg4", dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.05, tau=(0.5019, 0.5019)),
+     (128, 128, 128), 1000, 50),
+]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--precision", type=int, default=None, choices=[32, 64])
+    ap.add_argument("--grid", type=int, nargs=3, default=None, help="override the grid (profiling runs)")
+    ap.add_argument("--no-extras", action="store_true", help="skip per_model, e2e and cpu_baseline (profiling runs)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3                                       # timing rule: W >= 3
+    over = {} if args.precision is None else {"precision": args.precision}
+    cfg = workloads.config(args.workload, grid=args.grid, **over)
+    if args.impl == "reference":
+        run_reference(args, cfg, args.workload)
+        return
+
+    import torch
+    import paper_2502_12955_b200 as lbm
+    lbm.lib()                                                 # fails loudly when liblbm.so is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    device = "cuda:%d" % local
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peak, peak_kind = measured_peak()
+    sampler = ClockSampler(index=local) if rank == 0 else None
+    # replicas only: rank r runs its own seeded copy of the workload (no data-path collective)
+    r = time_device(cfg, args.steps, args.warmup, device, seed=1 + rank, sampler=sampler, barrier=barrier)
+    ms = r["ms"]
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)              # max over ranks
+        ms = float(t.item())
+    s = shape_of(cfg)
+    step_b, psi_b = algorithmic_bytes(cfg)
+    value = world * s["N"] * args.steps / (ms * 1e-3) / 1e6
+    e2e = None
+    if not args.no_extras:
+        e = time_e2e(cfg, args.steps, device, seed=1 + rank)
+        ems = e["ms"]
+        if dist is not None:
+            t = torch.tensor([ems], dtype=torch.float64, device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ems = float(t.item())
+        e2e = {"value": round(world * s["N"] * args.steps / (ems * 1e-3) / 1e6, 1), "unit": "MLUPS",
+               "h2d_bytes_per_step": e["h2d"] / args.steps, "d2h_bytes_per_step": e["d2h"] / args.steps,
+               "call": "lbm_run_host(f_host, n=%d, rho_host, u_host): one upload of the populations, %d steps, "
+                       "one download of rho and u, pinned host memory" % (args.steps, args.steps),
+               "ms": round(ems, 3), "finite": e["finite"]}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (the fused step kernel): algorithmic bytes per launch / its
+    # average launch duration, measured live with CUDA event pairs on the launching stream
+    k_ms = r["step_ms"] / max(1, r["step_n"])
+    achieved = step_b * s["N"] / (k_ms * 1e-3) / 1e9
+    traffic = ncu_traffic(workload_name(args.workload, cfg))
+    line = {
+        "metric": "MLUPS", "value": round(value, 1), "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64" if s["B"] == 8 else "f32", "data": "synthetic",
+        "config": {"workload": workload_name(args.workload, cfg), "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "inputs larger than L2 (%.0f MB populations vs 126 MB), no flush" %
+                         ((s["S"] * s["Q"] + s["Qs"]) * s["N"] * s["B"] / 1e6),
+                   "streaming": "in-place AA pattern, one population copy"},
+        "hbm_gbs": round((step_b + psi_b) * s["N"] * args.steps / (ms * 1e-3) / 1e9 , 1),
+        "roofline": {"bound": "hbm", "kernel": "k_step (fused collide+stream)", "achieved": round(achieved, 1),
+                     "peak": peak, "peak_kind": "of " + peak_kind, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                     "frac_of_nominal_8TBs": round(achieved / HBM_NOMINAL_GBS, 4),
+                     "algorithmic_bytes_per_update": step_b, "kernel_ms": round(k_ms, 5), "traffic": traffic},
+        "gpu_launches": r["launches"],
+        "clocks": sampler.summary() if sampler is not None else None,
+        "finite": r["finite"],
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    if not args.no_extras and world == 1:
+        per = [model_line(workload_name(args.workload, cfg), cfg, r, args.steps, peak)]
+        for key, ov, grid, k, w in EXTRAS:
+            c = workloads.config(key, grid=grid, **ov)
+            rr = time_device(c, k, w, device, seed=1)
+            ml = model_line(workload_name(key, c), c, rr, k, peak)
+            if ml["population_mb"] < 126.0:
+                ml["l2_resident"] = True
+            per.append(ml)
+        line["per_model"] = per
+        mlups, desc, _ = time_oracle(cfg, 6, 1, seconds=20.0)
+        line["cpu_baseline"] = {"value": round(mlups, 3), "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": desc}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
