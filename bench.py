@@ -83,6 +83,25 @@ def algorithmic_bytes(cfg):
     return step, psi
 
 
+def max_over_ranks(ms, dist=None, device="cpu"):
+    """max over ranks of a per-rank elapsed time (the contract's multi-GPU timing rule)"""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_mlups(world, cells_per_replica, steps, ms):
+    """whole-job MLUPS of `world` independent replicas that all finished within `ms` (replicas only)"""
+    return world * cells_per_replica * steps / (ms * 1e-3) / 1e6
+
+
+def replica_seed(rank):
+    return 1 + rank
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (NVML; B200_PROFILING.md clocks line)."""
 
@@ -377,24 +396,16 @@ def main():
     peak, peak_kind = measured_peak()
     sampler = ClockSampler(index=local) if rank == 0 else None
     # replicas only: rank r runs its own seeded copy of the workload (no data-path collective)
-    r = time_device(cfg, args.steps, args.warmup, device, seed=1 + rank, sampler=sampler, barrier=barrier)
-    ms = r["ms"]
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)              # max over ranks
-        ms = float(t.item())
+    r = time_device(cfg, args.steps, args.warmup, device, seed=replica_seed(rank), sampler=sampler, barrier=barrier)
+    ms = max_over_ranks(r["ms"], dist, device)
     s = shape_of(cfg)
     step_b, psi_b = algorithmic_bytes(cfg)
-    value = world * s["N"] * args.steps / (ms * 1e-3) / 1e6
+    value = aggregate_mlups(world, s["N"], args.steps, ms)
     e2e = None
     if not args.no_extras:
-        e = time_e2e(cfg, args.steps, device, seed=1 + rank)
-        ems = e["ms"]
-        if dist is not None:
-            t = torch.tensor([ems], dtype=torch.float64, device=device)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        e2e = {"value": round(world * s["N"] * args.steps / (ems * 1e-3) / 1e6, 1), "unit": "MLUPS",
+        e = time_e2e(cfg, args.steps, device, seed=replica_seed(rank))
+        ems = max_over_ranks(e["ms"], dist, device)
+        e2e = {"value": round(aggregate_mlups(world, s["N"], args.steps, ems), 1), "unit": "MLUPS",
                "h2d_bytes_per_step": e["h2d"] / args.steps, "d2h_bytes_per_step": e["d2h"] / args.steps,
                "call": "lbm_run_host(f_host, n=%d, rho_host, u_host): one upload of the populations, %d steps, "
                        "one download of rho and u, pinned host memory" % (args.steps, args.steps),

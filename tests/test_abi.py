@@ -1,0 +1,152 @@
+"""The C-ABI boundary without a GPU: liblbm.so loads, exports every symbol include/lbm.h declares,
+validates its arguments on the host, reports the lattice tables the kernels use, and refuses to run
+without a CUDA device (no CPU fallback).  No compute call is made here.  `-m "not gpu"`."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lbm():
+    import __graft_entry__ as ge
+    ge.build()                       # nvcc cross-compiles for sm_100a without a GPU
+    import paper_2502_12955_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def declared_symbols():
+    """function names declared in include/lbm.h"""
+    src = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lbm_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol(lbm):
+    names = declared_symbols()
+    assert "lbm_create" in names and "lbm_step" in names and "lbm_get_macros" in names
+    assert "lbm_init_from_seed" in names and "lbm_destroy" in names
+    L = lbm.lib()
+    for n in names:
+        assert hasattr(L, n), "liblbm.so does not export %s" % n
+    assert sorted(lbm.SYMBOLS) == names          # the binding lists exactly the header's functions
+
+
+def test_params_struct_matches_header(lbm):
+    """struct_size is checked by the library: a ctypes layout that disagreed with the C struct would
+    make every call fail with 'struct_size'."""
+    p = lbm.make_params(**workloads.config("cfg4")["params"])
+    n = lbm.lib().lbm_workspace_bytes(256, 256, 256, lbm.D3Q19, lbm.BGK, C.byref(p))
+    assert n >= 19 * 256 ** 3 * 8 and n < 19 * 256 ** 3 * 8 + 4096     # ONE population copy, no psi
+    p.struct_size -= 8
+    assert lbm.lib().lbm_workspace_bytes(256, 256, 256, lbm.D3Q19, lbm.BGK, C.byref(p)) == 0
+    assert "struct_size" in lbm.lbm.last_error()
+
+
+@pytest.mark.parametrize("name,expect", [
+    ("cfg1", 9 * 8), ("cfg2", (9 + 1) * 8), ("cfg3", (18 + 2) * 8), ("cfg4", 19 * 8), ("cfg5", (38 + 7 + 2) * 4)])
+def test_workspace_is_one_population_copy_plus_psi(lbm, name, expect):
+    """in-place streaming: S*Q + Qs values per cell and S values of psi, nothing else"""
+    cfg = workloads.config(name)
+    p = lbm.make_params(**cfg["params"])
+    nx, ny, nz = cfg["grid"]
+    n = lbm.lib().lbm_workspace_bytes(nx, ny, nz, lbm.lbm.LATTICES[cfg["lattice"]], lbm.lbm.MODELS[cfg["model"]], C.byref(p))
+    N = nx * ny * nz
+    assert expect * N <= n <= expect * N + 3 * 256
+
+
+@pytest.mark.parametrize("grid,lattice,model,over,msg", [
+    ((8, 8, 2), "D2Q9", "BGK", {}, "nz == 1"),
+    ((8, 8, 1), "D2Q9", "SC1", dict(bc=(1, 0, 0)), "walls"),
+    ((8, 8, 8), "D3Q19", "BGK", dict(tau=(0.5, 0.5)), "tau"),
+    ((8, 8, 8), "D3Q19", "BGK", dict(precision=16), "precision"),
+    ((8, 8, 8), "D3Q19", "SC2_ADE", dict(tau_c=0.4, bc=(0, 0, 0)), "tau_c"),
+    ((0, 8, 8), "D3Q19", "BGK", {}, "extents"),
+    ((2048, 2048, 1024), "D3Q19", "BGK", {}, "2^31"),
+    ((8, 8, 8), "D3Q19", "BGK", dict(forcing=1), "Guo"),
+    ((8, 8, 8), "D3Q19", "SC2", dict(psi_kind=2, bc=(0, 0, 0)), "psi_kind"),
+    ((8, 8, 8), "D3Q19", "SC1", dict(psi_kind=0, rho0_psi=0.0, bc=(0, 0, 0)), "rho0_psi"),
+    ((8, 8, 1), "D2Q9", "BGK", dict(bc=(0, 0, 1)), "bc[2]"),
+])
+def test_validation_messages(lbm, grid, lattice, model, over, msg):
+    p = lbm.make_params(**dict(workloads.config("cfg4")["params"], **over))
+    n = lbm.lib().lbm_workspace_bytes(grid[0], grid[1], grid[2], lbm.lbm.LATTICES[lattice], lbm.lbm.MODELS[model], C.byref(p))
+    assert n == 0
+    assert msg in lbm.lbm.last_error()
+
+
+def test_null_arguments_are_errors_not_crashes(lbm):
+    L = lbm.lib()
+    assert L.lbm_step(None, 1) == lbm.lbm.EINVAL
+    assert L.lbm_init_from_seed(None, 0) == lbm.lbm.EINVAL
+    assert L.lbm_get_macros(None, None, None, None, None) == lbm.lbm.EINVAL
+    assert L.lbm_population_count(None) == 0
+    assert L.lbm_time(None) == -1 and L.lbm_launch_count(None) == -1
+    L.lbm_destroy(None)
+    assert L.lbm_workspace_bytes(8, 8, 8, 1, 0, None) == 0
+
+
+def test_lattice_tables_of_the_kernels_match_the_paper(lbm):
+    """lbm_lattice_table (the compile-time tables the kernels unroll over) against the paper's
+    Tables 1-3 stored in tests/golden/lattice_tables.txt (w_4 of D2Q9: R1)."""
+    from fractions import Fraction
+    blocks, cur = {}, None
+    for line in open(os.path.join(ROOT, "tests", "golden", "lattice_tables.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        if line.startswith("["):
+            cur = line[1:-1]
+            blocks[cur] = {}
+        else:
+            k, *v = line.split()
+            blocks[cur][k] = v
+    for name, lattice, kind in [("D3Q19", "D3Q19", 0), ("D2Q9", "D2Q9", 0), ("D2Q5", "D2Q9", 1)]:
+        c, w, opp = lbm.lattice_table(lattice, kind)
+        b = blocks[name]
+        assert len(w) == len(b["w"])
+        assert np.allclose(w, [float(Fraction(x)) for x in b["w"]], rtol=0, atol=1e-16)
+        assert list(c[:, 0]) == [int(x) for x in b["cx"]]
+        assert list(c[:, 1]) == [int(x) for x in b["cy"]]
+        if "cz" in b:
+            assert list(c[:, 2]) == [int(x) for x in b["cz"]]
+        for i in range(len(w)):
+            assert (c[opp[i]] == -c[i]).all()
+        assert abs(w.sum() - 1) < 1e-15
+    c, w, opp = lbm.lattice_table("D3Q19", 1)          # D3Q7 (R6)
+    assert len(w) == 7 and w[0] == 0.25 and np.all(w[1:] == 0.125)
+    assert [tuple(r) for r in c[1:]] == [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+
+
+def test_no_cpu_fallback(lbm):
+    """Without a CUDA device lbm_create must fail loudly (and the binding must not route elsewhere)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    p = lbm.make_params(**workloads.config("cfg1")["params"])
+    h = lbm.lib().lbm_create(8, 8, 1, lbm.D2Q9, lbm.BGK, C.byref(p))
+    assert not h
+    assert "no usable CUDA device" in lbm.lbm.last_error() and "no CPU path" in lbm.lbm.last_error()
+    with pytest.raises(lbm.LbmError):
+        lbm.LBM(8, 8, 1, "D2Q9", "BGK")
+
+
+def test_product_path_never_touches_the_oracle():
+    """Neither the package nor the C/CUDA sources mention oracle/ or ref_lbm (independence of the two paths)."""
+    pkg = os.path.join(ROOT, "paper_2502_12955_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "ref_lbm" not in text and "import oracle" not in text and "from oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".h")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "liblbm" not in text and "kernels.cuh" not in text and "import paper_2502_12955_b200" not in text, f
