@@ -5,13 +5,15 @@
 
 namespace lbm {
 
-inline unsigned grid_for(int N) { return (unsigned)(((long long)N + BLOCK - 1) / BLOCK); }
+// one block per BLOCK-cell segment of one x-row: grid (ceil(nx/BLOCK), ny, nz)
+template <class KPT>
+inline dim3 grid_for(const KPT& p) { return dim3((unsigned)((p.nx + BLOCK - 1) / BLOCK), (unsigned)p.ny, (unsigned)p.nz); }
 
 template <class R, class L>
 struct Launch {
     template <int MODEL, int PARITY>
     static void psi2(const KP<R>& p, cudaStream_t st) {
-        k_psi<R, L, MODEL, PARITY><<<grid_for(p.N), BLOCK, 0, st>>>(p);
+        k_psi<R, L, MODEL, PARITY><<<grid_for(p), BLOCK, 0, st>>>(p);
     }
     static cudaError_t psi(const void* kp, int model, int parity, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
@@ -23,8 +25,8 @@ struct Launch {
 
     template <int MODEL, bool WALLS, bool FORCED>
     static void step3(const KP<R>& p, int parity, cudaStream_t st) {
-        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p.N), BLOCK, 0, st>>>(p);
-        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p.N), BLOCK, 0, st>>>(p);
+        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p), BLOCK, 0, st>>>(p);
+        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p), BLOCK, 0, st>>>(p);
     }
     static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
@@ -43,8 +45,8 @@ struct Launch {
 
     template <int MODEL, bool WALLS>
     static void macros2(const KP<R>& p, int parity, R* rho, R* u, R* phi, R* C, R* F, cudaStream_t st) {
-        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p.N), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
-        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p.N), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
+        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
+        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
     }
     static cudaError_t macros(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
                               void* F, cudaStream_t st) {
@@ -62,7 +64,7 @@ struct Launch {
 
     template <class LL, bool TOC>
     static void permute2(const KP<R>& p, int parity, int walls, R* slots, R* canon, int nl, cudaStream_t st) {
-        const unsigned g = grid_for(p.N);
+        const dim3 g = grid_for(p);
         if (parity) {
             if (walls) k_permute<R, LL, 1, true, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
             else k_permute<R, LL, 1, false, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
@@ -88,7 +90,7 @@ struct Launch {
 
     static cudaError_t init(const void* kp, int model, const InitArgs* ia, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
-        const unsigned g = grid_for(p.N);
+        const dim3 g = grid_for(p);
         switch (model) {
         case M_BGK: k_init<R, L, M_BGK><<<g, BLOCK, 0, st>>>(p, *ia); break;
         case M_SC1: k_init<R, L, M_SC1><<<g, BLOCK, 0, st>>>(p, *ia); break;

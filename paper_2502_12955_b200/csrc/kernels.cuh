@@ -61,29 +61,30 @@ template <int MODEL> struct ModelTraits {
 };
 
 // ------------------------------------------------------------------------------------------
-// neighbourhood of one cell: signed index offsets to coordinate -1 / 0 / +1 on each axis
-// (periodic wrap folded in) and the wall flags
+// Thread mapping: grid (ceil(nx/BLOCK), ny, nz), one block per segment of one x-row.  y and z are
+// block-uniform, so the row bases of the 9 (cy,cz) neighbour rows (periodic wrap folded in) live
+// in uniform registers; only x-1 / x / x+1 are per-thread.  An address is then
+// (uniform slot base + uniform row base) + per-thread x: no integer division, one add per access.
 // ------------------------------------------------------------------------------------------
 template <int D, bool WALLS>
 struct Nbr {
-    int cell;
-    int dx[3], dy[3], dz[3];
+    int cell;              // x + nx*(y + ny*z)
+    int xx[3];             // x-1, x, x+1 with periodic wrap (per thread)
+    int ry[3], rz[3];      // nx*y', nx*ny*z' for y' = y-1,y,y+1 / z' = z-1,z,z+1 with wrap (uniform)
     bool lo[3], hi[3];
 
     template <class R>
-    __device__ __forceinline__ Nbr(const KP<R>& p, int cell_) : cell(cell_) {
+    __device__ __forceinline__ Nbr(const KP<R>& p, int x, int y, int z) {
         const int nx = p.nx, ny = p.ny;
-        const int x = cell % nx, t = cell / nx;
-        int y, z;
-        if constexpr (D == 3) { y = t % ny; z = t / ny; } else { y = t; z = 0; }
-        dx[0] = (x == 0) ? nx - 1 : -1;          dx[1] = 0; dx[2] = (x == nx - 1) ? -(nx - 1) : 1;
-        dy[0] = ((y == 0) ? ny - 1 : -1) * nx;   dy[1] = 0; dy[2] = ((y == ny - 1) ? -(ny - 1) : 1) * nx;
+        xx[0] = (x == 0) ? nx - 1 : x - 1; xx[1] = x; xx[2] = (x == nx - 1) ? 0 : x + 1;
+        ry[0] = ((y == 0) ? ny - 1 : y - 1) * nx; ry[1] = y * nx; ry[2] = ((y == ny - 1) ? 0 : y + 1) * nx;
         if constexpr (D == 3) {
             const int nz = p.nz, sxy = nx * ny;
-            dz[0] = ((z == 0) ? nz - 1 : -1) * sxy; dz[1] = 0; dz[2] = ((z == nz - 1) ? -(nz - 1) : 1) * sxy;
+            rz[0] = ((z == 0) ? nz - 1 : z - 1) * sxy; rz[1] = z * sxy; rz[2] = ((z == nz - 1) ? 0 : z + 1) * sxy;
         } else {
-            dz[0] = dz[1] = dz[2] = 0;
+            rz[0] = rz[1] = rz[2] = 0;
         }
+        cell = rz[1] + ry[1] + x;
         if constexpr (WALLS) {
             lo[0] = p.bc[0] && x == 0; hi[0] = p.bc[0] && x == nx - 1;
             lo[1] = p.bc[1] && y == 0; hi[1] = p.bc[1] && y == ny - 1;
@@ -92,9 +93,13 @@ struct Nbr {
             lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
         }
     }
-    // index of the cell at offset (cx,cy,cz), components in {-1,0,1}
+    // uniform part / per-thread part of the index of the cell at offset (cx,cy,cz)
+    template <int CY, int CZ>
+    __device__ __forceinline__ int row() const { return rz[CZ + 1] + ry[CY + 1]; }
+    template <int CX>
+    __device__ __forceinline__ int col() const { return xx[CX + 1]; }
     template <int CX, int CY, int CZ>
-    __device__ __forceinline__ int at() const { return cell + dx[CX + 1] + dy[CY + 1] + dz[CZ + 1]; }
+    __device__ __forceinline__ int at() const { return row<CY, CZ>() + col<CX>(); }
     // does the offset cross a bounce-back wall?
     template <int CX, int CY, int CZ>
     __device__ __forceinline__ bool outside() const {
@@ -110,20 +115,25 @@ struct Nbr {
     }
 };
 
-// element index (relative to the lattice base) of P_I(x): where f_I(x,t) is read and
-// f*_{opp(I)}(x,t) is written
-template <class L, int PARITY, bool WALLS, int I, class NB>
-__device__ __forceinline__ size_t slot_of(const NB& nb, size_t N) {
+// the cell of this thread: false when the thread lies beyond the end of the row
+__device__ __forceinline__ bool thread_cell(int nx, int& x, int& y, int& z) {
+    x = blockIdx.x * BLOCK + threadIdx.x; y = blockIdx.y; z = blockIdx.z;
+    return x < nx;
+}
+
+// address of P_I(x): where f_I(x,t) is read and f*_{opp(I)}(x,t) is written
+template <class L, int PARITY, bool WALLS, int I, class R, class NB>
+__device__ __forceinline__ R* slot_of(R* base, const NB& nb, size_t N) {
     if constexpr (PARITY == 0 || I == 0) {
-        return (size_t)I * N + (size_t)nb.cell;
+        return (base + ((size_t)I * N + (size_t)nb.template row<0, 0>())) + nb.template col<0>();
     } else {
         constexpr int CX = -L::c(I, 0), CY = -L::c(I, 1), CZ = -L::c(I, 2);
-        const int src = nb.template at<CX, CY, CZ>();
+        R* nbr = (base + ((size_t)L::opp(I) * N + (size_t)nb.template row<CY, CZ>())) + nb.template col<CX>();
         if constexpr (WALLS) {
-            return nb.template outside<CX, CY, CZ>() ? (size_t)I * N + (size_t)nb.cell
-                                                     : (size_t)L::opp(I) * N + (size_t)src;
+            R* own = (base + ((size_t)I * N + (size_t)nb.template row<0, 0>())) + nb.template col<0>();
+            return nb.template outside<CX, CY, CZ>() ? own : nbr;
         } else {
-            return (size_t)L::opp(I) * N + (size_t)src;
+            return nbr;
         }
     }
 }
@@ -177,10 +187,10 @@ __device__ __forceinline__ R psi_of(R rho, int kind, R rho0) {
 }
 
 template <class L, int PARITY, bool WALLS, class R, class NB>
-__device__ __forceinline__ void load_pops(const R* __restrict__ base, const NB& nb, size_t N, R* fl) {
+__device__ __forceinline__ void load_pops(R* __restrict__ base, const NB& nb, size_t N, R* fl) {
     static_for<0, L::Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        fl[i] = base[slot_of<L, PARITY, WALLS, i>(nb, N)];
+        fl[i] = *slot_of<L, PARITY, WALLS, i>(base, nb, N);
     });
 }
 // writes fl[opp(i)] (post-collision) to P_i
@@ -188,7 +198,7 @@ template <class L, int PARITY, bool WALLS, class R, class NB>
 __device__ __forceinline__ void store_pops(R* __restrict__ base, const NB& nb, size_t N, const R* fl) {
     static_for<0, L::Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        base[slot_of<L, PARITY, WALLS, i>(nb, N)] = fl[L::opp(i)];
+        *slot_of<L, PARITY, WALLS, i>(base, nb, N) = fl[L::opp(i)];
     });
 }
 
@@ -202,7 +212,7 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
         static_for<1, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-            const R wp = (R)L::w(i) * __ldg(ps + nb.template at<CX, CY, CZ>());
+            const R wp = (R)L::w(i) * __ldg((ps + nb.template row<CY, CZ>()) + nb.template col<CX>());
             static_for<0, L::D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 constexpr int c = L::c(i, a);
@@ -358,10 +368,11 @@ __device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB
 template <class R, class L, int MODEL, int PARITY>
 __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
     constexpr int S = ModelTraits<MODEL>::S, Q = L::Q;
-    const int cell = blockIdx.x * BLOCK + threadIdx.x;
-    if (cell >= p.N) return;
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, false> nb(p, cell);
+    const Nbr<L::D, false> nb(p, x, y, z);
+    const int cell = nb.cell;
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         R fl[Q];
@@ -380,10 +391,11 @@ __global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p)
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q;
-    const int cell = blockIdx.x * BLOCK + threadIdx.x;
-    if (cell >= p.N) return;
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, WALLS> nb(p, cell);
+    const Nbr<L::D, WALLS> nb(p, x, y, z);
+    const int cell = nb.cell;
 
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
@@ -417,10 +429,11 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q, D = L::D;
-    const int cell = blockIdx.x * BLOCK + threadIdx.x;
-    if (cell >= p.N) return;
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<D, WALLS> nb(p, cell);
+    const Nbr<D, WALLS> nb(p, x, y, z);
+    const int cell = nb.cell;
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
@@ -458,18 +471,19 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
 template <class R, class L, int PARITY, bool WALLS, bool TO_CANONICAL>
 __global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R> p, R* __restrict__ slots,
                                                    R* __restrict__ canon, int n_lattices) {
-    const int cell = blockIdx.x * BLOCK + threadIdx.x;
-    if (cell >= p.N) return;
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, WALLS> nb(p, cell);
+    const Nbr<L::D, WALLS> nb(p, x, y, z);
+    const int cell = nb.cell;
     for (int s = 0; s < n_lattices; ++s) {
         R* sb = slots + (size_t)s * L::Q * N;
         R* cb = canon + (size_t)s * L::Q * N;
         static_for<0, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            const size_t P = slot_of<L, PARITY, WALLS, i>(nb, N);
-            if constexpr (TO_CANONICAL) cb[(size_t)i * N + cell] = sb[P];
-            else sb[P] = cb[(size_t)i * N + cell];
+            R* P = slot_of<L, PARITY, WALLS, i>(sb, nb, N);
+            if constexpr (TO_CANONICAL) cb[(size_t)i * N + cell] = *P;
+            else *P = cb[(size_t)i * N + cell];
         });
     }
 }
@@ -498,11 +512,11 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q, D = L::D;
-    const int cell = blockIdx.x * BLOCK + threadIdx.x;
-    if (cell >= p.N) return;
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
     const int nx = p.nx, ny = p.ny, nz = p.nz;
-    const int x = cell % nx, t = cell / nx, y = t % ny, z = t / ny;
+    const int cell = x + nx * (y + ny * z);
     const double PI = 3.14159265358979323846;
     double r0[2] = {ia.rho_init[0], ia.rho_init[1]};
     double u0[3] = {0.0, 0.0, 0.0};
