@@ -408,14 +408,18 @@ __global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p)
     CellMacro<R, L, MODEL> m;
     cell_macros<R, L, MODEL, FORCED>(p, nb, fl, m);
 
+    // the store addresses are recomputed from laundered column offsets instead of being kept in
+    // registers from the loads on (one 64-bit pair per slot otherwise)
+    Nbr<L::D, WALLS> ns = nb;
+    asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
-        store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
+        store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
     });
     if constexpr (MT::SCALAR) {
         collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
-        store_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+        store_pops<LS, PARITY, WALLS>(p.h, ns, N, hl);
     }
 }
 
