@@ -125,6 +125,24 @@ int lbm_set_populations(lbm_ctx* ctx, const void* f);
 int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
                  void* rho_host, void* u_host, void* phi_host, void* C_host);
 
+/* Shan-Chen models can advance a time step in ONE persistent launch: a schedule of psi rows (step a2)
+ * and step rows (a1, a3-a8) in which every psi row a step row needs comes earlier (DESIGN.md
+ * "Wavefront"), so the populations cross HBM once per step (Eq. 11 / 13 need psi of all neighbours at
+ * the same time level: PAPER.md:128, 136; R9).  lbm_set_wavefront(ctx, 1, rows_per_pencil, lead_rows)
+ * switches it on and (re)builds the schedule (values <= 0: defaults); (ctx, 0, 0, 0) returns to the
+ * two-launch path (psi pass, then fused step), the default.  Both paths compute the same bits.
+ * Synchronises the stream.  LBM_EINVAL when enabling it for LBM_BGK. */
+int lbm_set_wavefront(lbm_ctx* ctx, int enable, int rows_per_pencil, int lead_rows);
+
+/* The schedule the wavefront kernel would use for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1,
+ * ns = ny): *count items; if items != NULL (HOST, capacity items of 3 int32: kind 1 = psi row / 0 = step
+ * row, m, s) they are written out.  Host-only, needs no GPU. */
+int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity,
+                           size_t* count);
+
+/* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a wavefront wait timed out). */
+int lbm_check(lbm_ctx* ctx);
+
 /* number of time steps taken since init / set_populations */
 int64_t lbm_time(const lbm_ctx* ctx);
 

@@ -2,18 +2,30 @@
 #pragma once
 #include "dispatch.h"
 #include "kernels.cuh"
+#include "wave.cuh"
+#include <cstdlib>
 
 namespace lbm {
 
-// one block per BLOCK-cell segment of one x-row: grid (ceil(nx/BLOCK), ny, nz)
-template <class KPT>
-inline dim3 grid_for(const KPT& p) { return dim3((unsigned)((p.nx + BLOCK - 1) / BLOCK), (unsigned)p.ny, (unsigned)p.nz); }
+// threads per block: 128 (64 and 256 measured within 1 % for BGK, 256 slower for Shan-Chen), less for short rows
+template <class R>
+inline int block_for(const KP<R>& p) {
+    int b = 128;
+#ifdef LBM_TUNING
+    if (const char* e = getenv("LBM_BLOCK")) b = atoi(e);
+#endif
+    while (b > 32 && b / 2 >= p.nx) b /= 2;
+    return b;
+}
+// one block per segment of one x-row: grid (ceil(nx/block), ny, nz)
+template <class R>
+inline dim3 grid_for(const KP<R>& p) { const int b = block_for(p); return dim3((unsigned)((p.nx + b - 1) / b), (unsigned)p.ny, (unsigned)p.nz); }
 
 template <class R, class L>
 struct Launch {
     template <int MODEL, int PARITY>
     static void psi2(const KP<R>& p, cudaStream_t st) {
-        k_psi<R, L, MODEL, PARITY><<<grid_for(p), BLOCK, 0, st>>>(p);
+        k_psi<R, L, MODEL, PARITY><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
     static cudaError_t psi(const void* kp, int model, int parity, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
@@ -25,8 +37,8 @@ struct Launch {
 
     template <int MODEL, bool WALLS, bool FORCED>
     static void step3(const KP<R>& p, int parity, cudaStream_t st) {
-        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p), BLOCK, 0, st>>>(p);
-        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p), BLOCK, 0, st>>>(p);
+        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p), block_for(p), 0, st>>>(p);
+        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
     static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
@@ -45,8 +57,8 @@ struct Launch {
 
     template <int MODEL, bool WALLS>
     static void macros2(const KP<R>& p, int parity, R* rho, R* u, R* phi, R* C, R* F, cudaStream_t st) {
-        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
-        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p), BLOCK, 0, st>>>(p, rho, u, phi, C, F);
+        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p), block_for(p), 0, st>>>(p, rho, u, phi, C, F);
+        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p), block_for(p), 0, st>>>(p, rho, u, phi, C, F);
     }
     static cudaError_t macros(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
                               void* F, cudaStream_t st) {
@@ -66,10 +78,10 @@ struct Launch {
     static void permute2(const KP<R>& p, int parity, int walls, R* slots, R* canon, int nl, cudaStream_t st) {
         const dim3 g = grid_for(p);
         if (parity) {
-            if (walls) k_permute<R, LL, 1, true, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
-            else k_permute<R, LL, 1, false, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
+            if (walls) k_permute<R, LL, 1, true, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
+            else k_permute<R, LL, 1, false, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
         } else {
-            k_permute<R, LL, 0, false, TOC><<<g, BLOCK, 0, st>>>(p, slots, canon, nl);
+            k_permute<R, LL, 0, false, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
         }
     }
     static cudaError_t permute(const void* kp, int model, int parity, int walls, void* canon, int to_canonical,
@@ -92,17 +104,50 @@ struct Launch {
         const KP<R>& p = *(const KP<R>*)kp;
         const dim3 g = grid_for(p);
         switch (model) {
-        case M_BGK: k_init<R, L, M_BGK><<<g, BLOCK, 0, st>>>(p, *ia); break;
-        case M_SC1: k_init<R, L, M_SC1><<<g, BLOCK, 0, st>>>(p, *ia); break;
-        case M_SC2: k_init<R, L, M_SC2><<<g, BLOCK, 0, st>>>(p, *ia); break;
-        case M_SC2_ADE: k_init<R, L, M_SC2_ADE><<<g, BLOCK, 0, st>>>(p, *ia); break;
+        case M_BGK: k_init<R, L, M_BGK><<<g, block_for(p), 0, st>>>(p, *ia); break;
+        case M_SC1: k_init<R, L, M_SC1><<<g, block_for(p), 0, st>>>(p, *ia); break;
+        case M_SC2: k_init<R, L, M_SC2><<<g, block_for(p), 0, st>>>(p, *ia); break;
+        case M_SC2_ADE: k_init<R, L, M_SC2_ADE><<<g, block_for(p), 0, st>>>(p, *ia); break;
         default: return cudaErrorInvalidValue;
         }
         return cudaGetLastError();
     }
 
+    template <int MODEL>
+    static cudaError_t wave2(const KP<R>& p, int parity, const WaveArgs& wa, int blocks, cudaStream_t st) {
+        if (parity) k_wave<R, L, MODEL, 1><<<blocks, WAVE_SEG, 0, st>>>(p, wa);
+        else k_wave<R, L, MODEL, 0><<<blocks, WAVE_SEG, 0, st>>>(p, wa);
+        return cudaGetLastError();
+    }
+    static cudaError_t wave(const void* kp, int model, int parity, const WaveArgs* wa, int blocks, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        switch (model) {
+        case M_SC1: return wave2<M_SC1>(p, parity, *wa, blocks, st);
+        case M_SC2: return wave2<M_SC2>(p, parity, *wa, blocks, st);
+        case M_SC2_ADE: return wave2<M_SC2_ADE>(p, parity, *wa, blocks, st);
+        default: return cudaErrorInvalidValue;
+        }
+    }
+    template <int MODEL>
+    static int wave_blocks2(int parity) {
+        int per_sm = 0, dev = 0, sms = 0;
+        cudaError_t e = parity ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_wave<R, L, MODEL, 1>, WAVE_SEG, 0)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_wave<R, L, MODEL, 0>, WAVE_SEG, 0);
+        if (e != cudaSuccess || cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return 0; }
+        return per_sm * sms;
+    }
+    static int wave_blocks(int model, int parity) {
+        switch (model) {
+        case M_SC1: return wave_blocks2<M_SC1>(parity);
+        case M_SC2: return wave_blocks2<M_SC2>(parity);
+        case M_SC2_ADE: return wave_blocks2<M_SC2_ADE>(parity);
+        default: return 0;
+        }
+    }
+
     static const Ops* ops() {
-        static const Ops o = {&psi, &step, &macros, &permute, &init};
+        static const Ops o = {&psi, &step, &macros, &permute, &init, &wave, &wave_blocks};
         return &o;
     }
 };

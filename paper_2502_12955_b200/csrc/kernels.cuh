@@ -27,7 +27,7 @@ namespace lbm {
 enum { M_BGK = 0, M_SC1 = 1, M_SC2 = 2, M_SC2_ADE = 3 };
 enum { I_REST = 0, I_TAYLOR_GREEN = 1, I_DROPLET = 2, I_UNIFORM_NOISE = 3, I_RANDOM_DROPLETS = 4 };
 
-constexpr int BLOCK = 128;
+constexpr int BLOCK = 256;   // largest block any kernel is launched with; the launchers pick blockDim.x (inst.cuh)
 
 template <class R>
 struct KP {
@@ -61,7 +61,7 @@ template <int MODEL> struct ModelTraits {
 };
 
 // ------------------------------------------------------------------------------------------
-// Thread mapping: grid (ceil(nx/BLOCK), ny, nz), one block per segment of one x-row.  y and z are
+// Thread mapping: grid (ceil(nx/blockDim.x), ny, nz), one block per segment of one x-row.  y and z are
 // block-uniform, so the row bases of the 9 (cy,cz) neighbour rows (periodic wrap folded in) live
 // in uniform registers; only x-1 / x / x+1 are per-thread.  An address is then
 // (uniform slot base + uniform row base) + per-thread x: no integer division, one add per access.
@@ -117,7 +117,7 @@ struct Nbr {
 
 // the cell of this thread: false when the thread lies beyond the end of the row
 __device__ __forceinline__ bool thread_cell(int nx, int& x, int& y, int& z) {
-    x = blockIdx.x * BLOCK + threadIdx.x; y = blockIdx.y; z = blockIdx.z;
+    x = blockIdx.x * blockDim.x + threadIdx.x; y = blockIdx.y; z = blockIdx.z;
     return x < nx;
 }
 
@@ -203,7 +203,14 @@ __device__ __forceinline__ void store_pops(R* __restrict__ base, const NB& nb, s
 }
 
 // Shan-Chen stencil sums acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a}: Eq. 11 / 13
-template <class L, int S, class R, class NB>
+// COH: psi was written by other blocks of the SAME launch (wavefront kernel): read it from L2 (ld.global.cg),
+// never from a possibly stale L1 line; otherwise through the read-only path
+template <bool COH, class R>
+__device__ __forceinline__ R load_psi(const R* q) {
+    if constexpr (COH) return __ldcg(q); else return __ldg(q);
+}
+
+template <class L, int S, bool COH, class R, class NB>
 __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& nb, size_t N, R (*acc)[3]) {
     static_for<0, S>([&](auto tc) {
         constexpr int t = decltype(tc)::value;
@@ -212,7 +219,7 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
         static_for<1, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-            const R wp = (R)L::w(i) * __ldg((ps + nb.template row<CY, CZ>()) + nb.template col<CX>());
+            const R wp = (R)L::w(i) * load_psi<COH>((ps + nb.template row<CY, CZ>()) + nb.template col<CX>());
             static_for<0, L::D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 constexpr int c = L::c(i, a);
@@ -238,7 +245,7 @@ struct CellMacro {
 };
 
 // steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field
-template <class R, class L, int MODEL, bool FORCED, class NB>
+template <class R, class L, int MODEL, bool FORCED, bool COH = false, class NB>
 __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const R (*fl)[L::Q], CellMacro<R, L, MODEL>& m) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
@@ -254,11 +261,11 @@ __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const 
     m.inv_rho = (R)1 / rho_t;
     if constexpr (FORCED) {
         R acc[S][3];
-        if constexpr (SC) sc_stencil<L, S>(p.psi, nb, N, acc);
+        if constexpr (SC) sc_stencil<L, S, COH>(p.psi, nb, N, acc);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
             R psi_s = (R)0;
-            if constexpr (SC) psi_s = p.psi[(size_t)s * N + nb.cell];
+            if constexpr (SC) psi_s = load_psi<COH>(p.psi + ((size_t)s * N + nb.cell));
             static_for<0, D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 R Fa = (R)0;
@@ -365,11 +372,10 @@ __device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB
 // ------------------------------------------------------------------------------------------
 // psi pass (step a2): rho^sigma from the populations at the current parity, psi^sigma to HBM
 // ------------------------------------------------------------------------------------------
+// psi^sigma of the cell (x,y,z) at the current parity
 template <class R, class L, int MODEL, int PARITY>
-__global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
+__device__ __forceinline__ void psi_cell(const KP<R>& p, int x, int y, int z) {
     constexpr int S = ModelTraits<MODEL>::S, Q = L::Q;
-    int x, y, z;
-    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
     const Nbr<L::D, false> nb(p, x, y, z);
     const int cell = nb.cell;
@@ -383,19 +389,23 @@ __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) 
     });
 }
 
+template <class R, class L, int MODEL, int PARITY>
+__global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
+    psi_cell<R, L, MODEL, PARITY>(p, x, y, z);
+}
+
 // ------------------------------------------------------------------------------------------
 // fused step (a1, a3-a8): one thread per cell
 // ------------------------------------------------------------------------------------------
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED>
-__global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p) {
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false>
+__device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q;
-    int x, y, z;
-    if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
     const Nbr<L::D, WALLS> nb(p, x, y, z);
-    const int cell = nb.cell;
 
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
@@ -406,7 +416,7 @@ __global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p)
     if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
 
     CellMacro<R, L, MODEL> m;
-    cell_macros<R, L, MODEL, FORCED>(p, nb, fl, m);
+    cell_macros<R, L, MODEL, FORCED, COH>(p, nb, fl, m);
 
     // the store addresses are recomputed from laundered column offsets instead of being kept in
     // registers from the loads on (one 64-bit pair per slot otherwise)
@@ -421,6 +431,13 @@ __global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p)
         collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
         store_pops<LS, PARITY, WALLS>(p.h, ns, N, hl);
     }
+}
+
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED>
+__global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p) {
+    int x, y, z;
+    if (!thread_cell(p.nx, x, y, z)) return;
+    step_cell<R, L, MODEL, PARITY, WALLS, FORCED>(p, x, y, z);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -13,6 +13,7 @@
 
 #include "dispatch.h"
 #include "kernels.cuh"
+#include "wave.cuh"
 
 namespace {
 
@@ -116,6 +117,18 @@ struct lbm_ctx {
     // per-kernel timing (lbm_kernel_timing): event pairs around every launch of kind 0 (fused step) / 1 (psi pass)
     bool timing;
     std::vector<cudaEvent_t> ev[2];
+    // wavefront path of the Shan-Chen models (wave.cuh): psi pass + step in one persistent launch
+    bool wave_on;
+    int wave_py, wave_lead;           // schedule parameters in use
+    int wave_blocks[2];               // blocks per launch, by parity
+    lbm::WaveItem* wave_items;        // device copy of the schedule
+    long long wave_n_items;
+    int wave_nxs;
+    int* wave_flags;                  // one int per chunk, then the status word
+    size_t wave_n_chunks;
+    unsigned long long* wave_counter;
+    unsigned long long wave_base;
+    int wave_epoch;
 
     const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
 };
@@ -199,6 +212,78 @@ int run_psi(lbm_ctx* c) {
     return mark(c, 1);
 }
 
+void wave_free(lbm_ctx* c) {
+    if (c->wave_items) cudaFree(c->wave_items);
+    if (c->wave_flags) cudaFree(c->wave_flags);
+    if (c->wave_counter) cudaFree(c->wave_counter);
+    c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
+    c->wave_on = false;
+}
+
+// (re)build the schedule of the wavefront kernel and its device state; py / lead <= 0 pick the defaults
+int wave_setup(lbm_ctx* c, int py, int lead) {
+    CK(cudaStreamSynchronize(c->stream));
+    wave_free(c);
+    const Shape& sh = c->sh;
+    const int nm = sh.d == 3 ? c->ny : 1, ns = sh.d == 3 ? c->nz : c->ny;
+    const int nxs = (c->nx + lbm::WAVE_SEG - 1) / lbm::WAVE_SEG;
+    for (int par = 0; par < 2; ++par) {
+        c->wave_blocks[par] = c->ops->wave_blocks(c->model, par);
+        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "wavefront kernel: occupancy query failed");
+    }
+    if (py <= 0) {
+        // a pencil plane of about 4 MB of populations: psi item and step item of a row stay close in L2
+        const double row_bytes = (double)c->nx * (double)(sh.S * sh.Q + (sh.scalar ? sh.Qs : 0)) * (double)sh.B;
+        py = (int)(4.0e6 / row_bytes);
+    }
+    if (py < 1) py = 1;
+    if (py > nm) py = nm;
+    if (lead <= 0) lead = (c->wave_blocks[0] + 2 * nxs - 1) / (2 * nxs);   // psi items about half a wave of blocks ahead
+    if (lead < 1) lead = 1;
+    const std::vector<lbm::WaveItem> items = lbm::wave_schedule(nm, ns, py, lead);
+    c->wave_py = py; c->wave_lead = lead;
+    c->wave_n_items = (long long)items.size();
+    c->wave_nxs = nxs;
+    c->wave_n_chunks = (size_t)nm * ns * nxs;
+    cudaError_t e = cudaMalloc((void**)&c->wave_items, items.size() * sizeof(lbm::WaveItem));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_flags, (c->wave_n_chunks + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_counter, sizeof(unsigned long long));
+    if (e != cudaSuccess) { cudaGetLastError(); wave_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the wavefront schedule failed"); }
+    CK(cudaMemcpyAsync(c->wave_items, items.data(), items.size() * sizeof(lbm::WaveItem), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemsetAsync(c->wave_flags, 0, (c->wave_n_chunks + 1) * sizeof(int), c->stream));
+    CK(cudaMemsetAsync(c->wave_counter, 0, sizeof(unsigned long long), c->stream));
+    CK(cudaStreamSynchronize(c->stream));   // items goes out of scope
+    c->wave_base = 0;
+    c->wave_epoch = 0;
+    c->wave_on = true;
+    return 0;
+}
+
+int run_wave(lbm_ctx* c) {
+    const int parity = (int)(c->t & 1);
+    if (c->wave_epoch == 0x7fffffff) {   // epoch wrap: clear the flags (once per 2^31 - 1 launches)
+        CK(cudaMemsetAsync(c->wave_flags, 0, c->wave_n_chunks * sizeof(int), c->stream));
+        c->wave_epoch = 0;
+    }
+    lbm::WaveArgs wa;
+    wa.items = c->wave_items;
+    wa.n_tickets = c->wave_n_items * c->wave_nxs;
+    wa.nxs = c->wave_nxs;
+    wa.flags = c->wave_flags;
+    wa.counter = c->wave_counter;
+    wa.base = c->wave_base;
+    wa.epoch = ++c->wave_epoch;
+    wa.status = c->wave_flags + c->wave_n_chunks;
+    const int blocks = c->wave_blocks[parity];
+    int rc = mark(c, 0);
+    if (rc) return rc;
+    CK(c->ops->wave(c->kp(), c->model, parity, &wa, blocks, c->stream));
+    c->launches++;
+    // every block takes tickets until it draws one past the end: the counter ends at base + n_tickets + blocks
+    c->wave_base += (unsigned long long)wa.n_tickets + (unsigned long long)blocks;
+    return mark(c, 0);
+}
+
 int ensure_scratch(lbm_ctx* c, size_t bytes) {
     if (c->scratch_bytes >= bytes) return 0;
     if (c->scratch) { cudaFree(c->scratch); c->scratch = nullptr; c->scratch_bytes = 0; }
@@ -241,6 +326,8 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->inited = false; c->t = 0; c->launches = 0;
     c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
     c->timing = false;
+    c->wave_on = false; c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
+    c->wave_py = c->wave_lead = 0; c->wave_base = 0; c->wave_epoch = 0;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
         if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
@@ -275,6 +362,7 @@ void lbm_destroy(lbm_ctx* c) {
     drop_events(c);
     if (c->droplets_dev) cudaFree(c->droplets_dev);
     if (c->scratch) cudaFree(c->scratch);
+    wave_free(c);
     if (c->owns_ws && c->ws) cudaFree(c->ws);
     cudaGetLastError();
     delete c;
@@ -315,6 +403,11 @@ int lbm_step(lbm_ctx* c, int n) {
     for (int k = 0; k < n; ++k) {
         const int parity = (int)(c->t & 1);
         int rc;
+        if (c->wave_on) {   // Shan-Chen: psi pass + fused step in one persistent launch (wave.cuh)
+            if ((rc = run_wave(c))) return rc;
+            c->t++;
+            continue;
+        }
         if (c->sh.sc) {   // a2: psi of every cell at this time level (full-field barrier, R9)
             rc = run_psi(c);
             if (rc) return rc;
@@ -441,6 +534,46 @@ int lbm_kernel_time_ms(lbm_ctx* c, int kind, double* total_ms, int64_t* launches
     }
     *total_ms = sum;
     *launches = (int64_t)(v.size() / 2);
+    return 0;
+}
+
+int lbm_set_wavefront(lbm_ctx* c, int enable, int rows_per_pencil, int lead_rows) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (!c->sh.sc) return enable ? fail(LBM_EINVAL, "the wavefront path exists for the Shan-Chen models only") : 0;
+    DeviceGuard g(c->device);
+    if (!enable) {
+        CK(cudaStreamSynchronize(c->stream));
+        wave_free(c);
+        return 0;
+    }
+    return wave_setup(c, rows_per_pencil, lead_rows);
+}
+
+int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity, size_t* count) {
+    if (!count) return fail(LBM_EINVAL, "count is NULL");
+    if (nm < 1 || ns < 1) return fail(LBM_EINVAL, "nm and ns must be >= 1");
+    const std::vector<lbm::WaveItem> v = lbm::wave_schedule(nm, ns, rows_per_pencil, lead_rows);
+    *count = v.size();
+    if (items) {
+        if (capacity < v.size()) return fail(LBM_EINVAL, "capacity too small");
+        for (size_t k = 0; k < v.size(); ++k) {
+            items[3 * k + 0] = v[k].m < 0 ? 1 : 0;
+            items[3 * k + 1] = v[k].m & 0x7fffffff;
+            items[3 * k + 2] = v[k].s;
+        }
+    }
+    return 0;
+}
+
+int lbm_check(lbm_ctx* c) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    DeviceGuard g(c->device);
+    CK(cudaStreamSynchronize(c->stream));
+    if (c->wave_on) {
+        int st = 0;
+        CK(cudaMemcpy(&st, c->wave_flags + c->wave_n_chunks, sizeof(int), cudaMemcpyDeviceToHost));
+        if (st != 0) return fail(LBM_ECUDA, "wavefront kernel: a wait for published psi timed out; the state is invalid");
+    }
     return 0;
 }
 

@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_wavefront", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -75,6 +75,9 @@ def lib():
     L.lbm_get_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_set_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
+    L.lbm_set_wavefront.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+    L.lbm_wavefront_schedule.argtypes = [C.c_int] * 4 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
+    L.lbm_check.argtypes = [C.c_void_p]
     L.lbm_time.restype = C.c_int64
     L.lbm_time.argtypes = [C.c_void_p]
     L.lbm_launch_count.restype = C.c_int64
@@ -128,6 +131,21 @@ def make_params(**kw):
     p.workspace = None
     p.stream = None
     return p
+
+
+def wavefront_schedule(nm, ns, rows_per_pencil, lead_rows):
+    """The wavefront kernel's row schedule as an (n, 3) int32 array of (kind, m, s); host-only call."""
+    import numpy as np
+    L = lib()
+    n = C.c_size_t(0)
+    rc = L.lbm_wavefront_schedule(nm, ns, rows_per_pencil, lead_rows, None, 0, C.byref(n))
+    if rc != 0:
+        raise LbmError(rc, last_error())
+    out = np.zeros((n.value, 3), np.int32)
+    rc = L.lbm_wavefront_schedule(nm, ns, rows_per_pencil, lead_rows, out.ctypes.data, n.value, C.byref(n))
+    if rc != 0:
+        raise LbmError(rc, last_error())
+    return out
 
 
 def lattice_table(lattice, kind=0):
@@ -249,6 +267,14 @@ class LBM:
         ms, n = C.c_double(0.0), C.c_int64(0)
         self._chk(self.L.lbm_kernel_time_ms(self.h, int(kind), C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def set_wavefront(self, enable, rows_per_pencil=0, lead_rows=0):
+        """Shan-Chen models: one persistent launch per step (default) or psi pass + step (enable=False)"""
+        self._chk(self.L.lbm_set_wavefront(self.h, 1 if enable else 0, int(rows_per_pencil), int(lead_rows)))
+
+    def check(self):
+        """synchronise and raise on deferred device-side errors"""
+        self._chk(self.L.lbm_check(self.h))
 
     def synchronize(self):
         self.stream.synchronize()

@@ -150,3 +150,31 @@ def test_product_path_never_touches_the_oracle():
         if f.endswith((".py", ".cpp", ".h")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "liblbm" not in text and "kernels.cuh" not in text and "import paper_2502_12955_b200" not in text, f
+
+
+@pytest.mark.parametrize("nm,ns,py,lead", [(1, 1, 1, 0), (1, 7, 1, 1), (1, 64, 1, 5), (5, 4, 2, 3), (8, 8, 3, 0),
+                                           (8, 8, 8, 100), (2, 2, 1, 1), (3, 1, 2, 1), (16, 9, 5, 7), (6, 5, 100, 2)])
+def test_wavefront_schedule_is_valid(nm, ns, py, lead):
+    """Host logic of the wavefront kernel (wave_schedule.h): every row has exactly one psi item and one
+    step item, and every psi row a step row needs (itself and its 8 neighbours, periodic wrap) comes
+    EARLIER in the list -- the rule that makes the in-kernel waits deadlock-free and the results equal
+    to the two-pass order (psi of the whole field, then the step: DESIGN.md R9)."""
+    import paper_2502_12955_b200 as pkg
+    it = pkg.lbm.wavefront_schedule(nm, ns, py, lead)
+    assert it.shape == (2 * nm * ns, 3)
+    pos_psi, pos_step = {}, {}
+    for k, (kind, m, s) in enumerate(it.tolist()):
+        assert 0 <= m < nm and 0 <= s < ns
+        d = pos_psi if kind == 1 else pos_step
+        assert (m, s) not in d
+        d[(m, s)] = k
+    assert len(pos_psi) == nm * ns and len(pos_step) == nm * ns
+    for (m, s), k in pos_step.items():
+        for dm in (-1, 0, 1):
+            for ds in (-1, 0, 1):
+                assert pos_psi[((m + dm) % nm, (s + ds) % ns)] < k
+    # step rows march through pencils of py rows along s
+    steps = [(m, s) for kind, m, s in it.tolist() if kind == 0]
+    p = max(1, min(py, nm))
+    expect = [(m, s) for m0 in range(0, nm, p) for s in range(ns) for m in range(m0, min(m0 + p, nm))]
+    assert steps == expect

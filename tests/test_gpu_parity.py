@@ -359,3 +359,38 @@ def test_errors_and_state(gpu):
         gpu.LBM(8, 8, 2, "D2Q9", "BGK")               # D2Q9 needs nz == 1
     with pytest.raises(gpu.LbmError):
         gpu.LBM(8, 8, 1, "D2Q9", "SC1", bc=(1, 0, 0))  # Shan-Chen + walls: not implemented
+
+
+@pytest.mark.parametrize("name,grid,over", [
+    ("cfg2", (300, 21, 1), dict(radius=6.0)),
+    ("cfg3", (260, 37, 1), {}),
+    ("cfg3", (130, 5, 1), dict(precision=32)),
+    ("cfg5", (140, 9, 7), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
+    ("cfg5", (16, 3, 2), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
+    ("cfg5", (9, 1, 1), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
+], ids=lambda v: str(v).replace(" ", ""))
+@pytest.mark.parametrize("wave", [None, (1, 1), (3, 2), (1000, 100000)], ids=lambda v: "wave%s" % (v,))
+def test_wavefront_and_two_launch_paths_match_oracle(gpu, name, grid, over, wave):
+    """Shan-Chen models: the one-launch wavefront path (several schedules: pencils of 1 / 3 / all rows,
+    psi rows 1 / 2 / all rows ahead) and the two-launch path (psi pass, then step) against the oracle
+    at every step 1..7, on rows of several x-segments with a ragged tail and on degenerate extents."""
+    cfg = workloads.config(name, grid=grid, **over)
+    ref, dev = make_pair(gpu, cfg)
+    if wave is None:
+        dev.set_wavefront(False)
+    else:
+        dev.set_wavefront(True, *wave)
+    ref.init_from_seed(9)
+    dev.set_populations(torch.from_numpy(ref.get_populations()))
+    exact = not (cfg["model"] == "SC1" and cfg["params"].get("psi_kind", 0) == 0)
+    for step in range(1, 8):
+        ref.step(1)
+        dev.step(1)
+        fr = ref.get_populations()
+        fd = dev.get_populations().cpu().numpy()
+        if exact:
+            assert np.array_equal(fr, fd), "step %d" % step
+        else:
+            assert np.abs(fr - fd).max() <= 1e-13 * np.abs(fr).max(), "step %d" % step
+    dev.check()
+    assert dev.launch_count() >= 7
