@@ -163,13 +163,15 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------
 # GPU arm
 # --------------------------------------------------------------------------------------------
-def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None):
+def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None, path=None):
     """Times `steps` time steps with populations resident in HBM.  Returns a dict with the elapsed
     ms (CUDA events on the context's stream), the per-kernel device times measured with event pairs
     around every launch in a second pass of the same length, and the launch count."""
     import torch
     import paper_2502_12955_b200 as lbm
     sim = lbm.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], device=device, **cfg["params"])
+    if path is not None:
+        sim.set_path(*path)
     sim.init_from_seed(seed)
     sim.step(warmup)
     sim.synchronize()
@@ -363,6 +365,8 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(workloads.CONFIGS))
     ap.add_argument("--precision", type=int, default=None, choices=[32, 64])
     ap.add_argument("--grid", type=int, nargs=3, default=None, help="override the grid (profiling runs)")
+    ap.add_argument("--path", default=None, help="register | wavefront | pipeline[:rows_per_pencil:lead_rows] "
+                    "(default: the library's choice)")
     ap.add_argument("--no-extras", action="store_true", help="skip per_model, e2e and cpu_baseline (profiling runs)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -396,7 +400,12 @@ def main():
     peak, peak_kind = measured_peak()
     sampler = ClockSampler(index=local) if rank == 0 else None
     # replicas only: rank r runs its own seeded copy of the workload (no data-path collective)
-    r = time_device(cfg, args.steps, args.warmup, device, seed=replica_seed(rank), sampler=sampler, barrier=barrier)
+    path = None
+    if args.path:
+        pp = args.path.split(":")
+        path = (pp[0], int(pp[1]) if len(pp) > 1 else 0, int(pp[2]) if len(pp) > 2 else 0)
+    r = time_device(cfg, args.steps, args.warmup, device, seed=replica_seed(rank), sampler=sampler, barrier=barrier,
+                    path=path)
     ms = max_over_ranks(r["ms"], dist, device)
     s = shape_of(cfg)
     step_b, psi_b = algorithmic_bytes(cfg)

@@ -125,22 +125,32 @@ int lbm_set_populations(lbm_ctx* ctx, const void* f);
 int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
                  void* rho_host, void* u_host, void* phi_host, void* C_host);
 
-/* Shan-Chen models can advance a time step in ONE persistent launch: a schedule of psi rows (step a2)
- * and step rows (a1, a3-a8) in which every psi row a step row needs comes earlier (DESIGN.md
- * "Wavefront"), so the populations cross HBM once per step (Eq. 11 / 13 need psi of all neighbours at
- * the same time level: PAPER.md:128, 136; R9).  lbm_set_wavefront(ctx, 1, rows_per_pencil, lead_rows)
- * switches it on and (re)builds the schedule (values <= 0: defaults); (ctx, 0, 0, 0) returns to the
- * two-launch path (psi pass, then fused step), the default.  Both paths compute the same bits.
- * Synchronises the stream.  LBM_EINVAL when enabling it for LBM_BGK. */
-int lbm_set_wavefront(lbm_ctx* ctx, int enable, int rows_per_pencil, int lead_rows);
+/* Which kernels lbm_step launches.  All paths compute the same bits (same expression tree per cell).
+ *   LBM_PATH_REGISTER   one thread per cell, populations loaded straight into registers: one launch of the
+ *                       fused step kernel per time step, preceded by the psi pass for Shan-Chen models.
+ *                       Works for every shape and boundary.
+ *   LBM_PATH_PIPELINE   ONE persistent launch per time step: a ticket counter hands out 128-cell row segments
+ *                       whose populations (and psi tile) are staged in shared memory by 16-byte asynchronous
+ *                       copies, double buffered.  Shan-Chen models run psi segments (step a2) and step
+ *                       segments (a1, a3-a8) in the same launch, ordered so that every psi value a step
+ *                       segment needs was published by a lower ticket (Eq. 11 / 13 need psi of all neighbours
+ *                       at the same time level: PAPER.md:128, 136; R9): the populations cross HBM once per
+ *                       step, the second read hits L2.  Needs nx * sizeof(value) % 16 == 0 and periodic x
+ *                       (LBM_EINVAL otherwise).
+ * lbm_create starts with LBM_PATH_REGISTER.
+ * rows_per_pencil / lead_rows: schedule parameters of the pipelined path for Shan-Chen models (<= 0: defaults; DESIGN.md
+ * "Wavefront").  Synchronises the stream. */
+enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1 };
+int lbm_set_path(lbm_ctx* ctx, int path, int rows_per_pencil, int lead_rows);
+int lbm_get_path(const lbm_ctx* ctx);
 
-/* The schedule the wavefront kernel would use for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1,
+/* The row schedule of the pipelined path for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1,
  * ns = ny): *count items; if items != NULL (HOST, capacity items of 3 int32: kind 1 = psi row / 0 = step
  * row, m, s) they are written out.  Host-only, needs no GPU. */
 int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity,
                            size_t* count);
 
-/* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a wavefront wait timed out). */
+/* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a wait for published psi timed out). */
 int lbm_check(lbm_ctx* ctx);
 
 /* number of time steps taken since init / set_populations */

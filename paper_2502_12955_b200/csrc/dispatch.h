@@ -7,7 +7,7 @@
 namespace lbm {
 
 struct InitArgs;
-struct WaveArgs;
+struct PipeArgs;
 
 struct Ops {
     // kp points at a KP<R> of the matching precision
@@ -19,10 +19,10 @@ struct Ops {
     cudaError_t (*permute)(const void* kp, int model, int parity, int walls, void* canon, int to_canonical,
                            cudaStream_t st);
     cudaError_t (*init)(const void* kp, int model, const InitArgs* ia, cudaStream_t st);
-    // psi pass + fused step of one time step in one persistent launch (Shan-Chen models, wave.cuh);
-    // wave_blocks: how many blocks to launch (resident blocks per SM x SMs of the current device)
-    cudaError_t (*wave)(const void* kp, int model, int parity, const WaveArgs* wa, int blocks, cudaStream_t st);
-    int (*wave_blocks)(int model, int parity);
+    // pipelined persistent kernel (pipe.cuh); walls: bounce-back walls in y and / or z (x must be periodic)
+    cudaError_t (*pipe)(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
+                        cudaStream_t st);
+    int (*pipe_blocks)(int model, int parity, int walls, int forced);
 };
 
 const Ops* ops_f64_d2q9();

@@ -2,7 +2,7 @@
 #pragma once
 #include "dispatch.h"
 #include "kernels.cuh"
-#include "wave.cuh"
+#include "pipe.cuh"
 #include <cstdlib>
 
 namespace lbm {
@@ -113,41 +113,59 @@ struct Launch {
         return cudaGetLastError();
     }
 
-    template <int MODEL>
-    static cudaError_t wave2(const KP<R>& p, int parity, const WaveArgs& wa, int blocks, cudaStream_t st) {
-        if (parity) k_wave<R, L, MODEL, 1><<<blocks, WAVE_SEG, 0, st>>>(p, wa);
-        else k_wave<R, L, MODEL, 0><<<blocks, WAVE_SEG, 0, st>>>(p, wa);
+    // pipelined kernel: blocks == 0 -> only return the number of co-resident blocks through *out_blocks
+    template <int MODEL, bool WALLYZ, bool FORCED>
+    static cudaError_t pipe3(const KP<R>& p, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
+        constexpr size_t smem = pipe_smem_bytes<R, L, MODEL>();
+        auto k0 = k_pipe<R, L, MODEL, 0, WALLYZ, FORCED>;
+        auto k1 = k_pipe<R, L, MODEL, 1, WALLYZ, FORCED>;
+        auto k = parity ? k1 : k0;
+        static bool attr_set[2] = {false, false};
+        if (!attr_set[parity]) {
+            cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            attr_set[parity] = true;
+        }
+        if (out_blocks) {
+            int per_sm = 0, dev = 0, sms = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PIPE_TX, smem);
+            if (e == cudaSuccess) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess) return e;
+            *out_blocks = per_sm * sms;
+            return cudaSuccess;
+        }
+        k<<<blocks, PIPE_TX, smem, st>>>(p, *wa);
         return cudaGetLastError();
     }
-    static cudaError_t wave(const void* kp, int model, int parity, const WaveArgs* wa, int blocks, cudaStream_t st) {
+    static cudaError_t pipe_any(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
+                                cudaStream_t st, int* out_blocks) {
         const KP<R>& p = *(const KP<R>*)kp;
         switch (model) {
-        case M_SC1: return wave2<M_SC1>(p, parity, *wa, blocks, st);
-        case M_SC2: return wave2<M_SC2>(p, parity, *wa, blocks, st);
-        case M_SC2_ADE: return wave2<M_SC2_ADE>(p, parity, *wa, blocks, st);
+        case M_BGK:
+            if (walls) return forced ? pipe3<M_BGK, true, true>(p, parity, wa, blocks, st, out_blocks)
+                                     : pipe3<M_BGK, true, false>(p, parity, wa, blocks, st, out_blocks);
+            return forced ? pipe3<M_BGK, false, true>(p, parity, wa, blocks, st, out_blocks)
+                          : pipe3<M_BGK, false, false>(p, parity, wa, blocks, st, out_blocks);
+        case M_SC1: return pipe3<M_SC1, false, true>(p, parity, wa, blocks, st, out_blocks);
+        case M_SC2: return pipe3<M_SC2, false, true>(p, parity, wa, blocks, st, out_blocks);
+        case M_SC2_ADE: return pipe3<M_SC2_ADE, false, true>(p, parity, wa, blocks, st, out_blocks);
         default: return cudaErrorInvalidValue;
         }
     }
-    template <int MODEL>
-    static int wave_blocks2(int parity) {
-        int per_sm = 0, dev = 0, sms = 0;
-        cudaError_t e = parity ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_wave<R, L, MODEL, 1>, WAVE_SEG, 0)
-                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_wave<R, L, MODEL, 0>, WAVE_SEG, 0);
-        if (e != cudaSuccess || cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return 0; }
-        return per_sm * sms;
+    static cudaError_t pipe(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
+                            cudaStream_t st) {
+        return pipe_any(kp, model, parity, walls, forced, wa, blocks, st, nullptr);
     }
-    static int wave_blocks(int model, int parity) {
-        switch (model) {
-        case M_SC1: return wave_blocks2<M_SC1>(parity);
-        case M_SC2: return wave_blocks2<M_SC2>(parity);
-        case M_SC2_ADE: return wave_blocks2<M_SC2_ADE>(parity);
-        default: return 0;
-        }
+    static int pipe_blocks(int model, int parity, int walls, int forced) {
+        int b = 0;
+        KP<R> dummy{};
+        if (pipe_any(&dummy, model, parity, walls, forced, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
+        return b;
     }
 
     static const Ops* ops() {
-        static const Ops o = {&psi, &step, &macros, &permute, &init, &wave, &wave_blocks};
+        static const Ops o = {&psi, &step, &macros, &permute, &init, &pipe, &pipe_blocks};
         return &o;
     }
 };

@@ -244,12 +244,13 @@ struct CellMacro {
     R inv_rho;
 };
 
-// steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field
-template <class R, class L, int MODEL, bool FORCED, bool COH = false, class NB>
-__device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const R (*fl)[L::Q], CellMacro<R, L, MODEL>& m) {
+// steps a1, a3 (given the stencil sums), a4: moments, force, barycentric velocity.
+// acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a} and psi_own[s] = psi^s(x) are read only for Shan-Chen models.
+template <class R, class L, int MODEL, bool FORCED>
+__device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L::Q], const R (*acc)[3], const R* psi_own,
+                                                 CellMacro<R, L, MODEL>& m) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
-    const size_t N = (size_t)p.N;
     R j[S][3];
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
@@ -260,19 +261,15 @@ __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const 
     if constexpr (S == 2) rho_t = rho_t + m.rho[1];
     m.inv_rho = (R)1 / rho_t;
     if constexpr (FORCED) {
-        R acc[S][3];
-        if constexpr (SC) sc_stencil<L, S, COH>(p.psi, nb, N, acc);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
-            R psi_s = (R)0;
-            if constexpr (SC) psi_s = load_psi<COH>(p.psi + ((size_t)s * N + nb.cell));
             static_for<0, D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 R Fa = (R)0;
                 if constexpr (SC) {
                     R t = p.G[s][0] * acc[0][a];
                     if constexpr (S == 2) t = t + p.G[s][1] * acc[1][a];
-                    Fa = -(psi_s * t);
+                    Fa = -(psi_own[s] * t);
                 }
                 // constant body-force density, split by mass fraction for S = 2 (R5)
                 R Fext;
@@ -294,6 +291,23 @@ __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const 
             m.u[a] = jt * m.inv_rho;
         }
     });
+}
+
+// steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field in global memory
+template <class R, class L, int MODEL, bool FORCED, bool COH = false, class NB>
+__device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const R (*fl)[L::Q], CellMacro<R, L, MODEL>& m) {
+    constexpr int S = ModelTraits<MODEL>::S;
+    constexpr bool SC = ModelTraits<MODEL>::SC;
+    const size_t N = (size_t)p.N;
+    R acc[S][3], psi_own[S];
+    if constexpr (FORCED && SC) {
+        sc_stencil<L, S, COH>(p.psi, nb, N, acc);
+        static_for<0, S>([&](auto sc) {
+            constexpr int s = decltype(sc)::value;
+            psi_own[s] = load_psi<COH>(p.psi + ((size_t)s * N + nb.cell));
+        });
+    }
+    cell_macros_core<R, L, MODEL, FORCED>(p, fl, acc, psi_own, m);
 }
 
 // step a5 for one component: f* = f - (f - f^eq)/tau + (1 - 1/(2 tau)) F_i

@@ -13,7 +13,7 @@
 
 #include "dispatch.h"
 #include "kernels.cuh"
-#include "wave.cuh"
+#include "pipe.cuh"
 
 namespace {
 
@@ -117,11 +117,11 @@ struct lbm_ctx {
     // per-kernel timing (lbm_kernel_timing): event pairs around every launch of kind 0 (fused step) / 1 (psi pass)
     bool timing;
     std::vector<cudaEvent_t> ev[2];
-    // wavefront path of the Shan-Chen models (wave.cuh): psi pass + step in one persistent launch
-    bool wave_on;
+    // pipelined persistent path (pipe.cuh): one ticketed launch per time step
+    int path;                         // LBM_PATH_*: which kernels lbm_step launches
     int wave_py, wave_lead;           // schedule parameters in use
     int wave_blocks[2];               // blocks per launch, by parity
-    lbm::WaveItem* wave_items;        // device copy of the schedule
+    lbm::PipeItem* wave_items;        // device copy of the schedule, one entry per ticket
     long long wave_n_items;
     int wave_nxs;
     int* wave_flags;                  // one int per chunk, then the status word
@@ -217,57 +217,81 @@ void wave_free(lbm_ctx* c) {
     if (c->wave_flags) cudaFree(c->wave_flags);
     if (c->wave_counter) cudaFree(c->wave_counter);
     c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
-    c->wave_on = false;
+    c->path = LBM_PATH_REGISTER;
 }
 
-// (re)build the schedule of the wavefront kernel and its device state; py / lead <= 0 pick the defaults
-int wave_setup(lbm_ctx* c, int py, int lead) {
+bool pipe_eligible(const lbm_ctx* c) {
+    return ((size_t)c->nx * c->sh.B) % 16 == 0 && c->p.bc[0] == 0;
+}
+
+// Switch to the pipelined path: (re)build the schedule (one entry per ticket) and the device state of the
+// ticket counter; py / lead <= 0 pick the defaults
+int path_setup(lbm_ctx* c, int py, int lead) {
     CK(cudaStreamSynchronize(c->stream));
     wave_free(c);
     const Shape& sh = c->sh;
     const int nm = sh.d == 3 ? c->ny : 1, ns = sh.d == 3 ? c->nz : c->ny;
-    const int nxs = (c->nx + lbm::WAVE_SEG - 1) / lbm::WAVE_SEG;
+    const int nxs = (c->nx + lbm::PIPE_TX - 1) / lbm::PIPE_TX;
     for (int par = 0; par < 2; ++par) {
-        c->wave_blocks[par] = c->ops->wave_blocks(c->model, par);
-        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "wavefront kernel: occupancy query failed");
+        c->wave_blocks[par] = c->ops->pipe_blocks(c->model, par, c->walls, c->forced);
+        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "pipelined kernel: occupancy query failed");
     }
-    if (py <= 0) {
-        // a pencil plane of about 4 MB of populations: psi item and step item of a row stay close in L2
-        const double row_bytes = (double)c->nx * (double)(sh.S * sh.Q + (sh.scalar ? sh.Qs : 0)) * (double)sh.B;
-        py = (int)(4.0e6 / row_bytes);
+    std::vector<lbm::WaveItem> rows;
+    if (sh.sc) {
+        if (py <= 0) {
+            // a pencil plane of about 4 MB of populations: psi item and step item of a row stay close in L2
+            const double row_bytes = (double)c->nx * (double)(sh.S * sh.Q + (sh.scalar ? sh.Qs : 0)) * (double)sh.B;
+            py = (int)(4.0e6 / row_bytes);
+        }
+        if (py < 1) py = 1;
+        if (py > nm) py = nm;
+        if (lead <= 0) lead = (2 * c->wave_blocks[0] + nxs - 1) / nxs;   // psi items about two waves of blocks ahead
+        if (lead < 1) lead = 1;
+        rows = lbm::wave_schedule(nm, ns, py, lead);
+        c->wave_py = py; c->wave_lead = lead;
+    } else {
+        c->wave_py = c->wave_lead = 0;
+        rows.reserve((size_t)nm * ns);
+        for (int s = 0; s < ns; ++s)
+            for (int m = 0; m < nm; ++m) rows.push_back(lbm::WaveItem{m, s});     // step rows only
     }
-    if (py < 1) py = 1;
-    if (py > nm) py = nm;
-    if (lead <= 0) lead = (c->wave_blocks[0] + 2 * nxs - 1) / (2 * nxs);   // psi items about half a wave of blocks ahead
-    if (lead < 1) lead = 1;
-    const std::vector<lbm::WaveItem> items = lbm::wave_schedule(nm, ns, py, lead);
-    c->wave_py = py; c->wave_lead = lead;
+    if ((double)rows.size() * nxs > 2.0e9) return fail(LBM_EINVAL, "pipelined path: more than 2e9 tickets");
+    std::vector<lbm::PipeItem> items;
+    items.reserve(rows.size() * (size_t)nxs);
+    for (const lbm::WaveItem& r : rows) {
+        const int m = r.m & 0x7fffffff;
+        lbm::PipeItem it;
+        it.kind = r.m < 0 ? lbm::ITEM_PSI : lbm::ITEM_STEP;
+        it.y = sh.d == 3 ? m : r.s;
+        it.z = sh.d == 3 ? r.s : 0;
+        for (int xs = 0; xs < nxs; ++xs) { it.xs = xs; items.push_back(it); }
+    }
     c->wave_n_items = (long long)items.size();
     c->wave_nxs = nxs;
     c->wave_n_chunks = (size_t)nm * ns * nxs;
-    cudaError_t e = cudaMalloc((void**)&c->wave_items, items.size() * sizeof(lbm::WaveItem));
+    cudaError_t e = cudaMalloc((void**)&c->wave_items, items.size() * sizeof(lbm::PipeItem));
     if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_flags, (c->wave_n_chunks + 1) * sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_counter, sizeof(unsigned long long));
-    if (e != cudaSuccess) { cudaGetLastError(); wave_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the wavefront schedule failed"); }
-    CK(cudaMemcpyAsync(c->wave_items, items.data(), items.size() * sizeof(lbm::WaveItem), cudaMemcpyHostToDevice, c->stream));
+    if (e != cudaSuccess) { cudaGetLastError(); wave_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
+    CK(cudaMemcpyAsync(c->wave_items, items.data(), items.size() * sizeof(lbm::PipeItem), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemsetAsync(c->wave_flags, 0, (c->wave_n_chunks + 1) * sizeof(int), c->stream));
     CK(cudaMemsetAsync(c->wave_counter, 0, sizeof(unsigned long long), c->stream));
     CK(cudaStreamSynchronize(c->stream));   // items goes out of scope
     c->wave_base = 0;
     c->wave_epoch = 0;
-    c->wave_on = true;
+    c->path = LBM_PATH_PIPELINE;
     return 0;
 }
 
-int run_wave(lbm_ctx* c) {
+int run_pipe(lbm_ctx* c) {
     const int parity = (int)(c->t & 1);
     if (c->wave_epoch == 0x7fffffff) {   // epoch wrap: clear the flags (once per 2^31 - 1 launches)
         CK(cudaMemsetAsync(c->wave_flags, 0, c->wave_n_chunks * sizeof(int), c->stream));
         c->wave_epoch = 0;
     }
-    lbm::WaveArgs wa;
+    lbm::PipeArgs wa;
     wa.items = c->wave_items;
-    wa.n_tickets = c->wave_n_items * c->wave_nxs;
+    wa.n_tickets = (unsigned)c->wave_n_items;
     wa.nxs = c->wave_nxs;
     wa.flags = c->wave_flags;
     wa.counter = c->wave_counter;
@@ -277,10 +301,10 @@ int run_wave(lbm_ctx* c) {
     const int blocks = c->wave_blocks[parity];
     int rc = mark(c, 0);
     if (rc) return rc;
-    CK(c->ops->wave(c->kp(), c->model, parity, &wa, blocks, c->stream));
+    CK(c->ops->pipe(c->kp(), c->model, parity, c->walls, c->forced, &wa, blocks, c->stream));
+    // every block draws tickets until three of them lie past the end (pipe.cuh)
+    c->wave_base += (unsigned long long)wa.n_tickets + 3ULL * (unsigned long long)blocks;
     c->launches++;
-    // every block takes tickets until it draws one past the end: the counter ends at base + n_tickets + blocks
-    c->wave_base += (unsigned long long)wa.n_tickets + (unsigned long long)blocks;
     return mark(c, 0);
 }
 
@@ -326,7 +350,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->inited = false; c->t = 0; c->launches = 0;
     c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
     c->timing = false;
-    c->wave_on = false; c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
+    c->path = LBM_PATH_REGISTER; c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
     c->wave_py = c->wave_lead = 0; c->wave_base = 0; c->wave_epoch = 0;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
@@ -403,8 +427,8 @@ int lbm_step(lbm_ctx* c, int n) {
     for (int k = 0; k < n; ++k) {
         const int parity = (int)(c->t & 1);
         int rc;
-        if (c->wave_on) {   // Shan-Chen: psi pass + fused step in one persistent launch (wave.cuh)
-            if ((rc = run_wave(c))) return rc;
+        if (c->path != LBM_PATH_REGISTER) {   // one persistent ticketed launch per step (pipe.cuh)
+            if ((rc = run_pipe(c))) return rc;
             c->t++;
             continue;
         }
@@ -537,17 +561,21 @@ int lbm_kernel_time_ms(lbm_ctx* c, int kind, double* total_ms, int64_t* launches
     return 0;
 }
 
-int lbm_set_wavefront(lbm_ctx* c, int enable, int rows_per_pencil, int lead_rows) {
+int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
-    if (!c->sh.sc) return enable ? fail(LBM_EINVAL, "the wavefront path exists for the Shan-Chen models only") : 0;
     DeviceGuard g(c->device);
-    if (!enable) {
+    if (path == LBM_PATH_REGISTER) {
         CK(cudaStreamSynchronize(c->stream));
         wave_free(c);
         return 0;
     }
-    return wave_setup(c, rows_per_pencil, lead_rows);
+    if (path != LBM_PATH_PIPELINE) return fail(LBM_EINVAL, "unknown path");
+    if (!pipe_eligible(c))
+        return fail(LBM_EINVAL, "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes and periodic x");
+    return path_setup(c, rows_per_pencil, lead_rows);
 }
+
+int lbm_get_path(const lbm_ctx* c) { return c ? c->path : LBM_EINVAL; }
 
 int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity, size_t* count) {
     if (!count) return fail(LBM_EINVAL, "count is NULL");
@@ -569,10 +597,10 @@ int lbm_check(lbm_ctx* c) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
     DeviceGuard g(c->device);
     CK(cudaStreamSynchronize(c->stream));
-    if (c->wave_on) {
+    if (c->path != LBM_PATH_REGISTER) {
         int st = 0;
         CK(cudaMemcpy(&st, c->wave_flags + c->wave_n_chunks, sizeof(int), cudaMemcpyDeviceToHost));
-        if (st != 0) return fail(LBM_ECUDA, "wavefront kernel: a wait for published psi timed out; the state is invalid");
+        if (st != 0) return fail(LBM_ECUDA, "persistent kernel: a wait for published psi timed out; the state is invalid");
     }
     return 0;
 }

@@ -1,4 +1,4 @@
-// Host-side schedule of the wavefront kernel (wave.cuh): the order in which one launch works through the
+// Host-side row schedule of the pipelined kernel (pipe.cuh): the order in which one launch works through the
 // psi rows (step a2) and the step rows (a1, a3-a8) of one time step of a Shan-Chen model.
 //
 // Why: psi^sigma(x + c_i, t) must be known for all neighbours before cell x is collided (Eq. 11 / 13,

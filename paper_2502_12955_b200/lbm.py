@@ -17,11 +17,12 @@ LATTICES = {"D2Q9": D2Q9, "D3Q19": D3Q19}
 MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE}
 INITS = {"REST": 0, "TAYLOR_GREEN": 1, "DROPLET": 2, "UNIFORM_NOISE": 3, "RANDOM_DROPLETS": 4}
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+PATHS = {"register": 0, "pipeline": 1}
 
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_set_wavefront", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -75,7 +76,8 @@ def lib():
     L.lbm_get_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_set_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
-    L.lbm_set_wavefront.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+    L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+    L.lbm_get_path.argtypes = [C.c_void_p]
     L.lbm_wavefront_schedule.argtypes = [C.c_int] * 4 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
     L.lbm_check.argtypes = [C.c_void_p]
     L.lbm_time.restype = C.c_int64
@@ -268,9 +270,13 @@ class LBM:
         self._chk(self.L.lbm_kernel_time_ms(self.h, int(kind), C.byref(ms), C.byref(n)))
         return ms.value, n.value
 
-    def set_wavefront(self, enable, rows_per_pencil=0, lead_rows=0):
-        """Shan-Chen models: one persistent launch per step (default) or psi pass + step (enable=False)"""
-        self._chk(self.L.lbm_set_wavefront(self.h, 1 if enable else 0, int(rows_per_pencil), int(lead_rows)))
+    def set_path(self, path, rows_per_pencil=0, lead_rows=0):
+        """which kernels step() launches: "register" or "pipeline" (include/lbm.h)"""
+        path = PATHS[path] if isinstance(path, str) else int(path)
+        self._chk(self.L.lbm_set_path(self.h, path, int(rows_per_pencil), int(lead_rows)))
+
+    def get_path(self):
+        return {v: k for k, v in PATHS.items()}[self.L.lbm_get_path(self.h)]
 
     def check(self):
         """synchronise and raise on deferred device-side errors"""

@@ -361,25 +361,35 @@ def test_errors_and_state(gpu):
         gpu.LBM(8, 8, 1, "D2Q9", "SC1", bc=(1, 0, 0))  # Shan-Chen + walls: not implemented
 
 
-@pytest.mark.parametrize("name,grid,over", [
+PATH_CASES = [
     ("cfg2", (300, 21, 1), dict(radius=6.0)),
     ("cfg3", (260, 37, 1), {}),
-    ("cfg3", (130, 5, 1), dict(precision=32)),
+    ("cfg3", (132, 5, 1), dict(precision=32)),
     ("cfg5", (140, 9, 7), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
     ("cfg5", (16, 3, 2), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
-    ("cfg5", (9, 1, 1), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
-], ids=lambda v: str(v).replace(" ", ""))
-@pytest.mark.parametrize("wave", [None, (1, 1), (3, 2), (1000, 100000)], ids=lambda v: "wave%s" % (v,))
-def test_wavefront_and_two_launch_paths_match_oracle(gpu, name, grid, over, wave):
-    """Shan-Chen models: the one-launch wavefront path (several schedules: pencils of 1 / 3 / all rows,
-    psi rows 1 / 2 / all rows ahead) and the two-launch path (psi pass, then step) against the oracle
-    at every step 1..7, on rows of several x-segments with a ragged tail and on degenerate extents."""
+    ("cfg5", (8, 1, 1), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
+    ("cfg5", (4, 2, 3), dict(rmin=1.0, rmax=2.0, vol_frac=0.1)),
+    ("cfg1", (260, 9, 1), {}),
+    ("cfg1", (130, 7, 1), dict(bc=(0, 1, 0), force=(2e-5, 1e-5, 0.0))),
+    ("cfg4", (136, 5, 6), {}),
+    ("cfg4", (132, 6, 5), dict(precision=32)),
+    ("cfg4", (12, 6, 5), dict(precision=32, bc=(0, 1, 1), force=(1e-6, 2e-6, -1e-6))),
+    ("cfg4", (8, 6, 5), dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.03)),
+]
+PATHS = [("register", 0, 0), ("pipeline", 0, 0), ("pipeline", 1, 1), ("pipeline", 3, 2), ("pipeline", 1000, 100000)]
+
+
+@pytest.mark.parametrize("name,grid,over", PATH_CASES, ids=lambda v: str(v).replace(" ", ""))
+@pytest.mark.parametrize("path", PATHS, ids=lambda v: "%s-%d-%d" % v)
+def test_every_path_matches_oracle(gpu, name, grid, over, path):
+    """Both launch paths of lbm_step (include/lbm.h LBM_PATH_*: register kernels; persistent shared-memory
+    pipeline) with several schedules (pencils of 1 / 3 / all rows, psi rows 1 / 2 / all rows
+    ahead) against the oracle at every step 1..7, on rows of several x-segments with a ragged tail, on
+    degenerate extents, with walls in y / z, fp64 and fp32."""
     cfg = workloads.config(name, grid=grid, **over)
     ref, dev = make_pair(gpu, cfg)
-    if wave is None:
-        dev.set_wavefront(False)
-    else:
-        dev.set_wavefront(True, *wave)
+    dev.set_path(*path)
+    assert dev.get_path() == path[0]
     ref.init_from_seed(9)
     dev.set_populations(torch.from_numpy(ref.get_populations()))
     exact = not (cfg["model"] == "SC1" and cfg["params"].get("psi_kind", 0) == 0)
@@ -394,3 +404,15 @@ def test_wavefront_and_two_launch_paths_match_oracle(gpu, name, grid, over, wave
             assert np.abs(fr - fd).max() <= 1e-13 * np.abs(fr).max(), "step %d" % step
     dev.check()
     assert dev.launch_count() >= 7
+
+
+def test_pipeline_path_rejects_unaligned_rows_and_x_walls(gpu):
+    cfg = workloads.config("cfg4", grid=(9, 4, 4))
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    with pytest.raises(gpu.LbmError):
+        dev.set_path("pipeline")                     # 9 doubles per row: rows are not 16-byte aligned
+    assert dev.get_path() == "register"
+    cfg = workloads.config("cfg4", grid=(8, 4, 4), bc=(1, 0, 1))
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    with pytest.raises(gpu.LbmError):
+        dev.set_path("pipeline")                     # walls in x
