@@ -121,19 +121,22 @@ __device__ __forceinline__ bool thread_cell(int nx, int& x, int& y, int& z) {
     return x < nx;
 }
 
-// address of P_I(x): where f_I(x,t) is read and f*_{opp(I)}(x,t) is written
+// address of P_I(x): where f_I(x,t) is read and f*_{opp(I)}(x,t) is written.  The element index within one
+// lattice (Q * N < 2^32, checked by lbm_create) is formed in 32 bits -- a uniform (slot, row) part plus the
+// per-thread column -- so that an access costs one integer add and one IMAD.WIDE.
 template <class L, int PARITY, bool WALLS, int I, class R, class NB>
 __device__ __forceinline__ R* slot_of(R* base, const NB& nb, size_t N) {
+    const unsigned n = (unsigned)N;
     if constexpr (PARITY == 0 || I == 0) {
-        return (base + ((size_t)I * N + (size_t)nb.template row<0, 0>())) + nb.template col<0>();
+        return base + (((unsigned)I * n + (unsigned)nb.template row<0, 0>()) + (unsigned)nb.template col<0>());
     } else {
         constexpr int CX = -L::c(I, 0), CY = -L::c(I, 1), CZ = -L::c(I, 2);
-        R* nbr = (base + ((size_t)L::opp(I) * N + (size_t)nb.template row<CY, CZ>())) + nb.template col<CX>();
+        const unsigned nbr = ((unsigned)L::opp(I) * n + (unsigned)nb.template row<CY, CZ>()) + (unsigned)nb.template col<CX>();
         if constexpr (WALLS) {
-            R* own = (base + ((size_t)I * N + (size_t)nb.template row<0, 0>())) + nb.template col<0>();
-            return nb.template outside<CX, CY, CZ>() ? own : nbr;
+            const unsigned own = ((unsigned)I * n + (unsigned)nb.template row<0, 0>()) + (unsigned)nb.template col<0>();
+            return base + (nb.template outside<CX, CY, CZ>() ? own : nbr);
         } else {
-            return nbr;
+            return base + nbr;
         }
     }
 }
@@ -219,7 +222,7 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
         static_for<1, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-            const R wp = (R)L::w(i) * load_psi<COH>((ps + nb.template row<CY, CZ>()) + nb.template col<CX>());
+            const R wp = (R)L::w(i) * load_psi<COH>(ps + ((unsigned)nb.template row<CY, CZ>() + (unsigned)nb.template col<CX>()));
             static_for<0, L::D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 constexpr int c = L::c(i, a);

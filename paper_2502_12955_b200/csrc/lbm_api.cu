@@ -55,6 +55,8 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (p->psi_kind != 0 && p->psi_kind != 1) return "psi_kind must be 0 or 1";
     if ((double)nx * (double)ny * (double)nz > 2147483647.0) return "grid has more than 2^31-1 cells";
     if (ny > 65535 || nz > 65535) return "ny and nz must not exceed 65535 (CUDA grid limits)";
+    if ((lattice == LBM_D3Q19 ? 19.0 : 9.0) * (double)nx * (double)ny * (double)nz >= 4294967296.0)
+        return "Q * nx * ny * nz must stay below 2^32 (the kernels index one lattice with 32 bits)";
     const int S = (model == LBM_SC2 || model == LBM_SC2_ADE) ? 2 : 1;
     for (int s = 0; s < S; ++s)
         if (!(p->tau[s] > 0.5)) return "tau must exceed 0.5";
