@@ -137,10 +137,12 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *                       at the same time level: PAPER.md:128, 136; R9): the populations cross HBM once per
  *                       step, the second read hits L2.  Needs nx * sizeof(value) % 16 == 0 and periodic x
  *                       (LBM_EINVAL otherwise).
+ *   LBM_PATH_WAVEFRONT  Shan-Chen models only: the same one-launch schedule of psi and step segments, with the
+ *                       populations loaded straight into registers as on LBM_PATH_REGISTER (any nx).
  * lbm_create starts with LBM_PATH_REGISTER.
- * rows_per_pencil / lead_rows: schedule parameters of the pipelined path for Shan-Chen models (<= 0: defaults; DESIGN.md
+ * rows_per_pencil / lead_rows: schedule parameters of the two one-launch paths for Shan-Chen models (<= 0: defaults; DESIGN.md
  * "Wavefront").  Synchronises the stream. */
-enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1 };
+enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1, LBM_PATH_WAVEFRONT = 2 };
 int lbm_set_path(lbm_ctx* ctx, int path, int rows_per_pencil, int lead_rows);
 int lbm_get_path(const lbm_ctx* ctx);
 

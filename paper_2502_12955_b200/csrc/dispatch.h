@@ -23,6 +23,9 @@ struct Ops {
     cudaError_t (*pipe)(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
                         cudaStream_t st);
     int (*pipe_blocks)(int model, int parity, int walls, int forced);
+    // register-flavoured wavefront kernel of the Shan-Chen models (wave.cuh)
+    cudaError_t (*wave)(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st);
+    int (*wave_blocks)(int model, int parity);
 };
 
 const Ops* ops_f64_d2q9();

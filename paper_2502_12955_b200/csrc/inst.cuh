@@ -3,6 +3,7 @@
 #include "dispatch.h"
 #include "kernels.cuh"
 #include "pipe.cuh"
+#include "wave.cuh"
 #include <cstdlib>
 
 namespace lbm {
@@ -164,8 +165,42 @@ struct Launch {
         return b;
     }
 
+    template <int MODEL>
+    static cudaError_t wave2(const KP<R>& p, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
+        auto k = parity ? k_wave<R, L, MODEL, 1> : k_wave<R, L, MODEL, 0>;
+        if (out_blocks) {
+            int per_sm = 0, dev = 0, sms = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PIPE_TX, 0);
+            if (e == cudaSuccess) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess) return e;
+            *out_blocks = per_sm * sms;
+            return cudaSuccess;
+        }
+        k<<<blocks, PIPE_TX, 0, st>>>(p, *wa);
+        return cudaGetLastError();
+    }
+    static cudaError_t wave_any(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* ob) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        switch (model) {
+        case M_SC1: return wave2<M_SC1>(p, parity, wa, blocks, st, ob);
+        case M_SC2: return wave2<M_SC2>(p, parity, wa, blocks, st, ob);
+        case M_SC2_ADE: return wave2<M_SC2_ADE>(p, parity, wa, blocks, st, ob);
+        default: return cudaErrorInvalidValue;
+        }
+    }
+    static cudaError_t wave(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st) {
+        return wave_any(kp, model, parity, wa, blocks, st, nullptr);
+    }
+    static int wave_blocks(int model, int parity) {
+        int b = 0;
+        KP<R> dummy{};
+        if (wave_any(&dummy, model, parity, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
+        return b;
+    }
+
     static const Ops* ops() {
-        static const Ops o = {&psi, &step, &macros, &permute, &init, &pipe, &pipe_blocks};
+        static const Ops o = {&psi, &step, &macros, &permute, &init, &pipe, &pipe_blocks, &wave, &wave_blocks};
         return &o;
     }
 };

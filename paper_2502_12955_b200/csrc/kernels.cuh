@@ -416,28 +416,32 @@ __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) 
 // ------------------------------------------------------------------------------------------
 // fused step (a1, a3-a8): one thread per cell
 // ------------------------------------------------------------------------------------------
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false>
-__device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
+// first half: the populations of the cell into registers
+template <class R, class L, int MODEL, int PARITY, bool WALLS, class NB>
+__device__ __forceinline__ void step_load(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, WALLS> nb(p, x, y, z);
-
-    R fl[S][Q];
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
     });
-    R hl[LS::Q];
     if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
-
+}
+// second half: moments, force (psi stencil), collision, stores
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH, class NB>
+__device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
+    using MT = ModelTraits<MODEL>;
+    using LS = typename ScalarOf<L>::type;
+    constexpr int S = MT::S, Q = L::Q;
+    const size_t N = (size_t)p.N;
     CellMacro<R, L, MODEL> m;
     cell_macros<R, L, MODEL, FORCED, COH>(p, nb, fl, m);
 
     // the store addresses are recomputed from laundered column offsets instead of being kept in
-    // registers from the loads on (one 64-bit pair per slot otherwise)
-    Nbr<L::D, WALLS> ns = nb;
+    // registers from the loads on
+    NB ns = nb;
     asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
@@ -450,8 +454,25 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     }
 }
 
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false>
+__device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
+    using LS = typename ScalarOf<L>::type;
+    const Nbr<L::D, WALLS> nb(p, x, y, z);
+    R fl[ModelTraits<MODEL>::S][L::Q];
+    R hl[LS::Q];
+    step_load<R, L, MODEL, PARITY, WALLS>(p, nb, fl, hl);
+    step_finish<R, L, MODEL, PARITY, WALLS, FORCED, COH>(p, nb, fl, hl);
+}
+
+// Shan-Chen variants always run with 128 threads; asking for 5 (6 for one component) resident blocks per SM
+// bounds their registers (measured on cfg5: 4 -> 3.28 ms, 5 -> 3.09 ms, 6 -> 3.30 ms per step at 512x512x128)
+template <int MODEL> struct StepBounds {
+    static constexpr int THREADS = MODEL == M_BGK ? BLOCK : 128;
+    static constexpr int MINB = MODEL == M_BGK ? 1 : (MODEL == M_SC1 ? 6 : 5);
+};
+
 template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED>
-__global__ void __launch_bounds__(BLOCK) k_step(const __grid_constant__ KP<R> p) {
+__global__ void __launch_bounds__(StepBounds<MODEL>::THREADS, StepBounds<MODEL>::MINB) k_step(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
     step_cell<R, L, MODEL, PARITY, WALLS, FORCED>(p, x, y, z);

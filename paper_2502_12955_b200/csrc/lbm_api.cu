@@ -228,15 +228,16 @@ bool pipe_eligible(const lbm_ctx* c) {
 
 // Switch to the pipelined path: (re)build the schedule (one entry per ticket) and the device state of the
 // ticket counter; py / lead <= 0 pick the defaults
-int path_setup(lbm_ctx* c, int py, int lead) {
+int path_setup(lbm_ctx* c, int path, int py, int lead) {
     CK(cudaStreamSynchronize(c->stream));
     wave_free(c);
     const Shape& sh = c->sh;
     const int nm = sh.d == 3 ? c->ny : 1, ns = sh.d == 3 ? c->nz : c->ny;
     const int nxs = (c->nx + lbm::PIPE_TX - 1) / lbm::PIPE_TX;
     for (int par = 0; par < 2; ++par) {
-        c->wave_blocks[par] = c->ops->pipe_blocks(c->model, par, c->walls, c->forced);
-        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "pipelined kernel: occupancy query failed");
+        c->wave_blocks[par] = path == LBM_PATH_WAVEFRONT ? c->ops->wave_blocks(c->model, par)
+                                                          : c->ops->pipe_blocks(c->model, par, c->walls, c->forced);
+        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "persistent kernel: occupancy query failed");
     }
     std::vector<lbm::WaveItem> rows;
     if (sh.sc) {
@@ -281,7 +282,7 @@ int path_setup(lbm_ctx* c, int py, int lead) {
     CK(cudaStreamSynchronize(c->stream));   // items goes out of scope
     c->wave_base = 0;
     c->wave_epoch = 0;
-    c->path = LBM_PATH_PIPELINE;
+    c->path = path;
     return 0;
 }
 
@@ -303,7 +304,8 @@ int run_pipe(lbm_ctx* c) {
     const int blocks = c->wave_blocks[parity];
     int rc = mark(c, 0);
     if (rc) return rc;
-    CK(c->ops->pipe(c->kp(), c->model, parity, c->walls, c->forced, &wa, blocks, c->stream));
+    if (c->path == LBM_PATH_WAVEFRONT) CK(c->ops->wave(c->kp(), c->model, parity, &wa, blocks, c->stream));
+    else CK(c->ops->pipe(c->kp(), c->model, parity, c->walls, c->forced, &wa, blocks, c->stream));
     // every block draws tickets until three of them lie past the end (pipe.cuh)
     c->wave_base += (unsigned long long)wa.n_tickets + 3ULL * (unsigned long long)blocks;
     c->launches++;
@@ -571,10 +573,15 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
         wave_free(c);
         return 0;
     }
-    if (path != LBM_PATH_PIPELINE) return fail(LBM_EINVAL, "unknown path");
-    if (!pipe_eligible(c))
-        return fail(LBM_EINVAL, "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes and periodic x");
-    return path_setup(c, rows_per_pencil, lead_rows);
+    if (path == LBM_PATH_WAVEFRONT) {
+        if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
+    } else if (path == LBM_PATH_PIPELINE) {
+        if (!pipe_eligible(c))
+            return fail(LBM_EINVAL, "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes and periodic x");
+    } else {
+        return fail(LBM_EINVAL, "unknown path");
+    }
+    return path_setup(c, path, rows_per_pencil, lead_rows);
 }
 
 int lbm_get_path(const lbm_ctx* c) { return c ? c->path : LBM_EINVAL; }

@@ -17,7 +17,7 @@ LATTICES = {"D2Q9": D2Q9, "D3Q19": D3Q19}
 MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE}
 INITS = {"REST": 0, "TAYLOR_GREEN": 1, "DROPLET": 2, "UNIFORM_NOISE": 3, "RANDOM_DROPLETS": 4}
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
-PATHS = {"register": 0, "pipeline": 1}
+PATHS = {"register": 0, "pipeline": 1, "wavefront": 2}
 
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
@@ -271,7 +271,7 @@ class LBM:
         return ms.value, n.value
 
     def set_path(self, path, rows_per_pencil=0, lead_rows=0):
-        """which kernels step() launches: "register" or "pipeline" (include/lbm.h)"""
+        """which kernels step() launches: "register", "pipeline" or "wavefront" (Shan-Chen only) (include/lbm.h)"""
         path = PATHS[path] if isinstance(path, str) else int(path)
         self._chk(self.L.lbm_set_path(self.h, path, int(rows_per_pencil), int(lead_rows)))
 
