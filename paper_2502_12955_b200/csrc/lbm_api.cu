@@ -119,8 +119,13 @@ struct lbm_ctx {
     // per-kernel timing (lbm_kernel_timing): event pairs around every launch of kind 0 (fused step) / 1 (psi pass)
     bool timing;
     std::vector<cudaEvent_t> ev[2];
-    // pipelined persistent path (pipe.cuh): one ticketed launch per time step
     int path;                         // LBM_PATH_*: which kernels lbm_step launches
+    // small grids (launch-latency bound): GRAPH_STEPS time steps of the register path captured once as a CUDA
+    // graph and replayed, so that consecutive kernels start back to back instead of one launch call each
+    cudaGraphExec_t graph_exec;
+    cudaStream_t graph_capture_stream;
+    bool graph_failed;
+    // one-launch persistent paths (pipe.cuh, wave.cuh): schedule, ticket counter, flags
     int wave_py, wave_lead;           // schedule parameters in use
     int wave_blocks[2];               // blocks per launch, by parity
     lbm::PipeItem* wave_items;        // device copy of the schedule, one entry per ticket
@@ -354,6 +359,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->inited = false; c->t = 0; c->launches = 0;
     c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
     c->timing = false;
+    c->graph_exec = nullptr; c->graph_capture_stream = nullptr; c->graph_failed = false;
     c->path = LBM_PATH_REGISTER; c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
     c->wave_py = c->wave_lead = 0; c->wave_base = 0; c->wave_epoch = 0;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
@@ -391,6 +397,8 @@ void lbm_destroy(lbm_ctx* c) {
     if (c->droplets_dev) cudaFree(c->droplets_dev);
     if (c->scratch) cudaFree(c->scratch);
     wave_free(c);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph_capture_stream) cudaStreamDestroy(c->graph_capture_stream);
     if (c->owns_ws && c->ws) cudaFree(c->ws);
     cudaGetLastError();
     delete c;
@@ -423,12 +431,59 @@ int lbm_init_from_seed(lbm_ctx* c, uint64_t seed) {
     return 0;
 }
 
+namespace {
+constexpr int GRAPH_STEPS = 32;                 // even: a replay starts and ends at even parity
+constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far longer than a launch call
+
+// the kernels of one time step of the register path, enqueued on st (no event marks, no counters)
+int enqueue_register_step(lbm_ctx* c, int parity, cudaStream_t st) {
+    if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, st));
+    CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, st));
+    return 0;
+}
+
+// capture GRAPH_STEPS steps on a private stream (nothing runs during capture) and instantiate the graph
+int build_graph(lbm_ctx* c) {
+    cudaGraph_t graph = nullptr;
+    if (!c->graph_capture_stream) CK(cudaStreamCreateWithFlags(&c->graph_capture_stream, cudaStreamNonBlocking));
+    CK(cudaStreamBeginCapture(c->graph_capture_stream, cudaStreamCaptureModeRelaxed));
+    int rc = 0;
+    for (int k = 0; k < GRAPH_STEPS && rc == 0; ++k) rc = enqueue_register_step(c, k & 1, c->graph_capture_stream);
+    cudaError_t e = cudaStreamEndCapture(c->graph_capture_stream, &graph);
+    if (rc != 0 || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return rc != 0 ? rc : fail(LBM_ECUDA, "CUDA graph capture failed");
+    }
+    e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { cudaGetLastError(); c->graph_exec = nullptr; return cuda_fail(e, "cudaGraphInstantiate"); }
+    return 0;
+}
+}  // namespace
+
 int lbm_step(lbm_ctx* c, int n) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
     if (!c->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init_from_seed / lbm_set_populations");
     if (n < 0) return fail(LBM_EINVAL, "n < 0");
     DeviceGuard g(c->device);
-    for (int k = 0; k < n; ++k) {
+    int done = 0;
+    if (c->path == LBM_PATH_REGISTER && !c->timing && !c->graph_failed && c->sh.N <= GRAPH_MAX_CELLS) {
+        if ((c->t & 1) && n >= GRAPH_STEPS + 1) {       // reach even parity with one ordinary step
+            int rc = enqueue_register_step(c, 1, c->stream);
+            if (rc) return rc;
+            c->launches += c->sh.sc ? 2 : 1; c->t++; done++;
+        }
+        if ((c->t & 1) == 0 && n - done >= GRAPH_STEPS) {
+            if (!c->graph_exec && build_graph(c) != 0) c->graph_failed = true;    // fall back to plain launches
+            while (c->graph_exec && n - done >= GRAPH_STEPS) {
+                CK(cudaGraphLaunch(c->graph_exec, c->stream));
+                c->launches += (int64_t)GRAPH_STEPS * (c->sh.sc ? 2 : 1);
+                c->t += GRAPH_STEPS; done += GRAPH_STEPS;
+            }
+        }
+    }
+    for (int k = done; k < n; ++k) {
         const int parity = (int)(c->t & 1);
         int rc;
         if (c->path != LBM_PATH_REGISTER) {   // one persistent ticketed launch per step (pipe.cuh)
