@@ -147,7 +147,7 @@ struct Sim : ref_ctx {
 
     /* constants, rounded once to R */
     R w[19], ws[7];
-    R omega[2], cf[2], omega_c, inv_cs2g;
+    R omega[2], cf[2], tau_r[2], omega_c, inv_cs2g;
     R G[2][2], rho0_psi, force[3], k_react;
 
     /* fields */
@@ -155,6 +155,7 @@ struct Sim : ref_ctx {
     std::vector<R> h, hnew;        /* [i][cell] */
     std::vector<R> rho, jm, psi;   /* rho[sigma][cell], jm[sigma][a][cell], psi[sigma][cell] */
     std::vector<R> Fv, ub;         /* Fv[sigma][a][cell], ub[a][cell] */
+    std::vector<R> ueq;            /* ueq[sigma][a][cell]: equilibrium velocity of the velocity-shift scheme, Eq. 16 */
 
     R& F_(std::vector<R>& v, int s, int i, size_t cell) { return v[((size_t)s * Q + i) * N + cell]; }
     R& H_(std::vector<R>& v, int i, size_t cell) { return v[(size_t)i * N + cell]; }
@@ -173,6 +174,7 @@ struct Sim : ref_ctx {
         for (int i = 0; i < Qs; ++i) ws[i] = (R)Ls.w[i];
         for (int s = 0; s < 2; ++s) {
             omega[s] = (R)(1.0 / pp.tau[s]);              /* 1/tau, Eq. 15 */
+            tau_r[s] = (R)pp.tau[s];
             cf[s] = (R)(1.0 - 0.5 / pp.tau[s]);           /* 1 - 1/(2 tau), Eq. 15 */
             for (int t = 0; t < 2; ++t) G[s][t] = (R)pp.G[s][t];
         }
@@ -188,6 +190,7 @@ struct Sim : ref_ctx {
         psi.assign((size_t)S * N, (R)0);
         Fv.assign((size_t)S * 3 * N, (R)0);
         ub.assign((size_t)3 * N, (R)0);
+        ueq.assign((size_t)S * 3 * N, (R)0);
     }
 
     size_t cell_of(int x, int y, int z) const { return (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * z); }
@@ -278,6 +281,23 @@ struct Sim : ref_ctx {
                         }
                         ub[(size_t)a * N + cell] = (jt + (R)0.5 * Ft) * inv_rho;
                     }
+                    /* Shan-Chen (velocity-shift) forcing scheme, p.forcing == 1: common velocity
+                     * u' = sum_s (j^s / tau^s) / sum_s (rho^s / tau^s), Eq. 17, and
+                     * u^eq,s = u' + tau^s F^s / rho^s, Eq. 16; rho^s u^s = j^s, Eq. 18 */
+                    if (p.forcing == 1) {
+                        R den = rho[cell] * omega[0];
+                        for (int s = 1; s < S; ++s) den = den + rho[(size_t)s * N + cell] * omega[s];
+                        R inv_den = (R)1 / den;
+                        for (int a = 0; a < 3; ++a) {
+                            R num = jm[(size_t)a * N + cell] * omega[0];
+                            for (int s = 1; s < S; ++s) num = num + jm[((size_t)s * 3 + a) * N + cell] * omega[s];
+                            R up = num * inv_den;
+                            for (int s = 0; s < S; ++s) {
+                                R inv_rs = (R)1 / rho[(size_t)s * N + cell];
+                                ueq[((size_t)s * 3 + a) * N + cell] = up + (tau_r[s] * Fv[((size_t)s * 3 + a) * N + cell]) * inv_rs;
+                            }
+                        }
+                    }
                 }
     }
 
@@ -296,15 +316,20 @@ struct Sim : ref_ctx {
                         R uF = (R)0;
                         for (int a = 0; a < d; ++a) uF = uF + u[a] * Fs[a];
                         R rho_s = rho[(size_t)s * N + cell];
+                        /* velocity-shift scheme: equilibrium at u^eq,s, no forcing term F_i */
+                        R us[3] = {u[0], u[1], u[2]};
+                        if (p.forcing == 1)
+                            for (int a = 0; a < 3; ++a) us[a] = ueq[((size_t)s * 3 + a) * N + cell];
                         for (int i = 0; i < Q; ++i) {
                             R fi = F_(f, s, i, cell);
-                            R fe = feq(i, rho_s, u);
+                            R fe = feq(i, rho_s, us);
                             R cu = (R)0, cF = (R)0;
                             for (int a = 0; a < d; ++a) cu = cu + (R)L.c[i][a] * u[a];
                             for (int a = 0; a < d; ++a) cF = cF + (R)L.c[i][a] * Fs[a];
                             /* F_i = w_i [ (c_i - u).F / c_s^2 + (c_i.u)(c_i.F) / c_s^4 ], Eq. 22 */
                             R Fi = w[i] * ((R)3 * (cF - uF) + ((R)9 * cu) * cF);
                             R fstar = (fi - omega[s] * (fi - fe)) + cf[s] * Fi;
+                            if (p.forcing == 1) fstar = fi - omega[s] * (fi - fe);
                             /* 7. stream, Eq. 5; halfway bounce-back at walls */
                             size_t nb;
                             if (neighbour(x, y, z, L.c[i], nb)) F_(fnew, s, i, nb) = fstar;
@@ -522,7 +547,7 @@ ref_ctx* ref_create(int nx, int ny, int nz, int lattice, int model, const ref_pa
     if (lattice == REF_D2Q9 && nz != 1) { g_err = "D2Q9 needs nz == 1"; return nullptr; }
     if (model < REF_BGK || model > REF_SC2_ADE) { g_err = "bad model"; return nullptr; }
     if (p->precision != 32 && p->precision != 64) { g_err = "precision must be 32 or 64"; return nullptr; }
-    if (p->forcing != 0) { g_err = "only Guo forcing (0) is implemented"; return nullptr; }
+    if (p->forcing != 0 && p->forcing != 1) { g_err = "forcing must be 0 (Guo) or 1 (velocity shift)"; return nullptr; }
     if (p->psi_kind != 0 && p->psi_kind != 1) { g_err = "bad psi_kind"; return nullptr; }
     int S = (model == REF_SC2 || model == REF_SC2_ADE) ? 2 : 1;
     for (int s = 0; s < S; ++s)

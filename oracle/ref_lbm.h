@@ -38,7 +38,7 @@ typedef struct ref_params {
     double   tau_c;         /* scalar relaxation time, Eq. 34 */
     double   G[2][2];       /* Shan-Chen coupling G_{sigma sigma~}, Eq. 11/13 */
     int32_t  psi_kind;      /* 0: rho0*(1-exp(-rho/rho0)) Eq. 10/24 ; 1: psi = rho */
-    int32_t  forcing;       /* 0: Guo, Eq. 20-23 (only value accepted) */
+    int32_t  forcing;       /* 0: Guo, Eq. 20-23; 1: Shan-Chen velocity shift, Eq. 16-19 */
     double   rho0_psi;      /* rho0 of Eq. 10 */
     double   force[3];      /* constant body-force density */
     int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls */

@@ -674,3 +674,83 @@ def test_errors():
     r = RefLBM(4, 4, 1, "D2Q9", "BGK")
     with pytest.raises(RuntimeError):
         r.step(1)                                                    # step before init
+
+
+# ----------------------------------------------------------------------------------------------
+# Shan-Chen (velocity-shift) forcing scheme, forcing = 1: Eq. 16-19
+# ----------------------------------------------------------------------------------------------
+def test_velocity_shift_without_force_is_plain_bgk():
+    """F = 0: u^eq = u' = j / rho (Eq. 16-17 with one component), so the scheme is the LBGK update itself."""
+    kw = dict(precision=64, tau=(0.8, 0.8), init_kind="TAYLOR_GREEN", u0=0.03, rho_init=(1.1, 1.0))
+    a = RefLBM(12, 10, 1, "D2Q9", "BGK", forcing=0, **kw)
+    b = RefLBM(12, 10, 1, "D2Q9", "BGK", forcing=1, **kw)
+    a.init_from_seed(0); b.init_from_seed(0)
+    a.step(60); b.step(60)
+    fa, fb = a.get_populations(), b.get_populations()
+    assert np.abs(fa - fb).max() <= 1e-14 * np.abs(fa).max()
+
+
+@pytest.mark.parametrize("lattice,grid,force", [("D2Q9", (6, 5, 1), (3e-5, -2e-5, 0.0)), ("D3Q19", (4, 5, 3), (1e-5, 2e-5, -3e-5))])
+def test_velocity_shift_uniform_force_momentum_growth(lattice, grid, force):
+    """The first moment of f^eq(rho, u' + tau F / rho) is j + tau F, so relaxing towards it adds exactly F to
+    the momentum of each cell per step (Eq. 15-16); the physical velocity carries F/2 (Eq. 19)."""
+    tau = 0.77
+    r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(tau, tau), force=force, rho_init=(1.25, 1.0), forcing=1)
+    r.init_from_seed(0)
+    c, _ = lattice_table(lattice)
+    done = 0
+    for t in (0, 1, 7, 40):
+        r.step(t - done); done = t
+        m = r.get_macros()
+        f, _ = r.split_populations(r.get_populations())
+        for a in range(r.d):
+            assert np.allclose(m["u"][a], force[a] * (t + 0.5) / 1.25, rtol=1e-11, atol=1e-19)
+            assert np.allclose((c[:, a, None] * f[0]).sum(0), force[a] * t, rtol=1e-10, atol=1e-18)
+        assert np.abs(m["rho"] - 1.25).max() < 1e-13
+
+
+@pytest.mark.parametrize("model,lattice,grid", [("SC2", "D2Q9", (16, 12, 1)), ("SC2_ADE", "D3Q19", (8, 8, 6)), ("SC1", "D2Q9", (16, 16, 1))])
+def test_velocity_shift_conserves_momentum_with_unequal_relaxation_times(model, lattice, grid):
+    """With u' weighted by rho^s / tau^s (Eq. 17) the relaxation terms of the components cancel in the sum:
+    sum_s (j^s - rho^s u') / tau^s = 0, so the total momentum of a periodic box changes by sum F = 0 only --
+    for ANY tau^A != tau^B (a plain average in Eq. 17 would break this).  Mass per component is invariant."""
+    r = noise_cfg(model, lattice, grid, tau=(1.0, 0.7), forcing=1)
+    r.init_from_seed(5)
+    c, _ = lattice_table(lattice)
+
+    def totals():
+        f, _ = r.split_populations(r.get_populations())
+        return f.sum(axis=(1, 2)), np.array([(c[:, a, None] * f.sum(0)).sum() for a in range(r.d)])
+
+    m0, p0 = totals()
+    r.step(150)
+    m1, p1 = totals()
+    assert np.abs(m1 - m0).max() / m0.max() < 1e-13
+    assert np.abs(p1 - p0).max() / m0.sum() < 1e-13
+    assert np.abs(r.get_force()).max() > 1e-5
+
+
+def test_velocity_shift_poiseuille_curvature():
+    """Body force + halfway bounce-back walls under the velocity-shift scheme: the steady profile is a parabola
+    of curvature -g / nu with nu = (tau - 1/2) / 3 (the extra tau^2 F F / rho momentum flux of this scheme is
+    uniform here), symmetric about the channel centre."""
+    nz, g, tau = 16, 1e-6, 0.9
+    cfg = workloads.config("cfg4", grid=(1, 1, nz), tau=(tau, tau), forcing=1)
+    r = make(cfg)
+    r.init_from_seed(0)
+    nu = (tau - 0.5) / 3
+    r.step(int(30 * nz * nz / nu))
+    u = r.get_macros()["u"][0]
+    d2 = u[2:] - 2 * u[1:-1] + u[:-2]
+    assert np.allclose(d2, -g / nu, rtol=1e-6)
+    assert np.allclose(u, u[::-1], rtol=1e-9)
+    assert u.max() > 0.9 * g * nz * nz / (8 * nu)
+
+
+def test_velocity_shift_uniform_state_is_stationary():
+    r = RefLBM(6, 5, 4, "D3Q19", "SC2", precision=64, tau=(1.3, 0.8), psi_kind=1, G=workloads.G12, forcing=1,
+               init_kind="REST", rho_init=(0.9, 1.2))
+    r.init_from_seed(0)
+    f0 = r.get_populations().copy()
+    r.step(25)
+    assert np.abs(r.get_populations() - f0).max() < 1e-15
