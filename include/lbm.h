@@ -63,7 +63,8 @@ typedef struct lbm_params {
     double   tau_c;         /* scalar-lattice relaxation time, > 0.5; Eq. 34 */
     double   G[2][2];       /* Shan-Chen coupling G_{sigma sigma~}; SC1 uses G[0][0]; Eq. 11/13 */
     int32_t  psi_kind;      /* 0: psi = rho0 (1 - exp(-rho/rho0)), Eq. 10/24 ; 1: psi = rho (R3) */
-    int32_t  forcing;       /* 0: Guo, Eq. 20-23 (the only accepted value) */
+    int32_t  forcing;       /* 0: Guo, Eq. 20-23; 1: Shan-Chen velocity shift, Eq. 16-19
+                               (PAPER.md:154-174): u_eq = u' + tau F / rho, no F_i term; LBM_PATH_REGISTER only */
     double   rho0_psi;      /* rho0 of Eq. 10 */
     double   force[3];      /* constant body-force density; S = 2: split by mass fraction (R5) */
     int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls on both faces;

@@ -36,13 +36,24 @@ struct Launch {
         return cudaGetLastError();
     }
 
-    template <int MODEL, bool WALLS, bool FORCED>
+    template <int MODEL, bool WALLS, bool FORCED, bool VSHIFT = false>
     static void step3(const KP<R>& p, int parity, cudaStream_t st) {
-        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED><<<grid_for(p), block_for(p), 0, st>>>(p);
-        else k_step<R, L, MODEL, 0, WALLS, FORCED><<<grid_for(p), block_for(p), 0, st>>>(p);
+        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED, VSHIFT><<<grid_for(p), block_for(p), 0, st>>>(p);
+        else k_step<R, L, MODEL, 0, WALLS, FORCED, VSHIFT><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
+    // forced: 0 no force, 1 Guo forcing (Eq. 20-23), 2 Shan-Chen velocity-shift forcing (Eq. 16-19)
     static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
+        if (forced == 2) {
+            switch (model) {
+            case M_BGK: if (walls) step3<M_BGK, true, true, true>(p, parity, st); else step3<M_BGK, false, true, true>(p, parity, st); break;
+            case M_SC1: step3<M_SC1, false, true, true>(p, parity, st); break;
+            case M_SC2: step3<M_SC2, false, true, true>(p, parity, st); break;
+            case M_SC2_ADE: step3<M_SC2_ADE, false, true, true>(p, parity, st); break;
+            default: return cudaErrorInvalidValue;
+            }
+            return cudaGetLastError();
+        }
         switch (model) {
         case M_BGK:
             if (walls) { if (forced) step3<M_BGK, true, true>(p, parity, st); else step3<M_BGK, true, false>(p, parity, st); }

@@ -38,6 +38,7 @@ struct KP {
     int bc[3];
     int psi_kind;
     R omega[2], cf[2];        // 1/tau, 1 - 1/(2 tau): Eq. 15
+    R tau[2];                 // tau itself (velocity-shift forcing, Eq. 16)
     R omega_c, inv_cs2g;      // 1/tau_c (Eq. 34), 1/c_{s,g}^2 = d/(1-w0) (Eq. 35, R6)
     R ws0, ws1;               // scalar-lattice weights
     R G[2][2];
@@ -242,6 +243,7 @@ template <class R, class L, int MODEL>
 struct CellMacro {
     static constexpr int S = ModelTraits<MODEL>::S;
     R rho[S];
+    R j[S][3];
     R F[S][3];
     R u[3];
     R inv_rho;
@@ -254,7 +256,7 @@ __device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L
                                                  CellMacro<R, L, MODEL>& m) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
-    R j[S][3];
+    R (&j)[S][3] = m.j;
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         j[s][0] = j[s][1] = j[s][2] = (R)0;
@@ -454,28 +456,81 @@ __device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl
     }
 }
 
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false>
+// both halves for one cell (k_step).  Written out rather than calling step_load / step_finish: ptxas keeps the
+// load addresses alive across the call boundary of the split form (fp32 BGK: 40 -> 80 registers).
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false, bool VSHIFT = false>
 __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
+    using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
+    constexpr int S = MT::S, Q = L::Q;
+    const size_t N = (size_t)p.N;
     const Nbr<L::D, WALLS> nb(p, x, y, z);
-    R fl[ModelTraits<MODEL>::S][L::Q];
+
+    R fl[S][Q];
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
+    });
     R hl[LS::Q];
-    step_load<R, L, MODEL, PARITY, WALLS>(p, nb, fl, hl);
-    step_finish<R, L, MODEL, PARITY, WALLS, FORCED, COH>(p, nb, fl, hl);
+    if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+
+    CellMacro<R, L, MODEL> m;
+    cell_macros<R, L, MODEL, FORCED, COH>(p, nb, fl, m);
+
+    // Shan-Chen (velocity-shift) forcing scheme: common velocity u' = sum_s (j^s / tau^s) / sum_s (rho^s / tau^s),
+    // Eq. 17; u^eq,s = u' + tau^s F^s / rho^s, Eq. 16; no forcing term F_i
+    R ueq[S][3];
+    if constexpr (VSHIFT) {
+        R den = m.rho[0] * p.omega[0];
+        if constexpr (S == 2) den = den + m.rho[1] * p.omega[1];
+        const R inv_den = (R)1 / den;
+        R inv_rs[S];
+        static_for<0, S>([&](auto sc) { inv_rs[decltype(sc)::value] = (R)1 / m.rho[decltype(sc)::value]; });
+        static_for<0, L::D>([&](auto ac) {
+            constexpr int a = decltype(ac)::value;
+            R num = m.j[0][a] * p.omega[0];
+            if constexpr (S == 2) num = num + m.j[1][a] * p.omega[1];
+            const R up = num * inv_den;
+            static_for<0, S>([&](auto sc) {
+                constexpr int s = decltype(sc)::value;
+                ueq[s][a] = up + (p.tau[s] * m.F[s][a]) * inv_rs[s];
+            });
+        });
+    }
+
+    Nbr<L::D, WALLS> ns = nb;
+    asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        if constexpr (VSHIFT) collide<R, L, false>(fl[s], m.rho[s], ueq[s], m.F[s], p.omega[s], p.cf[s]);
+        else collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+        store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
+    });
+    if constexpr (MT::SCALAR) {
+        collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
+        store_pops<LS, PARITY, WALLS>(p.h, ns, N, hl);
+    }
 }
 
-// Shan-Chen variants always run with 128 threads; asking for 5 (6 for one component) resident blocks per SM
-// bounds their registers (measured on cfg5: 4 -> 3.28 ms, 5 -> 3.09 ms, 6 -> 3.30 ms per step at 512x512x128)
-template <int MODEL> struct StepBounds {
-    static constexpr int THREADS = MODEL == M_BGK ? BLOCK : 128;
-    static constexpr int MINB = MODEL == M_BGK ? 1 : (MODEL == M_SC1 ? 6 : 5);
+// k_step always runs with 128 threads.  The minimum number of resident blocks per SM bounds its registers
+// (ptxas fills whatever the bound leaves: a bound of 1 block made fp64 BGK use 168 registers instead of 80).
+// Measured on cfg4: fp32 10 or 12 blocks 41.4 GLUPS, 8: 39.4, 16: 36.0; fp64 4-6 blocks 22.1, 8: 21.3.
+#ifndef LBM_MINB_BGK32
+#define LBM_MINB_BGK32 10
+#endif
+#ifndef LBM_MINB_BGK64
+#define LBM_MINB_BGK64 6
+#endif
+template <class R, int MODEL> struct StepBounds {
+    static constexpr int THREADS = 128;
+    static constexpr int MINB = MODEL == M_BGK ? (sizeof(R) == 4 ? LBM_MINB_BGK32 : LBM_MINB_BGK64) : (MODEL == M_SC1 ? 6 : 5);
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED>
-__global__ void __launch_bounds__(StepBounds<MODEL>::THREADS, StepBounds<MODEL>::MINB) k_step(const __grid_constant__ KP<R> p) {
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool VSHIFT = false>
+__global__ void __launch_bounds__(StepBounds<R, MODEL>::THREADS, StepBounds<R, MODEL>::MINB) k_step(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
-    step_cell<R, L, MODEL, PARITY, WALLS, FORCED>(p, x, y, z);
+    step_cell<R, L, MODEL, PARITY, WALLS, FORCED, false, VSHIFT>(p, x, y, z);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -51,7 +51,7 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (lattice == LBM_D2Q9 && nz != 1) return "D2Q9 needs nz == 1";
     if (model < LBM_BGK || model > LBM_SC2_ADE) return "unknown model";
     if (p->precision != 32 && p->precision != 64) return "precision must be 32 or 64";
-    if (p->forcing != 0) return "only Guo forcing (forcing = 0) is implemented";
+    if (p->forcing != 0 && p->forcing != 1) return "forcing must be 0 (Guo) or 1 (Shan-Chen velocity shift)";
     if (p->psi_kind != 0 && p->psi_kind != 1) return "psi_kind must be 0 or 1";
     if ((double)nx * (double)ny * (double)nz > 2147483647.0) return "grid has more than 2^31-1 cells";
     if (ny > 65535 || nz > 65535) return "ny and nz must not exceed 65535 (CUDA grid limits)";
@@ -109,7 +109,8 @@ struct lbm_ctx {
     const lbm::Ops* ops;
     lbm::KP<double> kp64;
     lbm::KP<float> kp32;
-    bool walls, forced;
+    bool walls;
+    int forced;           // 0 no force, 1 Guo forcing, 2 velocity-shift forcing (kernel variant)
     bool inited;
     int64_t t;
     int64_t launches;
@@ -153,6 +154,7 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     for (int s = 0; s < 2; ++s) {
         k.omega[s] = (R)(1.0 / p.tau[s]);
         k.cf[s] = (R)(1.0 - 0.5 / p.tau[s]);
+        k.tau[s] = (R)p.tau[s];
         for (int t = 0; t < 2; ++t) k.G[s][t] = (R)p.G[s][t];
     }
     const double w0s = p.w0_scalar > 0.0 ? p.w0_scalar : (c->lattice == LBM_D3Q19 ? 0.25 : 0.4);
@@ -381,7 +383,8 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->h = sh.scalar ? c->ws + sh.f_bytes : nullptr;
     c->psi = sh.sc ? c->ws + sh.f_bytes + sh.h_bytes : nullptr;
     c->walls = p->bc[0] || p->bc[1] || p->bc[2];
-    c->forced = sh.sc || p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0;
+    c->forced = (sh.sc || p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
+    if (p->forcing == 1) c->forced = 2;       // its own arithmetic even when the force is zero
     if (p->precision == 64) c->ops = lattice == LBM_D3Q19 ? lbm::ops_f64_d3q19() : lbm::ops_f64_d2q9();
     else c->ops = lattice == LBM_D3Q19 ? lbm::ops_f32_d3q19() : lbm::ops_f32_d2q9();
     fill_kp(c->kp64, c);
@@ -628,6 +631,7 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
         wave_free(c);
         return 0;
     }
+    if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
     if (path == LBM_PATH_WAVEFRONT) {
         if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
     } else if (path == LBM_PATH_PIPELINE) {

@@ -70,7 +70,8 @@ def test_workspace_is_one_population_copy_plus_psi(lbm, name, expect):
     ((8, 8, 8), "D3Q19", "SC2_ADE", dict(tau_c=0.4, bc=(0, 0, 0)), "tau_c"),
     ((0, 8, 8), "D3Q19", "BGK", {}, "extents"),
     ((2048, 2048, 1024), "D3Q19", "BGK", {}, "2^31"),
-    ((8, 8, 8), "D3Q19", "BGK", dict(forcing=1), "Guo"),
+    ((8, 8, 8), "D3Q19", "BGK", dict(forcing=2), "forcing"),
+    ((1024, 1024, 512), "D3Q19", "BGK", {}, "2^32"),
     ((8, 8, 8), "D3Q19", "SC2", dict(psi_kind=2, bc=(0, 0, 0)), "psi_kind"),
     ((8, 8, 8), "D3Q19", "SC1", dict(psi_kind=0, rho0_psi=0.0, bc=(0, 0, 0)), "rho0_psi"),
     ((8, 8, 1), "D2Q9", "BGK", dict(bc=(0, 0, 1)), "bc[2]"),

@@ -81,6 +81,15 @@ SMALL = [
     ("cfg5", (33, 17, 9), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
     ("cfg3", (16, 8, 1), dict(precision=32)),
+    # Shan-Chen velocity-shift forcing scheme (forcing = 1, Eq. 16-19)
+    ("cfg1", (9, 6, 1), dict(forcing=1, bc=(0, 1, 0), force=(2e-5, 0.0, 0.0))),
+    ("cfg1", (8, 8, 1), dict(forcing=1)),
+    ("cfg2", (33, 17, 1), dict(forcing=1, radius=5.0)),
+    ("cfg3", (33, 17, 1), dict(forcing=1, force=(1e-5, 2e-5, 0.0), tau=(0.8, 1.3))),
+    ("cfg4", (5, 4, 7), dict(forcing=1, bc=(1, 0, 1))),
+    ("cfg4", (33, 17, 9), dict(forcing=1, precision=32)),
+    ("cfg5", (33, 17, 9), dict(forcing=1, rmin=2.0, rmax=4.0, vol_frac=0.1, tau=(0.9, 1.2))),
+    ("cfg5", (12, 9, 7), dict(forcing=1, rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
 ]
 
 
