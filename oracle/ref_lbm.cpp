@@ -148,7 +148,8 @@ struct Sim : ref_ctx {
     /* constants, rounded once to R */
     R w[19], ws[7];
     R omega[2], cf[2], tau_r[2], omega_c, inv_cs2g;
-    R G[2][2], rho0_psi, force[3], k_react;
+    R G[2][2], G_ads[2], rho0_psi, force[3], k_react;
+    bool has_walls;
 
     /* fields */
     std::vector<R> f, fnew;        /* [sigma][i][cell] */
@@ -167,6 +168,7 @@ struct Sim : ref_ctx {
         Ls = make_scalar_lattice(lattice, w0s);
         S = (model == REF_SC2 || model == REF_SC2_ADE) ? 2 : 1;
         has_sc = (model != REF_BGK);
+        has_walls = pp.bc[0] || pp.bc[1] || pp.bc[2];
         has_scalar = (model == REF_SC2_ADE);
         d = L.d; Q = L.Q; Qs = Ls.Q;
         N = (size_t)nx * ny * nz;
@@ -175,6 +177,7 @@ struct Sim : ref_ctx {
         for (int s = 0; s < 2; ++s) {
             omega[s] = (R)(1.0 / pp.tau[s]);              /* 1/tau, Eq. 15 */
             tau_r[s] = (R)pp.tau[s];
+            G_ads[s] = (R)pp.G_ads[s];
             cf[s] = (R)(1.0 - 0.5 / pp.tau[s]);           /* 1 - 1/(2 tau), Eq. 15 */
             for (int t = 0; t < 2; ++t) G[s][t] = (R)pp.G[s][t];
         }
@@ -250,13 +253,21 @@ struct Sim : ref_ctx {
                     for (int s = 1; s < S; ++s) rho_t = rho_t + rho[(size_t)s * N + cell];
                     R inv_rho = (R)1 / rho_t;
                     R acc[2][3] = {{(R)0, (R)0, (R)0}, {(R)0, (R)0, (R)0}};
+                    R adh[3] = {(R)0, (R)0, (R)0};   /* sum_i w_i s(x + c_i) c_i over solid neighbours, Eq. 14 */
                     if (has_sc) {
                         for (int t = 0; t < S; ++t)
                             for (int i = 1; i < Q; ++i) {
                                 size_t nb;
-                                if (!neighbour(x, y, z, L.c[i], nb)) continue; /* create() rejects SC + walls */
+                                /* Eq. 11 / 12 sum over FLUID neighbours only: a node beyond a wall is solid */
+                                if (!neighbour(x, y, z, L.c[i], nb)) continue;
                                 R wp = w[i] * psi[(size_t)t * N + nb];
                                 for (int a = 0; a < d; ++a) acc[t][a] = acc[t][a] + wp * (R)L.c[i][a];
+                            }
+                        if (has_walls)
+                            for (int i = 1; i < Q; ++i) {
+                                size_t nb;
+                                if (neighbour(x, y, z, L.c[i], nb)) continue;
+                                for (int a = 0; a < d; ++a) adh[a] = adh[a] + w[i] * (R)L.c[i][a];
                             }
                     }
                     for (int s = 0; s < S; ++s)
@@ -266,6 +277,8 @@ struct Sim : ref_ctx {
                                 R t = G[s][0] * acc[0][a];
                                 if (S == 2) t = t + G[s][1] * acc[1][a];
                                 Fa = -(psi[(size_t)s * N + cell] * t);
+                                /* fluid-solid adhesion, Eq. 14: -G_ads rho^s sum_i w_i s c_i */
+                                if (has_walls) Fa = Fa + (-((G_ads[s] * rho[(size_t)s * N + cell]) * adh[a]));
                             }
                             /* constant body-force density; split by mass fraction for S=2 (DESIGN R5) */
                             R Fext = (S == 1) ? force[a] : force[a] * (rho[(size_t)s * N + cell] * inv_rho);
@@ -555,7 +568,7 @@ ref_ctx* ref_create(int nx, int ny, int nz, int lattice, int model, const ref_pa
     if (model == REF_SC2_ADE && !(p->tau_c > 0.5)) { g_err = "tau_c must exceed 0.5"; return nullptr; }
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != 0 && p->bc[a] != 1) { g_err = "bad bc"; return nullptr; }
-        if (p->bc[a] == 1 && model != REF_BGK) { g_err = "Shan-Chen models with walls are not implemented"; return nullptr; }
+
     }
     if (lattice == REF_D2Q9 && p->bc[2] != 0) { g_err = "2D: bc[2] must be 0"; return nullptr; }
     if (model != REF_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) { g_err = "rho0_psi must be > 0"; return nullptr; }

@@ -48,6 +48,7 @@ typedef struct ref_params {
     double   rho_init[2];
     double   c_init;
     double   rho_in, rho_out, radius, width, noise_amp, u0, rmin, rmax, vol_frac;
+    double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14; solid = beyond a wall */
 } ref_params;
 
 typedef struct ref_ctx ref_ctx;

@@ -670,7 +670,7 @@ def test_errors():
     with pytest.raises(ValueError):
         RefLBM(4, 4, 1, "D2Q9", "BGK", tau=(0.5, 1.0))
     with pytest.raises(ValueError):
-        RefLBM(4, 4, 1, "D2Q9", "SC1", bc=(0, 1, 0))               # Shan-Chen with walls: not implemented
+        RefLBM(4, 4, 1, "D2Q9", "BGK", forcing=2)
     r = RefLBM(4, 4, 1, "D2Q9", "BGK")
     with pytest.raises(RuntimeError):
         r.step(1)                                                    # step before init
@@ -754,3 +754,99 @@ def test_velocity_shift_uniform_state_is_stationary():
     f0 = r.get_populations().copy()
     r.step(25)
     assert np.abs(r.get_populations() - f0).max() < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# Shan-Chen models between bounce-back walls: fluid-only stencil (Eq. 11-12) and the
+# fluid-solid adhesion force (Eq. 14); the nodes beyond a wall face are the solid nodes
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lattice,grid,bc", [("D2Q9", (6, 7, 1), (0, 1, 0)), ("D3Q19", (5, 4, 6), (0, 0, 1)), ("D3Q19", (5, 6, 4), (1, 1, 0))])
+def test_adhesion_force_closed_form(lattice, grid, bc):
+    """G = 0, uniform rho: F_ads = -G_ads rho sum_i w_i s(x + c_i) c_i.  Next to one flat wall the solid
+    neighbours are the directions pointing into it: sum_i w_i c_i = -n/6 for D2Q9 (1/9 + 2/36) and D3Q19
+    (1/18 + 4/36) alike, n the inward wall normal; in an edge between two walls the face diagonal pointing into
+    both is counted once: by brute force over the lattice table."""
+    gads = (-0.3, 0.45)
+    rho = (0.8, 1.3)
+    r = RefLBM(*grid, lattice, "SC2", precision=64, tau=(1.0, 1.0), psi_kind=1, G=((0, 0), (0, 0)), G_ads=gads, bc=bc,
+               init_kind="REST", rho_init=rho)
+    r.init_from_seed(0)
+    F = r.get_force().reshape(2, r.d, grid[2], grid[1], grid[0])
+    c, w = lattice_table(lattice)
+    n = (grid[0], grid[1], grid[2])
+    for z in range(grid[2]):
+        for y in range(grid[1]):
+            for x in range(grid[0]):
+                pos = (x, y, z)
+                s = np.zeros(3)
+                for i in range(1, len(w)):
+                    out = any(bc[a] and not (0 <= pos[a] + c[i][a] < n[a]) for a in range(3))
+                    if out:
+                        s += w[i] * c[i]
+                for sg in range(2):
+                    for a in range(r.d):
+                        assert abs(F[sg, a, z, y, x] - (-gads[sg] * rho[sg] * s[a])) < 1e-15
+    # one flat wall: magnitude G_ads rho / 6 along the normal
+    a = bc.index(1)
+    idx = [slice(None)] * 3
+    if sum(bc) == 1:
+        lo = F[0, a].take(0, axis=2 - a)
+        assert np.allclose(lo, -gads[0] * rho[0] * (-1.0 / 6.0), atol=1e-15)
+
+
+@pytest.mark.parametrize("model,lattice,grid,bc", [("SC1", "D2Q9", (12, 10, 1), (0, 1, 0)), ("SC2", "D2Q9", (10, 12, 1), (1, 1, 0)),
+                                                   ("SC2_ADE", "D3Q19", (6, 6, 7), (0, 0, 1))])
+def test_shan_chen_between_walls_conserves_mass_and_stencil_skips_solid(model, lattice, grid, bc):
+    """Bounce-back returns every population, so the mass of each component is invariant also with the adhesion
+    force; and the interaction force of a fluid node next to a wall equals the literal pair sum of Eq. 9 over
+    the FLUID nodes only (Eq. 11: sum over fluid neighbours) plus the adhesion term."""
+    gads = (-0.2, 0.3)
+    r = noise_cfg(model, lattice, grid, tau=(0.9, 1.1), bc=bc, G_ads=gads)
+    r.init_from_seed(3)
+    f, _ = r.split_populations(r.get_populations())
+    m0 = f.sum(axis=(1, 2))
+    # force against brute force
+    rho = f.sum(1)                                            # [S][N]
+    psi = rho if model != "SC1" else 1.0 - np.exp(-rho)
+    G = np.array(workloads.G12) if model != "SC1" else np.array([[-5.0, 0.0], [0.0, 0.0]])
+    c, w = lattice_table(lattice)
+    nx, ny, nz = grid
+    F = r.get_force().reshape(r.S, r.d, nz, ny, nx)
+    P = psi.reshape(r.S, nz, ny, nx)
+    Rh = rho.reshape(r.S, nz, ny, nx)
+    n = (nx, ny, nz)
+    rng = np.random.default_rng(0)
+    for _ in range(60):
+        x, y, z = int(rng.integers(nx)), int(rng.integers(ny)), int(rng.integers(nz))
+        pos = (x, y, z)
+        for s in range(r.S):
+            acc = np.zeros(3)
+            adh = np.zeros(3)
+            for i in range(1, len(w)):
+                q = [pos[a] + c[i][a] for a in range(3)]
+                if any(bc[a] and not (0 <= q[a] < n[a]) for a in range(3)):
+                    adh += w[i] * c[i]
+                    continue
+                q = [q[a] % n[a] for a in range(3)]
+                for t in range(r.S):
+                    acc += G[s][t] * w[i] * P[t, q[2], q[1], q[0]] * c[i]
+            expect = -P[s, z, y, x] * acc - gads[s] * Rh[s, z, y, x] * adh
+            assert np.allclose(F[s, :, z, y, x], expect[:r.d], rtol=1e-12, atol=1e-16)
+    r.step(300)
+    f, _ = r.split_populations(r.get_populations())
+    assert np.abs(f.sum(axis=(1, 2)) - m0).max() / m0.max() < 1e-13
+    assert np.isfinite(f).all()
+
+
+def test_wetting_and_non_wetting_wall():
+    """Eq. 14: a negative G_ads attracts the component to the wall, a positive one repels it.
+    Two-component mixture between two walls, A wetting and B non-wetting: after relaxation the wall layer is
+    enriched in A and depleted in B, symmetrically at both walls."""
+    r = RefLBM(8, 24, 1, "D2Q9", "SC2", precision=64, tau=(1.0, 1.0), psi_kind=1, G=((0, 0.9), (0.9, 0)),
+               G_ads=(-0.3, 0.3), bc=(0, 1, 0), init_kind="REST", rho_init=(1.0, 1.0))
+    r.init_from_seed(0)
+    r.step(3000)
+    rho = r.get_macros()["rho"].reshape(2, 24, 8)
+    assert np.abs(rho - rho[:, :, :1]).max() < 1e-10           # stays x-invariant
+    assert np.allclose(rho, rho[:, ::-1, :], rtol=1e-9)        # and symmetric
+    assert rho[0, 0, 0] > rho[0, 12, 0] * 1.02 and rho[1, 0, 0] < rho[1, 12, 0] * 0.98
