@@ -67,8 +67,9 @@ typedef struct lbm_params {
                                (PAPER.md:154-174): u_eq = u' + tau F / rho, no F_i term; LBM_PATH_REGISTER only */
     double   rho0_psi;      /* rho0 of Eq. 10 */
     double   force[3];      /* constant body-force density; S = 2: split by mass fraction (R5) */
-    int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls on both faces;
-                               walls are accepted for LBM_BGK only */
+    int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls on both faces.
+                               For Shan-Chen models the nodes beyond a wall are solid: left out of the psi
+                               stencil (Eq. 11-12) and the source of the adhesion force (G_ads, Eq. 14) */
     int32_t  init_kind;     /* LBM_INIT_* */
     double   k_react;       /* k of the source R = -k C 4 rhoA rhoB/(rhoA+rhoB)^2 (R8) */
     double   w0_scalar;     /* rest weight of the scalar lattice; 0 -> 0.4 (D2Q5) / 0.25 (D3Q7) */
@@ -79,6 +80,8 @@ typedef struct lbm_params {
     double   noise_amp;         /* relative amplitude of the seeded uniform noise */
     double   u0;                /* TAYLOR_GREEN velocity amplitude */
     double   rmin, rmax, vol_frac;  /* RANDOM_DROPLETS: radius range and target volume fraction */
+    double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14:
+                               F_ads = -G_ads rho sum_i w_i s(x + c_i) c_i; < 0 wetting, > 0 non-wetting */
     void*    workspace;     /* DEVICE memory of >= lbm_workspace_bytes() bytes, 256-byte aligned (e.g. from
                                torch), or NULL: the library allocates (cudaMalloc) and frees it */
     void*    stream;        /* cudaStream_t, or NULL for the legacy default stream */

@@ -11,7 +11,7 @@ struct PipeArgs;
 
 struct Ops {
     // kp points at a KP<R> of the matching precision
-    cudaError_t (*psi)(const void* kp, int model, int parity, cudaStream_t st);
+    cudaError_t (*psi)(const void* kp, int model, int parity, int walls, cudaStream_t st);
     cudaError_t (*step)(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st);
     cudaError_t (*macros)(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
                           void* F, cudaStream_t st);

@@ -25,12 +25,13 @@ inline dim3 grid_for(const KP<R>& p) { const int b = block_for(p); return dim3((
 template <class R, class L>
 struct Launch {
     template <int MODEL, int PARITY>
-    static void psi2(const KP<R>& p, cudaStream_t st) {
-        k_psi<R, L, MODEL, PARITY><<<grid_for(p), block_for(p), 0, st>>>(p);
+    static void psi2(const KP<R>& p, int walls, cudaStream_t st) {
+        if (walls) k_psi<R, L, MODEL, PARITY, true><<<grid_for(p), block_for(p), 0, st>>>(p);
+        else k_psi<R, L, MODEL, PARITY, false><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
-    static cudaError_t psi(const void* kp, int model, int parity, cudaStream_t st) {
+    static cudaError_t psi(const void* kp, int model, int parity, int walls, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
-#define LBM_PSI(M) case M: parity ? psi2<M, 1>(p, st) : psi2<M, 0>(p, st); break;
+#define LBM_PSI(M) case M: parity ? psi2<M, 1>(p, walls, st) : psi2<M, 0>(p, walls, st); break;
         switch (model) { LBM_PSI(M_SC1) LBM_PSI(M_SC2) LBM_PSI(M_SC2_ADE) default: return cudaErrorInvalidValue; }
 #undef LBM_PSI
         return cudaGetLastError();
@@ -47,9 +48,9 @@ struct Launch {
         if (forced == 2) {
             switch (model) {
             case M_BGK: if (walls) step3<M_BGK, true, true, true>(p, parity, st); else step3<M_BGK, false, true, true>(p, parity, st); break;
-            case M_SC1: step3<M_SC1, false, true, true>(p, parity, st); break;
-            case M_SC2: step3<M_SC2, false, true, true>(p, parity, st); break;
-            case M_SC2_ADE: step3<M_SC2_ADE, false, true, true>(p, parity, st); break;
+            case M_SC1: if (walls) step3<M_SC1, true, true, true>(p, parity, st); else step3<M_SC1, false, true, true>(p, parity, st); break;
+            case M_SC2: if (walls) step3<M_SC2, true, true, true>(p, parity, st); else step3<M_SC2, false, true, true>(p, parity, st); break;
+            case M_SC2_ADE: if (walls) step3<M_SC2_ADE, true, true, true>(p, parity, st); else step3<M_SC2_ADE, false, true, true>(p, parity, st); break;
             default: return cudaErrorInvalidValue;
             }
             return cudaGetLastError();
@@ -59,9 +60,9 @@ struct Launch {
             if (walls) { if (forced) step3<M_BGK, true, true>(p, parity, st); else step3<M_BGK, true, false>(p, parity, st); }
             else { if (forced) step3<M_BGK, false, true>(p, parity, st); else step3<M_BGK, false, false>(p, parity, st); }
             break;
-        case M_SC1: step3<M_SC1, false, true>(p, parity, st); break;
-        case M_SC2: step3<M_SC2, false, true>(p, parity, st); break;
-        case M_SC2_ADE: step3<M_SC2_ADE, false, true>(p, parity, st); break;
+        case M_SC1: if (walls) step3<M_SC1, true, true>(p, parity, st); else step3<M_SC1, false, true>(p, parity, st); break;
+        case M_SC2: if (walls) step3<M_SC2, true, true>(p, parity, st); else step3<M_SC2, false, true>(p, parity, st); break;
+        case M_SC2_ADE: if (walls) step3<M_SC2_ADE, true, true>(p, parity, st); else step3<M_SC2_ADE, false, true>(p, parity, st); break;
         default: return cudaErrorInvalidValue;
         }
         return cudaGetLastError();
@@ -78,9 +79,9 @@ struct Launch {
         R *r = (R*)rho, *uu = (R*)u, *ph = (R*)phi, *c = (R*)C, *f = (R*)F;
         switch (model) {
         case M_BGK: if (walls) macros2<M_BGK, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_BGK, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC1: macros2<M_SC1, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC2: macros2<M_SC2, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC2_ADE: macros2<M_SC2_ADE, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC1: if (walls) macros2<M_SC1, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC1, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC2: if (walls) macros2<M_SC2, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC2, false>(p, parity, r, uu, ph, c, f, st); break;
+        case M_SC2_ADE: if (walls) macros2<M_SC2_ADE, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC2_ADE, false>(p, parity, r, uu, ph, c, f, st); break;
         default: return cudaErrorInvalidValue;
         }
         return cudaGetLastError();

@@ -42,6 +42,7 @@ struct KP {
     R omega_c, inv_cs2g;      // 1/tau_c (Eq. 34), 1/c_{s,g}^2 = d/(1-w0) (Eq. 35, R6)
     R ws0, ws1;               // scalar-lattice weights
     R G[2][2];
+    R G_ads[2];               // fluid-solid adhesion, Eq. 14
     R rho0_psi;
     R force[3];
     R k_react;
@@ -69,6 +70,7 @@ template <int MODEL> struct ModelTraits {
 // ------------------------------------------------------------------------------------------
 template <int D, bool WALLS>
 struct Nbr {
+    static constexpr bool HAS_WALLS = WALLS;
     int cell;              // x + nx*(y + ny*z)
     int xx[3];             // x-1, x, x+1 with periodic wrap (per thread)
     int ry[3], rz[3];      // nx*y', nx*ny*z' for y' = y-1,y,y+1 / z' = z-1,z,z+1 with wrap (uniform)
@@ -214,6 +216,8 @@ __device__ __forceinline__ R load_psi(const R* q) {
     if constexpr (COH) return __ldcg(q); else return __ldg(q);
 }
 
+// Neighbours beyond a bounce-back wall are solid nodes: they are left out of the sum (Eq. 11-12: sum over FLUID
+// neighbours; adding an exact zero instead of skipping changes no bit).
 template <class L, int S, bool COH, class R, class NB>
 __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& nb, size_t N, R (*acc)[3]) {
     static_for<0, S>([&](auto tc) {
@@ -223,7 +227,8 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
         static_for<1, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-            const R wp = (R)L::w(i) * load_psi<COH>(ps + ((unsigned)nb.template row<CY, CZ>() + (unsigned)nb.template col<CX>()));
+            R wp = (R)L::w(i) * load_psi<COH>(ps + ((unsigned)nb.template row<CY, CZ>() + (unsigned)nb.template col<CX>()));
+            if (nb.template outside<CX, CY, CZ>()) wp = (R)0;
             static_for<0, L::D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 constexpr int c = L::c(i, a);
@@ -232,6 +237,22 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
                     else acc[t][a] = c > 0 ? acc[t][a] + wp : acc[t][a] - wp;
                 }
             });
+        });
+    });
+}
+
+// adh[a] = sum_{i>=1} w_i s(x + c_i) c_{i,a}, s = 1 for the solid nodes beyond a wall: Eq. 14
+template <class L, class R, class NB>
+__device__ __forceinline__ void adhesion_sum(const NB& nb, R* adh) {
+    adh[0] = adh[1] = adh[2] = (R)0;
+    static_for<1, L::Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
+        const R ws = nb.template outside<CX, CY, CZ>() ? (R)L::w(i) : (R)0;
+        static_for<0, L::D>([&](auto ac) {
+            constexpr int a = decltype(ac)::value;
+            constexpr int c = L::c(i, a);
+            if constexpr (c != 0) adh[a] = c > 0 ? adh[a] + ws : adh[a] - ws;
         });
     });
 }
@@ -251,9 +272,9 @@ struct CellMacro {
 
 // steps a1, a3 (given the stencil sums), a4: moments, force, barycentric velocity.
 // acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a} and psi_own[s] = psi^s(x) are read only for Shan-Chen models.
-template <class R, class L, int MODEL, bool FORCED>
+template <class R, class L, int MODEL, bool FORCED, bool ADH = false>
 __device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L::Q], const R (*acc)[3], const R* psi_own,
-                                                 CellMacro<R, L, MODEL>& m) {
+                                                 CellMacro<R, L, MODEL>& m, const R* adh = nullptr) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
     R (&j)[S][3] = m.j;
@@ -275,6 +296,8 @@ __device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L
                     R t = p.G[s][0] * acc[0][a];
                     if constexpr (S == 2) t = t + p.G[s][1] * acc[1][a];
                     Fa = -(psi_own[s] * t);
+                    // fluid-solid adhesion at bounce-back walls, Eq. 14
+                    if constexpr (ADH) Fa = Fa + (-((p.G_ads[s] * m.rho[s]) * adh[a]));
                 }
                 // constant body-force density, split by mass fraction for S = 2 (R5)
                 R Fext;
@@ -304,15 +327,17 @@ __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const 
     constexpr int S = ModelTraits<MODEL>::S;
     constexpr bool SC = ModelTraits<MODEL>::SC;
     const size_t N = (size_t)p.N;
-    R acc[S][3], psi_own[S];
+    R acc[S][3], psi_own[S], adh[3];
+    constexpr bool ADH = FORCED && SC && NB::HAS_WALLS;
     if constexpr (FORCED && SC) {
         sc_stencil<L, S, COH>(p.psi, nb, N, acc);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
             psi_own[s] = load_psi<COH>(p.psi + ((size_t)s * N + nb.cell));
         });
+        if constexpr (ADH) adhesion_sum<L>(nb, adh);
     }
-    cell_macros_core<R, L, MODEL, FORCED>(p, fl, acc, psi_own, m);
+    cell_macros_core<R, L, MODEL, FORCED, ADH>(p, fl, acc, psi_own, m, adh);
 }
 
 // step a5 for one component: f* = f - (f - f^eq)/tau + (1 - 1/(2 tau)) F_i
@@ -392,27 +417,27 @@ __device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB
 // psi pass (step a2): rho^sigma from the populations at the current parity, psi^sigma to HBM
 // ------------------------------------------------------------------------------------------
 // psi^sigma of the cell (x,y,z) at the current parity
-template <class R, class L, int MODEL, int PARITY>
+template <class R, class L, int MODEL, int PARITY, bool WALLS = false>
 __device__ __forceinline__ void psi_cell(const KP<R>& p, int x, int y, int z) {
     constexpr int S = ModelTraits<MODEL>::S, Q = L::Q;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, false> nb(p, x, y, z);
+    const Nbr<L::D, WALLS> nb(p, x, y, z);
     const int cell = nb.cell;
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         R fl[Q];
-        load_pops<L, PARITY, false>(p.f + (size_t)s * Q * N, nb, N, fl);
+        load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl);
         R rho, j[3];
         moments<L>(fl, rho, j);
         p.psi[(size_t)s * N + cell] = psi_of(rho, p.psi_kind, p.rho0_psi);
     });
 }
 
-template <class R, class L, int MODEL, int PARITY>
+template <class R, class L, int MODEL, int PARITY, bool WALLS = false>
 __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
-    psi_cell<R, L, MODEL, PARITY>(p, x, y, z);
+    psi_cell<R, L, MODEL, PARITY, WALLS>(p, x, y, z);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -521,13 +546,15 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
 #ifndef LBM_MINB_BGK64
 #define LBM_MINB_BGK64 6
 #endif
-template <class R, int MODEL> struct StepBounds {
+template <class R, int MODEL, int Q = 9> struct StepBounds {
     static constexpr int THREADS = 128;
-    static constexpr int MINB = MODEL == M_BGK ? (sizeof(R) == 4 ? LBM_MINB_BGK32 : LBM_MINB_BGK64) : (MODEL == M_SC1 ? 6 : 5);
+    // two-component D3Q19 in fp64 holds 2 x 19 doubles per thread: 3 blocks (170 registers) avoid the spills of 5
+    static constexpr int MINB = MODEL == M_BGK ? (sizeof(R) == 4 ? LBM_MINB_BGK32 : LBM_MINB_BGK64)
+                              : (MODEL == M_SC1 ? 6 : (sizeof(R) == 8 && Q == 19 ? 3 : 5));
 };
 
 template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool VSHIFT = false>
-__global__ void __launch_bounds__(StepBounds<R, MODEL>::THREADS, StepBounds<R, MODEL>::MINB) k_step(const __grid_constant__ KP<R> p) {
+__global__ void __launch_bounds__(StepBounds<R, MODEL, L::Q>::THREADS, StepBounds<R, MODEL, L::Q>::MINB) k_step(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
     step_cell<R, L, MODEL, PARITY, WALLS, FORCED, false, VSHIFT>(p, x, y, z);

@@ -63,7 +63,6 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (model == LBM_SC2_ADE && !(p->tau_c > 0.5)) return "tau_c must exceed 0.5";
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != 0 && p->bc[a] != 1) return "bc must be 0 (periodic) or 1 (bounce-back walls)";
-        if (p->bc[a] == 1 && model != LBM_BGK) return "Shan-Chen models with walls are not implemented";
     }
     if (lattice == LBM_D2Q9 && p->bc[2] != 0) return "2D: bc[2] must be 0";
     if (model != LBM_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) return "rho0_psi must be > 0";
@@ -156,6 +155,7 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
         k.cf[s] = (R)(1.0 - 0.5 / p.tau[s]);
         k.tau[s] = (R)p.tau[s];
         for (int t = 0; t < 2; ++t) k.G[s][t] = (R)p.G[s][t];
+        k.G_ads[s] = (R)p.G_ads[s];
     }
     const double w0s = p.w0_scalar > 0.0 ? p.w0_scalar : (c->lattice == LBM_D3Q19 ? 0.25 : 0.4);
     k.omega_c = (R)(1.0 / p.tau_c);
@@ -216,7 +216,7 @@ void drop_events(lbm_ctx* c) {
 int run_psi(lbm_ctx* c) {
     int rc = mark(c, 1);
     if (rc) return rc;
-    CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->stream));
+    CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->walls, c->stream));
     c->launches++;
     return mark(c, 1);
 }
@@ -440,7 +440,7 @@ constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far l
 
 // the kernels of one time step of the register path, enqueued on st (no event marks, no counters)
 int enqueue_register_step(lbm_ctx* c, int parity, cudaStream_t st) {
-    if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, st));
+    if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, c->walls, st));
     CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, st));
     return 0;
 }
@@ -632,6 +632,7 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
         return 0;
     }
     if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
+    if (c->sh.sc && c->walls) return fail(LBM_EINVAL, "Shan-Chen models between walls run on LBM_PATH_REGISTER only");
     if (path == LBM_PATH_WAVEFRONT) {
         if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
     } else if (path == LBM_PATH_PIPELINE) {

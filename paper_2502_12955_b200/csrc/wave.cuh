@@ -12,7 +12,7 @@
 namespace lbm {
 
 template <class R, class L, int MODEL, int PARITY>
-__global__ void __launch_bounds__(PIPE_TX, StepBounds<R, MODEL>::MINB) k_wave(const __grid_constant__ KP<R> p,
+__global__ void __launch_bounds__(PIPE_TX, StepBounds<R, MODEL, L::Q>::MINB) k_wave(const __grid_constant__ KP<R> p,
                                                                          const __grid_constant__ PipeArgs w) {
     using LS = typename ScalarOf<L>::type;
     constexpr int D = L::D, S = ModelTraits<MODEL>::S;

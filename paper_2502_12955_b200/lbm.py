@@ -39,7 +39,7 @@ class LbmParams(C.Structure):
         ("rho_init", C.c_double * 2), ("c_init", C.c_double),
         ("rho_in", C.c_double), ("rho_out", C.c_double), ("radius", C.c_double), ("width", C.c_double),
         ("noise_amp", C.c_double), ("u0", C.c_double), ("rmin", C.c_double), ("rmax", C.c_double),
-        ("vol_frac", C.c_double),
+        ("vol_frac", C.c_double), ("G_ads", C.c_double * 2),
         ("workspace", C.c_void_p), ("stream", C.c_void_p),
     ]
 
@@ -130,6 +130,8 @@ def make_params(**kw):
     for k, dflt in (("rho_in", 1.0), ("rho_out", 1.0), ("radius", 0.0), ("width", 3.0), ("noise_amp", 0.0),
                     ("u0", 0.0), ("rmin", 0.0), ("rmax", 0.0), ("vol_frac", 0.0)):
         setattr(p, k, float(kw.get(k, dflt)))
+    ga = kw.get("G_ads", (0.0, 0.0))
+    p.G_ads[0], p.G_ads[1] = float(ga[0]), float(ga[1])
     p.workspace = None
     p.stream = None
     return p

@@ -64,7 +64,6 @@ def test_workspace_is_one_population_copy_plus_psi(lbm, name, expect):
 
 @pytest.mark.parametrize("grid,lattice,model,over,msg", [
     ((8, 8, 2), "D2Q9", "BGK", {}, "nz == 1"),
-    ((8, 8, 1), "D2Q9", "SC1", dict(bc=(1, 0, 0)), "walls"),
     ((8, 8, 8), "D3Q19", "BGK", dict(tau=(0.5, 0.5)), "tau"),
     ((8, 8, 8), "D3Q19", "BGK", dict(precision=16), "precision"),
     ((8, 8, 8), "D3Q19", "SC2_ADE", dict(tau_c=0.4, bc=(0, 0, 0)), "tau_c"),

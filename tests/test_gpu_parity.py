@@ -81,6 +81,12 @@ SMALL = [
     ("cfg5", (33, 17, 9), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
     ("cfg3", (16, 8, 1), dict(precision=32)),
+    # Shan-Chen models between bounce-back walls: fluid-only stencil + adhesion force (Eq. 11-12, 14)
+    ("cfg2", (33, 17, 1), dict(radius=5.0, bc=(0, 1, 0), G_ads=(-0.4, 0.0))),
+    ("cfg3", (16, 9, 1), dict(bc=(1, 1, 0), G_ads=(-0.2, 0.3), force=(1e-5, -2e-5, 0.0))),
+    ("cfg3", (9, 12, 1), dict(bc=(0, 1, 0), G_ads=(0.25, -0.25), forcing=1, tau=(0.8, 1.2))),
+    ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 0, 1), G_ads=(-0.3, 0.3))),
+    ("cfg5", (7, 6, 5), dict(rmin=1.0, rmax=2.0, vol_frac=0.2, bc=(1, 1, 1), G_ads=(0.1, -0.2), precision=64, tau=(0.9, 1.1))),
     # Shan-Chen velocity-shift forcing scheme (forcing = 1, Eq. 16-19)
     ("cfg1", (9, 6, 1), dict(forcing=1, bc=(0, 1, 0), force=(2e-5, 0.0, 0.0))),
     ("cfg1", (8, 8, 1), dict(forcing=1)),
@@ -366,8 +372,9 @@ def test_errors_and_state(gpu):
     assert "scalar" in gpu.lbm.last_error()
     with pytest.raises(gpu.LbmError):
         gpu.LBM(8, 8, 2, "D2Q9", "BGK")               # D2Q9 needs nz == 1
+    sc = gpu.LBM(8, 8, 1, "D2Q9", "SC1", bc=(1, 0, 0))
     with pytest.raises(gpu.LbmError):
-        gpu.LBM(8, 8, 1, "D2Q9", "SC1", bc=(1, 0, 0))  # Shan-Chen + walls: not implemented
+        sc.set_path("wavefront")                      # Shan-Chen between walls: register path only
 
 
 PATH_CASES = [
