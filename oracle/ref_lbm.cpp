@@ -149,6 +149,8 @@ struct Sim : ref_ctx {
     R w[19], ws[7];
     R omega[2], cf[2], tau_r[2], omega_c, inv_cs2g;
     R G[2][2], G_ads[2], rho0_psi, force[3], k_react;
+    R wall_u[3][2][3];
+    bool moving_walls;
     bool has_walls;
 
     /* fields */
@@ -169,6 +171,13 @@ struct Sim : ref_ctx {
         S = (model == REF_SC2 || model == REF_SC2_ADE) ? 2 : 1;
         has_sc = (model != REF_BGK);
         has_walls = pp.bc[0] || pp.bc[1] || pp.bc[2];
+        moving_walls = false;
+        for (int a = 0; a < 3; ++a)
+            for (int sd = 0; sd < 2; ++sd)
+                for (int b = 0; b < 3; ++b) {
+                    wall_u[a][sd][b] = (R)pp.wall_u[a][sd][b];
+                    if (pp.bc[a] == 1 && pp.wall_u[a][sd][b] != 0.0) moving_walls = true;
+                }
         has_scalar = (model == REF_SC2_ADE);
         d = L.d; Q = L.Q; Qs = Ls.Q;
         N = (size_t)nx * ny * nz;
@@ -210,6 +219,15 @@ struct Sim : ref_ctx {
         }
         out = cell_of(q[0], q[1], q[2]);
         return true;
+    }
+
+    /* velocity of the wall a population leaving (x, y, z) along c hits: the first wall axis (x, y, z order) it crosses */
+    const R* wall_velocity(int x, int y, int z, const int* c) const {
+        const int q[3] = {x + c[0], y + c[1], z + c[2]};
+        const int n[3] = {nx, ny, nz};
+        for (int a = 0; a < 3; ++a)
+            if (p.bc[a] == 1 && (q[a] < 0 || q[a] >= n[a])) return wall_u[a][q[a] < 0 ? 0 : 1];
+        return wall_u[0][0];
     }
 
     /* Eq. 10 / Eq. 24, or psi = rho (DESIGN R3) */
@@ -346,7 +364,18 @@ struct Sim : ref_ctx {
                             /* 7. stream, Eq. 5; halfway bounce-back at walls */
                             size_t nb;
                             if (neighbour(x, y, z, L.c[i], nb)) F_(fnew, s, i, nb) = fstar;
-                            else F_(fnew, s, L.opp[i], cell) = fstar;
+                            else {
+                                /* moving wall: the reflected population exchanges momentum with the wall,
+                                 * f_opp(i)(x, t+1) = f*_i(x, t) - 2 w_i rho (c_i . u_w) / c_s^2 ("Bounce Back
+                                 * ... incorporating an additional term"; DESIGN R24), rho the cell's density at t */
+                                if (moving_walls) {
+                                    const R* uw = wall_velocity(x, y, z, L.c[i]);
+                                    R cuw = (R)0;
+                                    for (int a = 0; a < d; ++a) cuw = cuw + (R)L.c[i][a] * uw[a];
+                                    fstar = fstar - (((R)6 * w[i]) * rho_s) * cuw;
+                                }
+                                F_(fnew, s, L.opp[i], cell) = fstar;
+                            }
                         }
                     }
                     /* 6. scalar lattice: Eq. 34-36 + first-order source (DESIGN R8) */

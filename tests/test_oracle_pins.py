@@ -850,3 +850,49 @@ def test_wetting_and_non_wetting_wall():
     assert np.abs(rho - rho[:, :, :1]).max() < 1e-10           # stays x-invariant
     assert np.allclose(rho, rho[:, ::-1, :], rtol=1e-9)        # and symmetric
     assert rho[0, 0, 0] > rho[0, 12, 0] * 1.02 and rho[1, 0, 0] < rho[1, 12, 0] * 0.98
+
+
+# ----------------------------------------------------------------------------------------------
+# moving-wall bounce-back: Couette flow, Eq. 41, Fig. 4
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lattice,grid,axis", [("D3Q19", (1, 1, 15), 2), ("D2Q9", (1, 15, 1), 1), ("D3Q19", (2, 15, 3), 1)])
+def test_couette_linear_profile(lattice, grid, axis):
+    """Top wall moving with U in x, bottom wall at rest, halfway bounce-back: the steady LBGK solution is the
+    linear profile u_x = U (s + 1/2) / H of Eq. 41 (walls half a cell outside the first / last node), exactly."""
+    U, H, tau = 2e-2, 15, 0.8
+    bc = [0, 0, 0]
+    bc[axis] = 1
+    r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(tau, tau), bc=tuple(bc), rho_init=(1.0, 1.0),
+               wall_u={(axis, 1): (U, 0.0, 0.0)})
+    r.init_from_seed(0)
+    r.step(int(12 * H * H / ((tau - 0.5) / 3)))
+    m = r.get_macros()
+    shape = (grid[2], grid[1], grid[0])
+    ux = m["u"][0].reshape(shape)
+    s = np.arange(H)
+    exact = U * (s + 0.5) / H
+    prof = np.moveaxis(ux, 2 - axis, 0).reshape(H, -1)
+    assert np.abs(prof - exact[:, None]).max() < 1e-10 * U
+    assert np.abs(m["u"][1:]).max() < 1e-14
+    assert np.abs(m["rho"] - 1.0).max() < 1e-10
+
+
+def test_walls_moving_together_drag_the_fluid_to_plug_flow():
+    """Both walls moving with the same velocity: the only steady state is rigid motion u = U everywhere."""
+    U = (1.5e-2, -0.5e-2, 0.0)
+    r = RefLBM(3, 2, 9, "D3Q19", "BGK", precision=64, tau=(0.9, 0.9), bc=(0, 0, 1), rho_init=(1.0, 1.0),
+               wall_u={(2, 0): U, (2, 1): U})
+    r.init_from_seed(0)
+    r.step(6000)
+    u = r.get_macros()["u"]
+    for a in range(3):
+        assert np.abs(u[a] - U[a]).max() < 1e-9 * 1.5e-2
+
+
+def test_wall_at_rest_is_plain_bounce_back():
+    kw = dict(precision=64, tau=(0.7, 0.7), bc=(1, 1, 0), force=(1e-5, 2e-5, 0.0), rho_init=(1.0, 1.0))
+    a = RefLBM(6, 5, 1, "D2Q9", "BGK", **kw)
+    b = RefLBM(6, 5, 1, "D2Q9", "BGK", wall_u={(0, 0): (0.0, 0.0, 0.0)}, **kw)
+    a.init_from_seed(0); b.init_from_seed(0)
+    a.step(30); b.step(30)
+    assert np.array_equal(a.get_populations(), b.get_populations())
