@@ -342,9 +342,12 @@ def run_reference(args, cfg, key):
 # per-model lines of the default run: (key, config overrides, steps, warmup).  BASELINE.json configs
 # 1-3 at paper size are L2-resident (0.3 / 4.7 / 38 MB): their rate is launch/L2-bound and their "HBM
 # fraction" is flagged l2_resident; the 8192^2 rows run the same D2Q9 kernels HBM-bound.
+# (key, overrides, grid, steps, warmup[, path[, note]])
 EXTRAS = [
     ("cfg4", dict(precision=32), None, 1000, 50),
     ("cfg5", dict(), None, 100, 10),
+    ("cfg5", dict(), None, 40, 5, ("pipeline", 0, 0), "one-launch shared-memory pipeline (DESIGN.md 6.3)"),
+    ("cfg5", dict(), None, 40, 5, ("wavefront", 0, 0), "one-launch register wavefront (DESIGN.md 6.3)"),
     ("cfg1", dict(), None, 2000, 100),
     ("cfg2", dict(), None, 2000, 100),
     ("cfg3", dict(), None, 1000, 50),
@@ -353,6 +356,10 @@ EXTRAS = [
     ("cfg3", dict(), (8192, 8192, 1), 50, 5),
     ("cfg4", dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.05, tau=(0.5019, 0.5019)),
      (128, 128, 128), 1000, 50),
+    # paper-shaped Rayleigh-Taylor setup: two components between walls in y, gravity, 1200 x 400
+    ("cfg3", dict(bc=(0, 1, 0), force=(0.0, -1e-5, 0.0), G_ads=(0.0, 0.0)), (1200, 400, 1), 500, 50, None,
+     "Rayleigh-Taylor-shaped: walls in y + body force"),
+    ("cfg3", dict(forcing=1), (8192, 8192, 1), 50, 5, None, "velocity-shift forcing scheme (Eq. 16-19)"),
 ]
 
 
@@ -450,10 +457,15 @@ def main():
         line["e2e"] = e2e
     if not args.no_extras and world == 1:
         per = [model_line(workload_name(args.workload, cfg), cfg, r, args.steps, peak)]
-        for key, ov, grid, k, w in EXTRAS:
+        for key, ov, grid, k, w, *rest in EXTRAS:
             c = workloads.config(key, grid=grid, **ov)
-            rr = time_device(c, k, w, device, seed=1)
+            epath = rest[0] if rest else None
+            rr = time_device(c, k, w, device, seed=1, path=epath)
             ml = model_line(workload_name(key, c), c, rr, k, peak)
+            if epath is not None:
+                ml["path"] = epath[0]
+            if len(rest) > 1:
+                ml["note"] = rest[1]
             if ml["population_mb"] < 126.0:
                 ml["l2_resident"] = True
             per.append(ml)

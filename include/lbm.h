@@ -82,6 +82,10 @@ typedef struct lbm_params {
     double   rmin, rmax, vol_frac;  /* RANDOM_DROPLETS: radius range and target volume fraction */
     double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14:
                                F_ads = -G_ads rho sum_i w_i s(x + c_i) c_i; < 0 wetting, > 0 non-wetting */
+    double   wall_u[3][2][3];  /* [axis][0 low face, 1 high face][component]: velocity of that wall (used where
+                               bc[axis] == 1).  A population reflected by a moving wall loses
+                               2 w_i rho (c_i . u_w) / c_s^2 (Couette flow Eq. 41).  LBM_BGK with
+                               forcing 0 on LBM_PATH_REGISTER only */
     void*    workspace;     /* DEVICE memory of >= lbm_workspace_bytes() bytes, 256-byte aligned (e.g. from
                                torch), or NULL: the library allocates (cudaMalloc) and frees it */
     void*    stream;        /* cudaStream_t, or NULL for the legacy default stream */

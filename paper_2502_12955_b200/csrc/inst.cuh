@@ -37,14 +37,21 @@ struct Launch {
         return cudaGetLastError();
     }
 
-    template <int MODEL, bool WALLS, bool FORCED, bool VSHIFT = false>
+    template <int MODEL, bool WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
     static void step3(const KP<R>& p, int parity, cudaStream_t st) {
-        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED, VSHIFT><<<grid_for(p), block_for(p), 0, st>>>(p);
-        else k_step<R, L, MODEL, 0, WALLS, FORCED, VSHIFT><<<grid_for(p), block_for(p), 0, st>>>(p);
+        if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED, VSHIFT, MOVING><<<grid_for(p), block_for(p), 0, st>>>(p);
+        else k_step<R, L, MODEL, 0, WALLS, FORCED, VSHIFT, MOVING><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
-    // forced: 0 no force, 1 Guo forcing (Eq. 20-23), 2 Shan-Chen velocity-shift forcing (Eq. 16-19)
+    // forced: 0 no force, 1 Guo forcing (Eq. 20-23), 2 Shan-Chen velocity-shift forcing (Eq. 16-19);
+    // walls: 0 none, 1 bounce-back walls at rest, 2 moving walls (LBM_BGK without velocity shift only)
     static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
+        if (walls == 2) {
+            if (model != M_BGK || forced == 2) return cudaErrorInvalidValue;
+            if (forced) step3<M_BGK, true, true, false, true>(p, parity, st);
+            else step3<M_BGK, true, false, false, true>(p, parity, st);
+            return cudaGetLastError();
+        }
         if (forced == 2) {
             switch (model) {
             case M_BGK: if (walls) step3<M_BGK, true, true, true>(p, parity, st); else step3<M_BGK, false, true, true>(p, parity, st); break;

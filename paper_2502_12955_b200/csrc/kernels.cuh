@@ -43,6 +43,7 @@ struct KP {
     R ws0, ws1;               // scalar-lattice weights
     R G[2][2];
     R G_ads[2];               // fluid-solid adhesion, Eq. 14
+    R wall_u[3][2][3];        // velocity of the wall at the low / high face of each axis (moving-wall bounce-back)
     R rho0_psi;
     R force[3];
     R k_react;
@@ -481,9 +482,31 @@ __device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl
     }
 }
 
+// Moving-wall halfway bounce-back (DESIGN R24): a post-collision population f*_k that leaves the
+// cell through a wall comes back as f_opp(k) minus 2 w_k rho (c_k . u_w) / c_s^2.  It is stored exactly once (to
+// P_opp(k)(x), the cell's own slot), so the correction is applied to the register value before the stores.
+// u_w: the first wall axis (x, y, z order) the direction crosses.
+template <class L, class R, class NB>
+__device__ __forceinline__ void moving_wall_correction(const KP<R>& p, const NB& nb, R rho_s, R* fl) {
+    static_for<1, L::Q>([&](auto kc) {
+        constexpr int k = decltype(kc)::value;
+        constexpr int CX = L::c(k, 0), CY = L::c(k, 1), CZ = L::c(k, 2);
+        if (nb.template outside<CX, CY, CZ>()) {
+            const R* uw = p.wall_u[0][0];
+            bool found = false;
+            if constexpr (CX != 0) { if (CX < 0 ? nb.lo[0] : nb.hi[0]) { uw = p.wall_u[0][CX < 0 ? 0 : 1]; found = true; } }
+            if constexpr (CY != 0) { if (!found && (CY < 0 ? nb.lo[1] : nb.hi[1])) { uw = p.wall_u[1][CY < 0 ? 0 : 1]; found = true; } }
+            if constexpr (CZ != 0) { if (!found && (CZ < 0 ? nb.lo[2] : nb.hi[2])) { uw = p.wall_u[2][CZ < 0 ? 0 : 1]; found = true; } }
+            const R u3[3] = {uw[0], uw[1], uw[2]};
+            const R cuw = dotc<L, k>(u3);
+            fl[k] = fl[k] - (((R)6 * (R)L::w(k)) * rho_s) * cuw;
+        }
+    });
+}
+
 // both halves for one cell (k_step).  Written out rather than calling step_load / step_finish: ptxas keeps the
 // load addresses alive across the call boundary of the split form (fp32 BGK: 40 -> 80 registers).
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false, bool VSHIFT = false>
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false, bool VSHIFT = false, bool MOVING = false>
 __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
@@ -529,6 +552,7 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
         constexpr int s = decltype(sc)::value;
         if constexpr (VSHIFT) collide<R, L, false>(fl[s], m.rho[s], ueq[s], m.F[s], p.omega[s], p.cf[s]);
         else collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+        if constexpr (MOVING && WALLS) moving_wall_correction<L>(p, nb, m.rho[s], fl[s]);
         store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
     });
     if constexpr (MT::SCALAR) {
@@ -553,11 +577,11 @@ template <class R, int MODEL, int Q = 9> struct StepBounds {
                               : (MODEL == M_SC1 ? 6 : (sizeof(R) == 8 && Q == 19 ? 3 : 5));
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool VSHIFT = false>
+template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
 __global__ void __launch_bounds__(StepBounds<R, MODEL, L::Q>::THREADS, StepBounds<R, MODEL, L::Q>::MINB) k_step(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
-    step_cell<R, L, MODEL, PARITY, WALLS, FORCED, false, VSHIFT>(p, x, y, z);
+    step_cell<R, L, MODEL, PARITY, WALLS, FORCED, false, VSHIFT, MOVING>(p, x, y, z);
 }
 
 // ------------------------------------------------------------------------------------------

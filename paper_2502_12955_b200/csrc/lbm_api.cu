@@ -68,6 +68,11 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (model != LBM_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) return "rho0_psi must be > 0";
     if (p->w0_scalar < 0.0 || p->w0_scalar >= 1.0) return "w0_scalar must lie in [0, 1)";
     if (p->init_kind < LBM_INIT_REST || p->init_kind > LBM_INIT_RANDOM_DROPLETS) return "unknown init_kind";
+    for (int a = 0; a < 3; ++a)
+        for (int sd = 0; sd < 2; ++sd)
+            for (int b = 0; b < 3; ++b)
+                if (p->bc[a] == 1 && p->wall_u[a][sd][b] != 0.0 && (model != LBM_BGK || p->forcing != 0))
+                    return "moving walls (wall_u) are implemented for LBM_BGK with Guo forcing only";
     if (sh) {
         sh->S = S;
         sh->d = lattice == LBM_D3Q19 ? 3 : 2;
@@ -109,6 +114,7 @@ struct lbm_ctx {
     lbm::KP<double> kp64;
     lbm::KP<float> kp32;
     bool walls;
+    bool moving;          // some wall has a velocity (moving-wall bounce-back)
     int forced;           // 0 no force, 1 Guo forcing, 2 velocity-shift forcing (kernel variant)
     bool inited;
     int64_t t;
@@ -162,6 +168,9 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     k.inv_cs2g = (R)((double)c->sh.d / (1.0 - w0s));
     k.ws0 = (R)w0s;
     k.ws1 = (R)((1.0 - w0s) / (double)(c->sh.Qs - 1));
+    for (int a = 0; a < 3; ++a)
+        for (int sd = 0; sd < 2; ++sd)
+            for (int b = 0; b < 3; ++b) k.wall_u[a][sd][b] = (R)p.wall_u[a][sd][b];
     k.rho0_psi = (R)p.rho0_psi;
     k.k_react = (R)p.k_react;
 }
@@ -383,6 +392,11 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->h = sh.scalar ? c->ws + sh.f_bytes : nullptr;
     c->psi = sh.sc ? c->ws + sh.f_bytes + sh.h_bytes : nullptr;
     c->walls = p->bc[0] || p->bc[1] || p->bc[2];
+    c->moving = false;
+    for (int a = 0; a < 3; ++a)
+        for (int sd = 0; sd < 2; ++sd)
+            for (int b = 0; b < 3; ++b)
+                if (p->bc[a] == 1 && p->wall_u[a][sd][b] != 0.0) c->moving = true;
     c->forced = (sh.sc || p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
     if (p->forcing == 1) c->forced = 2;       // its own arithmetic even when the force is zero
     if (p->precision == 64) c->ops = lattice == LBM_D3Q19 ? lbm::ops_f64_d3q19() : lbm::ops_f64_d2q9();
@@ -441,7 +455,7 @@ constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far l
 // the kernels of one time step of the register path, enqueued on st (no event marks, no counters)
 int enqueue_register_step(lbm_ctx* c, int parity, cudaStream_t st) {
     if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, c->walls, st));
-    CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, st));
+    CK(c->ops->step(c->kp(), c->model, parity, c->moving ? 2 : (c->walls ? 1 : 0), c->forced, st));
     return 0;
 }
 
@@ -499,7 +513,7 @@ int lbm_step(lbm_ctx* c, int n) {
             if (rc) return rc;
         }
         if ((rc = mark(c, 0))) return rc;
-        CK(c->ops->step(c->kp(), c->model, parity, c->walls, c->forced, c->stream));
+        CK(c->ops->step(c->kp(), c->model, parity, c->moving ? 2 : (c->walls ? 1 : 0), c->forced, c->stream));
         c->launches++;
         if ((rc = mark(c, 0))) return rc;
         c->t++;
@@ -633,6 +647,7 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
     }
     if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
     if (c->sh.sc && c->walls) return fail(LBM_EINVAL, "Shan-Chen models between walls run on LBM_PATH_REGISTER only");
+    if (c->moving) return fail(LBM_EINVAL, "moving walls run on LBM_PATH_REGISTER only");
     if (path == LBM_PATH_WAVEFRONT) {
         if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
     } else if (path == LBM_PATH_PIPELINE) {
