@@ -132,6 +132,7 @@ struct ref_ctx {
     virtual int get_populations(void* f) = 0;
     virtual int set_populations(const void* f) = 0;
     virtual size_t population_count() = 0;
+    virtual int set_mask(const unsigned char* m) = 0;
 };
 
 namespace {
@@ -159,6 +160,8 @@ struct Sim : ref_ctx {
     std::vector<R> rho, jm, psi;   /* rho[sigma][cell], jm[sigma][a][cell], psi[sigma][cell] */
     std::vector<R> Fv, ub;         /* Fv[sigma][a][cell], ub[a][cell] */
     std::vector<R> ueq;            /* ueq[sigma][a][cell]: equilibrium velocity of the velocity-shift scheme, Eq. 16 */
+    std::vector<unsigned char> solid;  /* 1: solid node (bounce-back obstacle), 0: fluid */
+    bool has_mask = false;
 
     R& F_(std::vector<R>& v, int s, int i, size_t cell) { return v[((size_t)s * Q + i) * N + cell]; }
     R& H_(std::vector<R>& v, int i, size_t cell) { return v[(size_t)i * N + cell]; }
@@ -203,6 +206,7 @@ struct Sim : ref_ctx {
         Fv.assign((size_t)S * 3 * N, (R)0);
         ub.assign((size_t)3 * N, (R)0);
         ueq.assign((size_t)S * 3 * N, (R)0);
+        solid.assign(N, 0);
     }
 
     size_t cell_of(int x, int y, int z) const { return (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * z); }
@@ -218,7 +222,7 @@ struct Sim : ref_ctx {
             }
         }
         out = cell_of(q[0], q[1], q[2]);
-        return true;
+        return !solid[out];          /* a solid node reflects like a wall */
     }
 
     /* velocity of the wall a population leaving (x, y, z) along c hits: the first wall axis (x, y, z order) it crosses */
@@ -227,8 +231,9 @@ struct Sim : ref_ctx {
         const int n[3] = {nx, ny, nz};
         for (int a = 0; a < 3; ++a)
             if (p.bc[a] == 1 && (q[a] < 0 || q[a] >= n[a])) return wall_u[a][q[a] < 0 ? 0 : 1];
-        return wall_u[0][0];
+        return zero3;                /* reflected by a solid node of the mask: at rest */
     }
+    R zero3[3] = {(R)0, (R)0, (R)0};
 
     /* Eq. 10 / Eq. 24, or psi = rho (DESIGN R3) */
     R psi_of(R r) const {
@@ -251,7 +256,7 @@ struct Sim : ref_ctx {
         for (int s = 0; s < S; ++s)
             for (size_t cell = 0; cell < N; ++cell) {
                 R r = (R)0, j[3] = {(R)0, (R)0, (R)0};
-                for (int i = 0; i < Q; ++i) {
+                for (int i = 0; i < Q && !solid[cell]; ++i) {
                     R fi = F_(f, s, i, cell);
                     r = r + fi;
                     for (int a = 0; a < d; ++a) j[a] = j[a] + (R)L.c[i][a] * fi;
@@ -261,12 +266,19 @@ struct Sim : ref_ctx {
             }
         /* 2. pseudopotential of every cell at this time level (full-field barrier; DESIGN R9) */
         for (int s = 0; s < S; ++s)
-            for (size_t cell = 0; cell < N; ++cell) psi[(size_t)s * N + cell] = psi_of(rho[(size_t)s * N + cell]);
+            for (size_t cell = 0; cell < N; ++cell)
+                psi[(size_t)s * N + cell] = solid[cell] ? (R)0 : psi_of(rho[(size_t)s * N + cell]);
         /* 3. Shan-Chen force, Eq. 11 / 13, plus the body force */
         for (int z = 0; z < nz; ++z)
             for (int y = 0; y < ny; ++y)
                 for (int x = 0; x < nx; ++x) {
                     size_t cell = cell_of(x, y, z);
+                    if (solid[cell]) {          /* no fluid here: all fields read as zero */
+                        for (int s = 0; s < S; ++s)
+                            for (int a = 0; a < 3; ++a) Fv[((size_t)s * 3 + a) * N + cell] = ueq[((size_t)s * 3 + a) * N + cell] = (R)0;
+                        for (int a = 0; a < 3; ++a) ub[(size_t)a * N + cell] = (R)0;
+                        continue;
+                    }
                     R rho_t = rho[cell];
                     for (int s = 1; s < S; ++s) rho_t = rho_t + rho[(size_t)s * N + cell];
                     R inv_rho = (R)1 / rho_t;
@@ -281,7 +293,7 @@ struct Sim : ref_ctx {
                                 R wp = w[i] * psi[(size_t)t * N + nb];
                                 for (int a = 0; a < d; ++a) acc[t][a] = acc[t][a] + wp * (R)L.c[i][a];
                             }
-                        if (has_walls)
+                        if (has_walls || has_mask)
                             for (int i = 1; i < Q; ++i) {
                                 size_t nb;
                                 if (neighbour(x, y, z, L.c[i], nb)) continue;
@@ -296,7 +308,7 @@ struct Sim : ref_ctx {
                                 if (S == 2) t = t + G[s][1] * acc[1][a];
                                 Fa = -(psi[(size_t)s * N + cell] * t);
                                 /* fluid-solid adhesion, Eq. 14: -G_ads rho^s sum_i w_i s c_i */
-                                if (has_walls) Fa = Fa + (-((G_ads[s] * rho[(size_t)s * N + cell]) * adh[a]));
+                                if (has_walls || has_mask) Fa = Fa + (-((G_ads[s] * rho[(size_t)s * N + cell]) * adh[a]));
                             }
                             /* constant body-force density; split by mass fraction for S=2 (DESIGN R5) */
                             R Fext = (S == 1) ? force[a] : force[a] * (rho[(size_t)s * N + cell] * inv_rho);
@@ -339,6 +351,12 @@ struct Sim : ref_ctx {
             for (int y = 0; y < ny; ++y)
                 for (int x = 0; x < nx; ++x) {
                     size_t cell = cell_of(x, y, z);
+                    if (solid[cell]) {          /* solid nodes are not updated: their (unused) populations stay */
+                        for (int s = 0; s < S; ++s)
+                            for (int i = 0; i < Q; ++i) F_(fnew, s, i, cell) = F_(f, s, i, cell);
+                        if (has_scalar) for (int i = 0; i < Qs; ++i) H_(hnew, i, cell) = H_(h, i, cell);
+                        continue;
+                    }
                     R u[3] = {ub[cell], ub[N + cell], ub[2 * N + cell]};
                     /* 5. collide each component: Eq. 15 with Eq. 6 and Eq. 22 */
                     for (int s = 0; s < S; ++s) {
@@ -368,7 +386,7 @@ struct Sim : ref_ctx {
                                 /* moving wall: the reflected population exchanges momentum with the wall,
                                  * f_opp(i)(x, t+1) = f*_i(x, t) - 2 w_i rho (c_i . u_w) / c_s^2 ("Bounce Back
                                  * ... incorporating an additional term"; DESIGN R24), rho the cell's density at t */
-                                if (moving_walls) {
+                                if (moving_walls) {   /* (mask solids are at rest) */
                                     const R* uw = wall_velocity(x, y, z, L.c[i]);
                                     R cuw = (R)0;
                                     for (int a = 0; a < d; ++a) cuw = cuw + (R)L.c[i][a] * uw[a];
@@ -530,6 +548,7 @@ struct Sim : ref_ctx {
         if (phi_o) {
             R* ph = (R*)phi_o;
             for (size_t cell = 0; cell < N; ++cell) {
+                if (solid[cell]) { ph[cell] = (R)0; continue; }
                 if (S == 2) {
                     R rA = rho[cell], rB = rho[N + cell];
                     R inv_rho = (R)1 / (rA + rB);
@@ -543,7 +562,7 @@ struct Sim : ref_ctx {
             R* Cc = (R*)C_o;
             for (size_t cell = 0; cell < N; ++cell) {
                 R C = (R)0;
-                for (int i = 0; i < Qs; ++i) C = C + H_(h, i, cell);
+                for (int i = 0; i < Qs && !solid[cell]; ++i) C = C + H_(h, i, cell);
                 Cc[cell] = C;
             }
         }
@@ -557,6 +576,15 @@ struct Sim : ref_ctx {
         for (int s = 0; s < S; ++s)
             for (int a = 0; a < d; ++a)
                 std::memcpy(o + ((size_t)s * d + a) * N, &Fv[((size_t)s * 3 + a) * N], sizeof(R) * N);
+        return 0;
+    }
+
+    int set_mask(const unsigned char* m) override {
+        has_mask = false;
+        for (size_t cell = 0; cell < N; ++cell) {
+            solid[cell] = m ? (m[cell] != 0) : 0;
+            if (solid[cell]) has_mask = true;
+        }
         return 0;
     }
 
@@ -614,6 +642,7 @@ int ref_init_from_seed(ref_ctx* c, uint64_t seed) { return c ? c->init(seed) : -
 int ref_step(ref_ctx* c, int n) { return c ? c->step(n) : -1; }
 int ref_get_macros(ref_ctx* c, void* rho, void* u, void* phi, void* C) { return c ? c->get_macros(rho, u, phi, C) : -1; }
 int ref_get_force(ref_ctx* c, void* F) { return c ? c->get_force(F) : -1; }
+int ref_set_mask(ref_ctx* c, const unsigned char* mask) { return c ? c->set_mask(mask) : -1; }
 int ref_get_populations(ref_ctx* c, void* f) { return c ? c->get_populations(f) : -1; }
 int ref_set_populations(ref_ctx* c, const void* f) { return c ? c->set_populations(f) : -1; }
 size_t ref_population_count(ref_ctx* c) { return c ? c->population_count() : 0; }

@@ -61,6 +61,9 @@ int  ref_step(ref_ctx*, int n);
 int  ref_get_macros(ref_ctx*, void* rho, void* u, void* phi, void* C);
 /* total force density per component (Shan-Chen + body), F[sigma][a][cell], S*d*N */
 int  ref_get_force(ref_ctx*, void* F);
+/* solid-node mask, N bytes (non-zero = solid), NULL clears it: solid nodes reflect populations like a wall
+ * (halfway bounce-back), are left out of the psi stencil (Eq. 11-12) and act in Eq. 14 */
+int  ref_set_mask(ref_ctx*, const unsigned char* mask);
 /* canonical populations f[sigma][i][cell] (S*Q*N) then h[i][cell] (Qs*N, scalar models only) */
 int  ref_get_populations(ref_ctx*, void* f);
 int  ref_set_populations(ref_ctx*, const void* f);

@@ -50,6 +50,7 @@ def lib():
         L.ref_step.argtypes = [C.c_void_p, C.c_int]
         L.ref_get_macros.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.ref_get_force.argtypes = [C.c_void_p, C.c_void_p]
+        L.ref_set_mask.argtypes = [C.c_void_p, C.c_void_p]
         L.ref_get_populations.argtypes = [C.c_void_p, C.c_void_p]
         L.ref_set_populations.argtypes = [C.c_void_p, C.c_void_p]
         L.ref_population_count.restype = C.c_size_t
@@ -146,6 +147,15 @@ class RefLBM:
         F = np.empty((self.S, self.d, self.N), self.dtype)
         self._chk(self.L.ref_get_force(self.h, F.ctypes.data))
         return F
+
+    def set_mask(self, mask):
+        """solid-node mask: N values, non-zero = solid; None clears it"""
+        if mask is None:
+            self._chk(self.L.ref_set_mask(self.h, None))
+        else:
+            m = np.ascontiguousarray(mask, dtype=np.uint8).ravel()
+            assert m.size == self.N
+            self._chk(self.L.ref_set_mask(self.h, m.ctypes.data))
 
     def population_count(self):
         return int(self.L.ref_population_count(self.h))
