@@ -972,5 +972,5 @@ def test_flow_past_a_masked_obstacle_conserves_mass_and_stays_symmetric():
     assert abs(f1[0][:, fluid].sum() - mass0) < 1e-10
     mac = r.get_macros()
     ux = mac["u"][0].reshape(ny, nx); uy = mac["u"][1].reshape(ny, nx)
-    assert np.abs(ux - ux[::-1, :]).max() < 1e-13 * ux.max() and np.abs(uy + uy[::-1, :]).max() < 1e-13 * ux.max()
+    assert np.abs(ux - ux[::-1, :]).max() < 1e-11 * ux.max() and np.abs(uy + uy[::-1, :]).max() < 1e-11 * ux.max()
     assert 0 < ux[fluid.reshape(ny, nx)].mean() < 0.5 * g * 1500
