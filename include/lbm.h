@@ -120,6 +120,14 @@ int lbm_get_macros(lbm_ctx* ctx, void* rho, void* u, void* phi, void* C);
 /* Total force density per component (Shan-Chen + body), F[sigma][a][cell] (S*d*N), device buffer. */
 int lbm_get_force(lbm_ctx* ctx, void* F);
 
+/* Solid-node mask: N bytes in DEVICE memory (non-zero = solid node), owned by the caller and valid until it is
+ * replaced, cleared (NULL) or the context is destroyed.  Solid nodes reflect populations like a wall (halfway
+ * bounce-back on arbitrary nodes), are not updated, are left out of the psi stencil (Eq. 11-12,
+ * PAPER.md:128-132) and act on the fluid through the adhesion force (G_ads, Eq. 14); all output fields read zero
+ * there.  LBM_PATH_REGISTER only; the mask may change at even time levels only (LBM_ESTATE otherwise: at odd
+ * levels the in-place layout depends on which neighbours reflect).  Synchronises the stream. */
+int lbm_set_mask(lbm_ctx* ctx, const unsigned char* mask);
+
 /* Canonical populations at the current time level, independent of the in-place slot permutation:
  * f[sigma][i][cell] (S*Q*N) followed by h[i][cell] (Qs*N, scalar models only).  Device buffers.
  * lbm_set_populations also marks the context initialised and resets the time level parity. */

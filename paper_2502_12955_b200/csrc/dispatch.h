@@ -12,7 +12,7 @@ struct PipeArgs;
 struct Ops {
     // kp points at a KP<R> of the matching precision
     cudaError_t (*psi)(const void* kp, int model, int parity, int walls, cudaStream_t st);
-    cudaError_t (*step)(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st);
+    cudaError_t (*step)(const void* kp, int model, int parity, int wmode, int forced, int moving, cudaStream_t st);
     cudaError_t (*macros)(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
                           void* F, cudaStream_t st);
     // canonical <-> slot permutation of the flow lattices (S of them) and of the scalar lattice

@@ -24,98 +24,113 @@ inline dim3 grid_for(const KP<R>& p) { const int b = block_for(p); return dim3((
 
 template <class R, class L>
 struct Launch {
-    template <int MODEL, int PARITY>
-    static void psi2(const KP<R>& p, int walls, cudaStream_t st) {
-        if (walls) k_psi<R, L, MODEL, PARITY, true><<<grid_for(p), block_for(p), 0, st>>>(p);
-        else k_psi<R, L, MODEL, PARITY, false><<<grid_for(p), block_for(p), 0, st>>>(p);
+    // run f(std::integral_constant<int, v>) for the run-time v in {0, ..., N-1}
+    template <int N, class F>
+    static bool with_int(int v, F&& f) {
+        bool hit = false;
+        static_for<0, N>([&](auto c) { if (decltype(c)::value == v) { f(c); hit = true; } });
+        return hit;
     }
-    static cudaError_t psi(const void* kp, int model, int parity, int walls, cudaStream_t st) {
-        const KP<R>& p = *(const KP<R>*)kp;
-#define LBM_PSI(M) case M: parity ? psi2<M, 1>(p, walls, st) : psi2<M, 0>(p, walls, st); break;
-        switch (model) { LBM_PSI(M_SC1) LBM_PSI(M_SC2) LBM_PSI(M_SC2_ADE) default: return cudaErrorInvalidValue; }
-#undef LBM_PSI
-        return cudaGetLastError();
+    template <class F>
+    static bool with_sc_model(int model, F&& f) {
+        switch (model) {
+        case M_SC1: f(std::integral_constant<int, M_SC1>{}); return true;
+        case M_SC2: f(std::integral_constant<int, M_SC2>{}); return true;
+        case M_SC2_ADE: f(std::integral_constant<int, M_SC2_ADE>{}); return true;
+        default: return false;
+        }
     }
 
-    template <int MODEL, bool WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
+    // wmode: 0 fully periodic, 1 bounce-back walls (bc), 2 walls and / or a solid-node mask
+    static cudaError_t psi(const void* kp, int model, int parity, int wmode, cudaStream_t st) {
+        const KP<R>& p = *(const KP<R>*)kp;
+        const bool ok = with_sc_model(model, [&](auto M) {
+            with_int<3>(wmode, [&](auto W) {
+                with_int<2>(parity, [&](auto P) {
+                    k_psi<R, L, decltype(M)::value, decltype(P)::value, decltype(W)::value><<<grid_for(p), block_for(p), 0, st>>>(p);
+                });
+            });
+        });
+        return ok ? cudaGetLastError() : cudaErrorInvalidValue;
+    }
+
+    template <int MODEL, int WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
     static void step3(const KP<R>& p, int parity, cudaStream_t st) {
         if (parity) k_step<R, L, MODEL, 1, WALLS, FORCED, VSHIFT, MOVING><<<grid_for(p), block_for(p), 0, st>>>(p);
         else k_step<R, L, MODEL, 0, WALLS, FORCED, VSHIFT, MOVING><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
     // forced: 0 no force, 1 Guo forcing (Eq. 20-23), 2 Shan-Chen velocity-shift forcing (Eq. 16-19);
-    // walls: 0 none, 1 bounce-back walls at rest, 2 moving walls (LBM_BGK without velocity shift only)
-    static cudaError_t step(const void* kp, int model, int parity, int walls, int forced, cudaStream_t st) {
+    // moving: some wall has a velocity (LBM_BGK with Guo forcing only)
+    static cudaError_t step(const void* kp, int model, int parity, int wmode, int forced, int moving, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
-        if (walls == 2) {
-            if (model != M_BGK || forced == 2) return cudaErrorInvalidValue;
-            if (forced) step3<M_BGK, true, true, false, true>(p, parity, st);
-            else step3<M_BGK, true, false, false, true>(p, parity, st);
-            return cudaGetLastError();
+        bool ok = false;
+        if (moving) {
+            if (model != M_BGK || forced == 2 || wmode == 0) return cudaErrorInvalidValue;
+            ok = with_int<3>(wmode, [&](auto W) {
+                constexpr int w = decltype(W)::value;
+                if constexpr (w != 0) {
+                    if (forced) step3<M_BGK, w, true, false, true>(p, parity, st);
+                    else step3<M_BGK, w, false, false, true>(p, parity, st);
+                }
+            });
+        } else if (model == M_BGK) {
+            ok = with_int<3>(wmode, [&](auto W) {
+                constexpr int w = decltype(W)::value;
+                if (forced == 2) step3<M_BGK, w, true, true>(p, parity, st);
+                else if (forced) step3<M_BGK, w, true>(p, parity, st);
+                else step3<M_BGK, w, false>(p, parity, st);
+            });
+        } else {
+            ok = with_sc_model(model, [&](auto M) {
+                with_int<3>(wmode, [&](auto W) {
+                    if (forced == 2) step3<decltype(M)::value, decltype(W)::value, true, true>(p, parity, st);
+                    else step3<decltype(M)::value, decltype(W)::value, true>(p, parity, st);
+                });
+            });
         }
-        if (forced == 2) {
-            switch (model) {
-            case M_BGK: if (walls) step3<M_BGK, true, true, true>(p, parity, st); else step3<M_BGK, false, true, true>(p, parity, st); break;
-            case M_SC1: if (walls) step3<M_SC1, true, true, true>(p, parity, st); else step3<M_SC1, false, true, true>(p, parity, st); break;
-            case M_SC2: if (walls) step3<M_SC2, true, true, true>(p, parity, st); else step3<M_SC2, false, true, true>(p, parity, st); break;
-            case M_SC2_ADE: if (walls) step3<M_SC2_ADE, true, true, true>(p, parity, st); else step3<M_SC2_ADE, false, true, true>(p, parity, st); break;
-            default: return cudaErrorInvalidValue;
-            }
-            return cudaGetLastError();
-        }
-        switch (model) {
-        case M_BGK:
-            if (walls) { if (forced) step3<M_BGK, true, true>(p, parity, st); else step3<M_BGK, true, false>(p, parity, st); }
-            else { if (forced) step3<M_BGK, false, true>(p, parity, st); else step3<M_BGK, false, false>(p, parity, st); }
-            break;
-        case M_SC1: if (walls) step3<M_SC1, true, true>(p, parity, st); else step3<M_SC1, false, true>(p, parity, st); break;
-        case M_SC2: if (walls) step3<M_SC2, true, true>(p, parity, st); else step3<M_SC2, false, true>(p, parity, st); break;
-        case M_SC2_ADE: if (walls) step3<M_SC2_ADE, true, true>(p, parity, st); else step3<M_SC2_ADE, false, true>(p, parity, st); break;
-        default: return cudaErrorInvalidValue;
-        }
-        return cudaGetLastError();
+        return ok ? cudaGetLastError() : cudaErrorInvalidValue;
     }
 
-    template <int MODEL, bool WALLS>
-    static void macros2(const KP<R>& p, int parity, R* rho, R* u, R* phi, R* C, R* F, cudaStream_t st) {
-        if (parity) k_macros<R, L, MODEL, 1, WALLS><<<grid_for(p), block_for(p), 0, st>>>(p, rho, u, phi, C, F);
-        else k_macros<R, L, MODEL, 0, WALLS><<<grid_for(p), block_for(p), 0, st>>>(p, rho, u, phi, C, F);
+    template <int MODEL>
+    static void macros2(const KP<R>& p, int parity, int wmode, R* rho, R* u, R* phi, R* C, R* F, cudaStream_t st) {
+        with_int<3>(wmode, [&](auto W) {
+            with_int<2>(parity, [&](auto P) {
+                k_macros<R, L, MODEL, decltype(P)::value, decltype(W)::value><<<grid_for(p), block_for(p), 0, st>>>(p, rho, u, phi, C, F);
+            });
+        });
     }
-    static cudaError_t macros(const void* kp, int model, int parity, int walls, void* rho, void* u, void* phi, void* C,
+    static cudaError_t macros(const void* kp, int model, int parity, int wmode, void* rho, void* u, void* phi, void* C,
                               void* F, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
         R *r = (R*)rho, *uu = (R*)u, *ph = (R*)phi, *c = (R*)C, *f = (R*)F;
-        switch (model) {
-        case M_BGK: if (walls) macros2<M_BGK, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_BGK, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC1: if (walls) macros2<M_SC1, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC1, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC2: if (walls) macros2<M_SC2, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC2, false>(p, parity, r, uu, ph, c, f, st); break;
-        case M_SC2_ADE: if (walls) macros2<M_SC2_ADE, true>(p, parity, r, uu, ph, c, f, st); else macros2<M_SC2_ADE, false>(p, parity, r, uu, ph, c, f, st); break;
-        default: return cudaErrorInvalidValue;
-        }
+        if (wmode < 0 || wmode > 2) return cudaErrorInvalidValue;
+        if (model == M_BGK) macros2<M_BGK>(p, parity, wmode, r, uu, ph, c, f, st);
+        else if (!with_sc_model(model, [&](auto M) { macros2<decltype(M)::value>(p, parity, wmode, r, uu, ph, c, f, st); }))
+            return cudaErrorInvalidValue;
         return cudaGetLastError();
     }
 
     template <class LL, bool TOC>
-    static void permute2(const KP<R>& p, int parity, int walls, R* slots, R* canon, int nl, cudaStream_t st) {
+    static void permute2(const KP<R>& p, int parity, int wmode, R* slots, R* canon, int nl, cudaStream_t st) {
         const dim3 g = grid_for(p);
         if (parity) {
-            if (walls) k_permute<R, LL, 1, true, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
-            else k_permute<R, LL, 1, false, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
+            with_int<3>(wmode, [&](auto W) { k_permute<R, LL, 1, decltype(W)::value, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl); });
         } else {
-            k_permute<R, LL, 0, false, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
+            k_permute<R, LL, 0, 0, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
         }
     }
-    static cudaError_t permute(const void* kp, int model, int parity, int walls, void* canon, int to_canonical,
+    static cudaError_t permute(const void* kp, int model, int parity, int wmode, void* canon, int to_canonical,
                                cudaStream_t st) {
         using LS = typename ScalarOf<L>::type;
         const KP<R>& p = *(const KP<R>*)kp;
         const int S = (model == M_SC2 || model == M_SC2_ADE) ? 2 : 1;
         R* cf = (R*)canon;
-        if (to_canonical) permute2<L, true>(p, parity, walls, p.f, cf, S, st);
-        else permute2<L, false>(p, parity, walls, p.f, cf, S, st);
+        if (to_canonical) permute2<L, true>(p, parity, wmode, p.f, cf, S, st);
+        else permute2<L, false>(p, parity, wmode, p.f, cf, S, st);
         if (model == M_SC2_ADE) {
             R* ch = cf + (size_t)S * L::Q * (size_t)p.N;
-            if (to_canonical) permute2<LS, true>(p, parity, walls, p.h, ch, 1, st);
-            else permute2<LS, false>(p, parity, walls, p.h, ch, 1, st);
+            if (to_canonical) permute2<LS, true>(p, parity, wmode, p.h, ch, 1, st);
+            else permute2<LS, false>(p, parity, wmode, p.h, ch, 1, st);
         }
         return cudaGetLastError();
     }

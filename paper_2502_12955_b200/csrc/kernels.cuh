@@ -44,6 +44,7 @@ struct KP {
     R G[2][2];
     R G_ads[2];               // fluid-solid adhesion, Eq. 14
     R wall_u[3][2][3];        // velocity of the wall at the low / high face of each axis (moving-wall bounce-back)
+    const unsigned char* mask;  // solid-node mask (N bytes, non-zero = solid) or nullptr; read by the WALLS == 2 variants
     R rho0_psi;
     R force[3];
     R k_react;
@@ -69,13 +70,16 @@ template <int MODEL> struct ModelTraits {
 // in uniform registers; only x-1 / x / x+1 are per-thread.  An address is then
 // (uniform slot base + uniform row base) + per-thread x: no integer division, one add per access.
 // ------------------------------------------------------------------------------------------
-template <int D, bool WALLS>
+// WALLS: 0 fully periodic; 1 bounce-back walls on the axes with bc = 1; 2 the same plus a solid-node mask
+template <int D, int WALLS>
 struct Nbr {
-    static constexpr bool HAS_WALLS = WALLS;
+    static constexpr bool HAS_WALLS = WALLS != 0;
     int cell;              // x + nx*(y + ny*z)
     int xx[3];             // x-1, x, x+1 with periodic wrap (per thread)
     int ry[3], rz[3];      // nx*y', nx*ny*z' for y' = y-1,y,y+1 / z' = z-1,z,z+1 with wrap (uniform)
     bool lo[3], hi[3];
+    unsigned blocked;      // bit (cx+1) + 3 (cy+1) + 9 (cz+1): the neighbour at that offset is a solid node of the mask
+    bool solid;            // this cell is a solid node itself
 
     template <class R>
     __device__ __forceinline__ Nbr(const KP<R>& p, int x, int y, int z) {
@@ -89,10 +93,24 @@ struct Nbr {
             rz[0] = rz[1] = rz[2] = 0;
         }
         cell = rz[1] + ry[1] + x;
+        blocked = 0u;
+        solid = false;
         if constexpr (WALLS) {
             lo[0] = p.bc[0] && x == 0; hi[0] = p.bc[0] && x == nx - 1;
             lo[1] = p.bc[1] && y == 0; hi[1] = p.bc[1] && y == ny - 1;
             lo[2] = D == 3 && p.bc[2] && z == 0; hi[2] = D == 3 && p.bc[2] && z == p.nz - 1;
+            if constexpr (WALLS == 2) {
+                // solid nodes of the mask reflect like a wall: one byte per lattice neighbour (L1 / L2 hits)
+                solid = p.mask[cell] != 0;
+                static_for<0, 27>([&](auto oc) {
+                    constexpr int o = decltype(oc)::value;
+                    constexpr int cx = o % 3 - 1, cy = (o / 3) % 3 - 1, cz = o / 9 - 1;
+                    constexpr int n2 = cx * cx + cy * cy + cz * cz;
+                    if constexpr ((D == 3 || cz == 0) && n2 >= 1 && n2 <= 2) {
+                        if (p.mask[(rz[cz + 1] + ry[cy + 1]) + xx[cx + 1]]) blocked |= 1u << o;
+                    }
+                });
+            }
         } else {
             lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
         }
@@ -104,11 +122,12 @@ struct Nbr {
     __device__ __forceinline__ int col() const { return xx[CX + 1]; }
     template <int CX, int CY, int CZ>
     __device__ __forceinline__ int at() const { return row<CY, CZ>() + col<CX>(); }
-    // does the offset cross a bounce-back wall?
+    // does the offset cross a bounce-back wall or end in a solid node?
     template <int CX, int CY, int CZ>
     __device__ __forceinline__ bool outside() const {
         if constexpr (!WALLS) return false;
         bool o = false;
+        if constexpr (WALLS == 2) o = ((blocked >> ((CX + 1) + 3 * (CY + 1) + 9 * (CZ + 1))) & 1u) != 0u;
         if constexpr (CX < 0) o = o || lo[0];
         if constexpr (CX > 0) o = o || hi[0];
         if constexpr (CY < 0) o = o || lo[1];
@@ -128,7 +147,7 @@ __device__ __forceinline__ bool thread_cell(int nx, int& x, int& y, int& z) {
 // address of P_I(x): where f_I(x,t) is read and f*_{opp(I)}(x,t) is written.  The element index within one
 // lattice (Q * N < 2^32, checked by lbm_create) is formed in 32 bits -- a uniform (slot, row) part plus the
 // per-thread column -- so that an access costs one integer add and one IMAD.WIDE.
-template <class L, int PARITY, bool WALLS, int I, class R, class NB>
+template <class L, int PARITY, int WALLS, int I, class R, class NB>
 __device__ __forceinline__ R* slot_of(R* base, const NB& nb, size_t N) {
     const unsigned n = (unsigned)N;
     if constexpr (PARITY == 0 || I == 0) {
@@ -193,7 +212,7 @@ __device__ __forceinline__ R psi_of(R rho, int kind, R rho0) {
     return rho0 * ((R)1 - exp(-(rho / rho0)));
 }
 
-template <class L, int PARITY, bool WALLS, class R, class NB>
+template <class L, int PARITY, int WALLS, class R, class NB>
 __device__ __forceinline__ void load_pops(R* __restrict__ base, const NB& nb, size_t N, R* fl) {
     static_for<0, L::Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
@@ -201,7 +220,7 @@ __device__ __forceinline__ void load_pops(R* __restrict__ base, const NB& nb, si
     });
 }
 // writes fl[opp(i)] (post-collision) to P_i
-template <class L, int PARITY, bool WALLS, class R, class NB>
+template <class L, int PARITY, int WALLS, class R, class NB>
 __device__ __forceinline__ void store_pops(R* __restrict__ base, const NB& nb, size_t N, const R* fl) {
     static_for<0, L::Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
@@ -418,12 +437,13 @@ __device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB
 // psi pass (step a2): rho^sigma from the populations at the current parity, psi^sigma to HBM
 // ------------------------------------------------------------------------------------------
 // psi^sigma of the cell (x,y,z) at the current parity
-template <class R, class L, int MODEL, int PARITY, bool WALLS = false>
+template <class R, class L, int MODEL, int PARITY, int WALLS = false>
 __device__ __forceinline__ void psi_cell(const KP<R>& p, int x, int y, int z) {
     constexpr int S = ModelTraits<MODEL>::S, Q = L::Q;
     const size_t N = (size_t)p.N;
     const Nbr<L::D, WALLS> nb(p, x, y, z);
     const int cell = nb.cell;
+    if (WALLS == 2 && nb.solid) return;
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         R fl[Q];
@@ -434,7 +454,7 @@ __device__ __forceinline__ void psi_cell(const KP<R>& p, int x, int y, int z) {
     });
 }
 
-template <class R, class L, int MODEL, int PARITY, bool WALLS = false>
+template <class R, class L, int MODEL, int PARITY, int WALLS = false>
 __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
@@ -445,7 +465,7 @@ __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) 
 // fused step (a1, a3-a8): one thread per cell
 // ------------------------------------------------------------------------------------------
 // first half: the populations of the cell into registers
-template <class R, class L, int MODEL, int PARITY, bool WALLS, class NB>
+template <class R, class L, int MODEL, int PARITY, int WALLS, class NB>
 __device__ __forceinline__ void step_load(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
@@ -458,7 +478,7 @@ __device__ __forceinline__ void step_load(const KP<R>& p, const NB& nb, R (*fl)[
     if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
 }
 // second half: moments, force (psi stencil), collision, stores
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH, class NB>
+template <class R, class L, int MODEL, int PARITY, int WALLS, bool FORCED, bool COH, class NB>
 __device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
@@ -492,7 +512,8 @@ __device__ __forceinline__ void moving_wall_correction(const KP<R>& p, const NB&
         constexpr int k = decltype(kc)::value;
         constexpr int CX = L::c(k, 0), CY = L::c(k, 1), CZ = L::c(k, 2);
         if (nb.template outside<CX, CY, CZ>()) {
-            const R* uw = p.wall_u[0][0];
+            const R zero[3] = {(R)0, (R)0, (R)0};   // a solid node of the mask is at rest
+            const R* uw = zero;
             bool found = false;
             if constexpr (CX != 0) { if (CX < 0 ? nb.lo[0] : nb.hi[0]) { uw = p.wall_u[0][CX < 0 ? 0 : 1]; found = true; } }
             if constexpr (CY != 0) { if (!found && (CY < 0 ? nb.lo[1] : nb.hi[1])) { uw = p.wall_u[1][CY < 0 ? 0 : 1]; found = true; } }
@@ -506,13 +527,14 @@ __device__ __forceinline__ void moving_wall_correction(const KP<R>& p, const NB&
 
 // both halves for one cell (k_step).  Written out rather than calling step_load / step_finish: ptxas keeps the
 // load addresses alive across the call boundary of the split form (fp32 BGK: 40 -> 80 registers).
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool COH = false, bool VSHIFT = false, bool MOVING = false>
+template <class R, class L, int MODEL, int PARITY, int WALLS, bool FORCED, bool COH = false, bool VSHIFT = false, bool MOVING = false>
 __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q;
     const size_t N = (size_t)p.N;
     const Nbr<L::D, WALLS> nb(p, x, y, z);
+    if (WALLS == 2 && nb.solid) return;              // solid nodes are not updated
 
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
@@ -577,7 +599,7 @@ template <class R, int MODEL, int Q = 9> struct StepBounds {
                               : (MODEL == M_SC1 ? 6 : (sizeof(R) == 8 && Q == 19 ? 3 : 5));
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
+template <class R, class L, int MODEL, int PARITY, int WALLS, bool FORCED, bool VSHIFT = false, bool MOVING = false>
 __global__ void __launch_bounds__(StepBounds<R, MODEL, L::Q>::THREADS, StepBounds<R, MODEL, L::Q>::MINB) k_step(const __grid_constant__ KP<R> p) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
@@ -587,7 +609,7 @@ __global__ void __launch_bounds__(StepBounds<R, MODEL, L::Q>::THREADS, StepBound
 // ------------------------------------------------------------------------------------------
 // macros out (step a9) and force diagnostic; psi must be current
 // ------------------------------------------------------------------------------------------
-template <class R, class L, int MODEL, int PARITY, bool WALLS>
+template <class R, class L, int MODEL, int PARITY, int WALLS>
 __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> p, R* __restrict__ rho_o,
                                                   R* __restrict__ u_o, R* __restrict__ phi_o, R* __restrict__ C_o,
                                                   R* __restrict__ F_o) {
@@ -599,6 +621,14 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
     const size_t N = (size_t)p.N;
     const Nbr<D, WALLS> nb(p, x, y, z);
     const int cell = nb.cell;
+    if (WALLS == 2 && nb.solid) {        // no fluid here: every field reads as zero
+        if (rho_o) static_for<0, S>([&](auto sc) { rho_o[(size_t)decltype(sc)::value * N + cell] = (R)0; });
+        if (u_o) static_for<0, D>([&](auto ac) { u_o[(size_t)decltype(ac)::value * N + cell] = (R)0; });
+        if (phi_o) phi_o[cell] = (R)0;
+        if (C_o) C_o[cell] = (R)0;
+        if (F_o) static_for<0, S * D>([&](auto kc) { F_o[(size_t)decltype(kc)::value * N + cell] = (R)0; });
+        return;
+    }
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
@@ -633,7 +663,7 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
 }
 
 // canonical populations f_i(x,t) out of the slot array at the current parity (and back)
-template <class R, class L, int PARITY, bool WALLS, bool TO_CANONICAL>
+template <class R, class L, int PARITY, int WALLS, bool TO_CANONICAL>
 __global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R> p, R* __restrict__ slots,
                                                    R* __restrict__ canon, int n_lattices) {
     int x, y, z;
@@ -647,6 +677,7 @@ __global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R>
         static_for<0, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             R* P = slot_of<L, PARITY, WALLS, i>(sb, nb, N);
+            if (WALLS == 2 && nb.solid) P = sb + ((size_t)i * N + cell);      // a solid node keeps its values in its own slots
             if constexpr (TO_CANONICAL) cb[(size_t)i * N + cell] = *P;
             else *P = cb[(size_t)i * N + cell];
         });

@@ -115,6 +115,7 @@ struct lbm_ctx {
     lbm::KP<float> kp32;
     bool walls;
     bool moving;          // some wall has a velocity (moving-wall bounce-back)
+    bool bc_walls;        // walls from lbm_params.bc (walls = bc_walls || a mask is set)
     int forced;           // 0 no force, 1 Guo forcing, 2 velocity-shift forcing (kernel variant)
     bool inited;
     int64_t t;
@@ -144,6 +145,8 @@ struct lbm_ctx {
     int wave_epoch;
 
     const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
+    // kernel variant: 0 fully periodic, 1 bounce-back walls (bc), 2 with a solid-node mask
+    int wmode() const { return kp64.mask ? 2 : (bc_walls ? 1 : 0); }
 };
 
 namespace {
@@ -171,6 +174,7 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
             for (int b = 0; b < 3; ++b) k.wall_u[a][sd][b] = (R)p.wall_u[a][sd][b];
+    k.mask = nullptr;
     k.rho0_psi = (R)p.rho0_psi;
     k.k_react = (R)p.k_react;
 }
@@ -225,7 +229,7 @@ void drop_events(lbm_ctx* c) {
 int run_psi(lbm_ctx* c) {
     int rc = mark(c, 1);
     if (rc) return rc;
-    CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->walls, c->stream));
+    CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->wmode(), c->stream));
     c->launches++;
     return mark(c, 1);
 }
@@ -391,7 +395,8 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->f = c->ws;
     c->h = sh.scalar ? c->ws + sh.f_bytes : nullptr;
     c->psi = sh.sc ? c->ws + sh.f_bytes + sh.h_bytes : nullptr;
-    c->walls = p->bc[0] || p->bc[1] || p->bc[2];
+    c->bc_walls = p->bc[0] || p->bc[1] || p->bc[2];
+    c->walls = c->bc_walls;
     c->moving = false;
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
@@ -454,8 +459,8 @@ constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far l
 
 // the kernels of one time step of the register path, enqueued on st (no event marks, no counters)
 int enqueue_register_step(lbm_ctx* c, int parity, cudaStream_t st) {
-    if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, c->walls, st));
-    CK(c->ops->step(c->kp(), c->model, parity, c->moving ? 2 : (c->walls ? 1 : 0), c->forced, st));
+    if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, c->wmode(), st));
+    CK(c->ops->step(c->kp(), c->model, parity, c->wmode(), c->forced, c->moving ? 1 : 0, st));
     return 0;
 }
 
@@ -513,7 +518,7 @@ int lbm_step(lbm_ctx* c, int n) {
             if (rc) return rc;
         }
         if ((rc = mark(c, 0))) return rc;
-        CK(c->ops->step(c->kp(), c->model, parity, c->moving ? 2 : (c->walls ? 1 : 0), c->forced, c->stream));
+        CK(c->ops->step(c->kp(), c->model, parity, c->wmode(), c->forced, c->moving ? 1 : 0, c->stream));
         c->launches++;
         if ((rc = mark(c, 0))) return rc;
         c->t++;
@@ -527,7 +532,7 @@ int lbm_get_macros(lbm_ctx* c, void* rho, void* u, void* phi, void* C) {
     if (C && !c->sh.scalar) return fail(LBM_EINVAL, "model has no scalar lattice");
     DeviceGuard g(c->device);
     if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
-    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->walls, rho, u, phi, C, nullptr, c->stream));
+    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->wmode(), rho, u, phi, C, nullptr, c->stream));
     c->launches++;
     return 0;
 }
@@ -538,7 +543,7 @@ int lbm_get_force(lbm_ctx* c, void* F) {
     if (!F) return fail(LBM_EINVAL, "F is NULL");
     DeviceGuard g(c->device);
     if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
-    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->walls, nullptr, nullptr, nullptr, nullptr, F, c->stream));
+    CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->wmode(), nullptr, nullptr, nullptr, nullptr, F, c->stream));
     c->launches++;
     return 0;
 }
@@ -557,7 +562,7 @@ int lbm_get_populations(lbm_ctx* c, void* f) {
         CK(cudaMemcpyAsync(f, c->f, nf, cudaMemcpyDeviceToDevice, c->stream));
         if (c->sh.scalar) CK(cudaMemcpyAsync((char*)f + nf, c->h, nh, cudaMemcpyDeviceToDevice, c->stream));
     } else {
-        CK(c->ops->permute(c->kp(), c->model, 1, c->walls, f, 1, c->stream));
+        CK(c->ops->permute(c->kp(), c->model, 1, c->wmode(), f, 1, c->stream));
         c->launches += c->sh.scalar ? 2 : 1;
     }
     return 0;
@@ -648,6 +653,7 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
     if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
     if (c->sh.sc && c->walls) return fail(LBM_EINVAL, "Shan-Chen models between walls run on LBM_PATH_REGISTER only");
     if (c->moving) return fail(LBM_EINVAL, "moving walls run on LBM_PATH_REGISTER only");
+    if (c->kp64.mask) return fail(LBM_EINVAL, "a solid-node mask runs on LBM_PATH_REGISTER only");
     if (path == LBM_PATH_WAVEFRONT) {
         if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
     } else if (path == LBM_PATH_PIPELINE) {
@@ -660,6 +666,21 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
 }
 
 int lbm_get_path(const lbm_ctx* c) { return c ? c->path : LBM_EINVAL; }
+
+int lbm_set_mask(lbm_ctx* c, const unsigned char* mask) {
+    if (!c) return fail(LBM_EINVAL, "ctx is NULL");
+    if (mask && c->path != LBM_PATH_REGISTER) return fail(LBM_EINVAL, "a solid-node mask runs on LBM_PATH_REGISTER only");
+    // at an odd time level the in-place layout depends on which neighbours reflect: the mask may only change
+    // when the populations sit in their own cells
+    if (c->inited && (c->t & 1)) return fail(LBM_ESTATE, "lbm_set_mask needs an even time level (lbm_time)");
+    DeviceGuard g(c->device);
+    CK(cudaStreamSynchronize(c->stream));
+    c->kp64.mask = mask;
+    c->kp32.mask = mask;
+    c->walls = c->bc_walls || mask != nullptr;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // the graph holds the old parameters
+    return 0;
+}
 
 int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity, size_t* count) {
     if (!count) return fail(LBM_EINVAL, "count is NULL");

@@ -22,7 +22,7 @@ PATHS = {"register": 0, "pipeline": 1, "wavefront": 2}
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -78,6 +78,7 @@ def lib():
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
     L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
     L.lbm_get_path.argtypes = [C.c_void_p]
+    L.lbm_set_mask.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_wavefront_schedule.argtypes = [C.c_int] * 4 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
     L.lbm_check.argtypes = [C.c_void_p]
     L.lbm_time.restype = C.c_int64
@@ -279,6 +280,17 @@ class LBM:
         """which kernels step() launches: "register", "pipeline" or "wavefront" (Shan-Chen only) (include/lbm.h)"""
         path = PATHS[path] if isinstance(path, str) else int(path)
         self._chk(self.L.lbm_set_path(self.h, path, int(rows_per_pencil), int(lead_rows)))
+
+    def set_mask(self, mask):
+        """solid-node mask (N values, non-zero = solid; any array-like or tensor) or None; kept alive here"""
+        if mask is None:
+            self._chk(self.L.lbm_set_mask(self.h, None))
+            self._mask = None
+            return
+        m = self.torch.as_tensor(mask).to(device=self.device, dtype=self.torch.uint8).contiguous().reshape(-1)
+        assert m.numel() == self.N
+        self._chk(self.L.lbm_set_mask(self.h, m.data_ptr()))
+        self._mask = m
 
     def get_path(self):
         return {v: k for k, v in PATHS.items()}[self.L.lbm_get_path(self.h)]
