@@ -142,7 +142,7 @@ struct Sim : ref_ctx {
     ref_params p;
     Lattice L, Ls;
     int S, d, Q, Qs;
-    bool has_sc, has_scalar;
+    bool has_sc, has_scalar, has_thermal;
     size_t N;
     bool inited = false;
 
@@ -157,6 +157,7 @@ struct Sim : ref_ctx {
     /* fields */
     std::vector<R> f, fnew;        /* [sigma][i][cell] */
     std::vector<R> h, hnew;        /* [i][cell] */
+    std::vector<R> g, gnew;        /* internal-energy lattice [i][cell] (REF_BGK_T), Q directions of the flow lattice */
     std::vector<R> rho, jm, psi;   /* rho[sigma][cell], jm[sigma][a][cell], psi[sigma][cell] */
     std::vector<R> Fv, ub;         /* Fv[sigma][a][cell], ub[a][cell] */
     std::vector<R> ueq;            /* ueq[sigma][a][cell]: equilibrium velocity of the velocity-shift scheme, Eq. 16 */
@@ -182,6 +183,7 @@ struct Sim : ref_ctx {
                     if (pp.bc[a] == 1 && pp.wall_u[a][sd][b] != 0.0) moving_walls = true;
                 }
         has_scalar = (model == REF_SC2_ADE);
+        has_thermal = (model == REF_BGK_T);
         d = L.d; Q = L.Q; Qs = Ls.Q;
         N = (size_t)nx * ny * nz;
         for (int i = 0; i < Q; ++i) w[i] = (R)L.w[i];
@@ -200,6 +202,7 @@ struct Sim : ref_ctx {
         k_react = (R)pp.k_react;
         f.assign((size_t)S * Q * N, (R)0); fnew = f;
         if (has_scalar) { h.assign((size_t)Qs * N, (R)0); hnew = h; }
+        if (has_thermal) { g.assign((size_t)Q * N, (R)0); gnew = g; }
         rho.assign((size_t)S * N, (R)0);
         jm.assign((size_t)S * 3 * N, (R)0);
         psi.assign((size_t)S * N, (R)0);
@@ -355,6 +358,7 @@ struct Sim : ref_ctx {
                         for (int s = 0; s < S; ++s)
                             for (int i = 0; i < Q; ++i) F_(fnew, s, i, cell) = F_(f, s, i, cell);
                         if (has_scalar) for (int i = 0; i < Qs; ++i) H_(hnew, i, cell) = H_(h, i, cell);
+                        if (has_thermal) for (int i = 0; i < Q; ++i) H_(gnew, i, cell) = H_(g, i, cell);
                         continue;
                     }
                     R u[3] = {ub[cell], ub[N + cell], ub[2 * N + cell]};
@@ -396,6 +400,20 @@ struct Sim : ref_ctx {
                             }
                         }
                     }
+                    /* internal-energy lattice (IEDDF), Eq. 27 with g^eq = w_i rho eps [1 + 3 cu + 4.5 cu^2
+                     * - 1.5 u.u], Eq. 30 (c_s^2 = 1/3), rho eps = sum_i g_i (Eq. 29); u: DESIGN R25 */
+                    if (has_thermal) {
+                        R E = (R)0;
+                        for (int i = 0; i < Q; ++i) E = E + H_(g, i, cell);
+                        for (int i = 0; i < Q; ++i) {
+                            R gi = H_(g, i, cell);
+                            R ge = feq(i, E, u);
+                            R gstar = gi - omega_c * (gi - ge);
+                            size_t nb;
+                            if (neighbour(x, y, z, L.c[i], nb)) H_(gnew, i, nb) = gstar;
+                            else H_(gnew, L.opp[i], cell) = gstar;     /* adiabatic wall: plain reflection */
+                        }
+                    }
                     /* 6. scalar lattice: Eq. 34-36 + first-order source (DESIGN R8) */
                     if (has_scalar) {
                         R C = (R)0;
@@ -418,6 +436,7 @@ struct Sim : ref_ctx {
                 }
         f.swap(fnew);
         if (has_scalar) h.swap(hnew);
+        if (has_thermal) g.swap(gnew);
     }
 
     int step(int n) override {
@@ -534,6 +553,8 @@ struct Sim : ref_ctx {
                             for (int a = 0; a < d; ++a) cu = cu + (R)Ls.c[i][a] * u[a];
                             H_(h, i, cell) = (ws[i] * (R)c0) * ((R)1 + inv_cs2g * cu);
                         }
+                    if (has_thermal)      /* g_i = g^eq(rho eps, u), eps = c_init */
+                        for (int i = 0; i < Q; ++i) H_(g, i, cell) = feq(i, (R)r0[0] * (R)c0, u);
                 }
         inited = true;
         return 0;
@@ -541,7 +562,7 @@ struct Sim : ref_ctx {
 
     int get_macros(void* rho_o, void* u_o, void* phi_o, void* C_o) override {
         if (!inited) { g_err = "get_macros before init"; return -4; }
-        if (C_o && !has_scalar) { g_err = "model has no scalar lattice"; return -1; }
+        if (C_o && !has_scalar && !has_thermal) { g_err = "model has no scalar lattice"; return -1; }
         moments_and_force();
         if (rho_o) std::memcpy(rho_o, rho.data(), sizeof(R) * S * N);
         if (u_o) std::memcpy(u_o, ub.data(), sizeof(R) * d * N);
@@ -562,6 +583,12 @@ struct Sim : ref_ctx {
             R* Cc = (R*)C_o;
             for (size_t cell = 0; cell < N; ++cell) {
                 R C = (R)0;
+                if (has_thermal) {      /* internal energy eps = sum_i g_i / rho, Eq. 29 */
+                    for (int i = 0; i < Q && !solid[cell]; ++i) C = C + H_(g, i, cell);
+                    if (!solid[cell]) C = C * ((R)1 / rho[cell]);
+                    Cc[cell] = C;
+                    continue;
+                }
                 for (int i = 0; i < Qs && !solid[cell]; ++i) C = C + H_(h, i, cell);
                 Cc[cell] = C;
             }
@@ -588,19 +615,21 @@ struct Sim : ref_ctx {
         return 0;
     }
 
-    size_t population_count() override { return (size_t)S * Q * N + (has_scalar ? (size_t)Qs * N : 0); }
+    size_t population_count() override { return (size_t)S * Q * N + (has_scalar ? (size_t)Qs * N : 0) + (has_thermal ? (size_t)Q * N : 0); }
 
     int get_populations(void* out) override {
         if (!inited) { g_err = "get_populations before init"; return -4; }
         R* o = (R*)out;
         std::memcpy(o, f.data(), sizeof(R) * f.size());
         if (has_scalar) std::memcpy(o + f.size(), h.data(), sizeof(R) * h.size());
+        if (has_thermal) std::memcpy(o + f.size(), g.data(), sizeof(R) * g.size());
         return 0;
     }
     int set_populations(const void* in) override {
         const R* o = (const R*)in;
         std::memcpy(f.data(), o, sizeof(R) * f.size());
         if (has_scalar) std::memcpy(h.data(), o + f.size(), sizeof(R) * h.size());
+        if (has_thermal) std::memcpy(g.data(), o + f.size(), sizeof(R) * g.size());
         inited = true;
         return 0;
     }
@@ -615,14 +644,14 @@ ref_ctx* ref_create(int nx, int ny, int nz, int lattice, int model, const ref_pa
     if (nx < 1 || ny < 1 || nz < 1) { g_err = "bad grid"; return nullptr; }
     if (lattice != REF_D2Q9 && lattice != REF_D3Q19) { g_err = "bad lattice"; return nullptr; }
     if (lattice == REF_D2Q9 && nz != 1) { g_err = "D2Q9 needs nz == 1"; return nullptr; }
-    if (model < REF_BGK || model > REF_SC2_ADE) { g_err = "bad model"; return nullptr; }
+    if (model < REF_BGK || model > REF_BGK_T) { g_err = "bad model"; return nullptr; }
     if (p->precision != 32 && p->precision != 64) { g_err = "precision must be 32 or 64"; return nullptr; }
     if (p->forcing != 0 && p->forcing != 1) { g_err = "forcing must be 0 (Guo) or 1 (velocity shift)"; return nullptr; }
     if (p->psi_kind != 0 && p->psi_kind != 1) { g_err = "bad psi_kind"; return nullptr; }
     int S = (model == REF_SC2 || model == REF_SC2_ADE) ? 2 : 1;
     for (int s = 0; s < S; ++s)
         if (!(p->tau[s] > 0.5)) { g_err = "tau must exceed 0.5"; return nullptr; }
-    if (model == REF_SC2_ADE && !(p->tau_c > 0.5)) { g_err = "tau_c must exceed 0.5"; return nullptr; }
+    if ((model == REF_SC2_ADE || model == REF_BGK_T) && !(p->tau_c > 0.5)) { g_err = "tau_c must exceed 0.5"; return nullptr; }
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != 0 && p->bc[a] != 1) { g_err = "bad bc"; return nullptr; }
 

@@ -26,7 +26,8 @@ extern "C" {
 enum { REF_D2Q9 = 0, REF_D3Q19 = 1 };
 /* model: BGK (Eq. 3-8), single-component Shan-Chen (Eq. 11), two-component Shan-Chen (Eq. 13),
  * two-component Shan-Chen + advection-diffusion scalar lattice (Eq. 34-36) with reaction source */
-enum { REF_BGK = 0, REF_SC1 = 1, REF_SC2 = 2, REF_SC2_ADE = 3 };
+enum { REF_BGK = 0, REF_SC1 = 1, REF_SC2 = 2, REF_SC2_ADE = 3,
+       REF_BGK_T = 4 /* BGK + internal-energy lattice g_i on the flow lattice, Eq. 27-30 */ };
 /* init kinds */
 enum { REF_INIT_REST = 0, REF_INIT_TAYLOR_GREEN = 1, REF_INIT_DROPLET = 2,
        REF_INIT_UNIFORM_NOISE = 3, REF_INIT_RANDOM_DROPLETS = 4 };

@@ -11,10 +11,10 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 
 D2Q9, D3Q19 = 0, 1
-BGK, SC1, SC2, SC2_ADE = 0, 1, 2, 3
+BGK, SC1, SC2, SC2_ADE, BGK_T = 0, 1, 2, 3, 4
 INIT_REST, INIT_TAYLOR_GREEN, INIT_DROPLET, INIT_UNIFORM_NOISE, INIT_RANDOM_DROPLETS = 0, 1, 2, 3, 4
 LATTICES = {"D2Q9": D2Q9, "D3Q19": D3Q19}
-MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE}
+MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE, "BGK_T": BGK_T}
 INITS = {"REST": INIT_REST, "TAYLOR_GREEN": INIT_TAYLOR_GREEN, "DROPLET": INIT_DROPLET,
          "UNIFORM_NOISE": INIT_UNIFORM_NOISE, "RANDOM_DROPLETS": INIT_RANDOM_DROPLETS}
 
@@ -118,6 +118,7 @@ class RefLBM:
         self.Q = 19 if self.lattice == D3Q19 else 9
         self.Qs = 7 if self.lattice == D3Q19 else 5
         self.has_scalar = self.model == SC2_ADE
+        self.has_thermal = self.model == BGK_T
         self.N = self.nx * self.ny * self.nz
         self.h = self.L.ref_create(self.nx, self.ny, self.nz, self.lattice, self.model, C.byref(self.p))
         if not self.h:
@@ -138,7 +139,7 @@ class RefLBM:
         rho = np.empty((self.S, self.N), self.dtype)
         u = np.empty((self.d, self.N), self.dtype)
         phi = np.empty(self.N, self.dtype)
-        Cc = np.empty(self.N, self.dtype) if self.has_scalar else None
+        Cc = np.empty(self.N, self.dtype) if (self.has_scalar or self.has_thermal) else None
         self._chk(self.L.ref_get_macros(self.h, rho.ctypes.data, u.ctypes.data, phi.ctypes.data,
                                         Cc.ctypes.data if Cc is not None else None))
         return {"rho": rho, "u": u, "phi": phi, "C": Cc}
@@ -174,7 +175,7 @@ class RefLBM:
         """canonical vector -> (f[S,Q,N], h[Qs,N] or None)"""
         nf = self.S * self.Q * self.N
         ff = f[:nf].reshape(self.S, self.Q, self.N)
-        hh = f[nf:].reshape(self.Qs, self.N) if self.has_scalar else None
+        hh = f[nf:].reshape(self.Qs, self.N) if self.has_scalar else (f[nf:].reshape(self.Q, self.N) if self.has_thermal else None)
         return ff, hh
 
     def close(self):

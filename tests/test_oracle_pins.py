@@ -974,3 +974,64 @@ def test_flow_past_a_masked_obstacle_conserves_mass_and_stays_symmetric():
     ux = mac["u"][0].reshape(ny, nx); uy = mac["u"][1].reshape(ny, nx)
     assert np.abs(ux - ux[::-1, :]).max() < 1e-11 * ux.max() and np.abs(uy + uy[::-1, :]).max() < 1e-11 * ux.max()
     assert 0 < ux[fluid.reshape(ny, nx)].mean() < 0.5 * g * 1500
+
+
+# ----------------------------------------------------------------------------------------------
+# internal-energy lattice (IEDDF), model BGK_T: Eq. 27-30
+# ----------------------------------------------------------------------------------------------
+def thermal_setup(lattice, grid, u, eps, rho=1.2, **kw):
+    """populations f = f^eq(rho, u), g = g^eq(rho eps, u) built here from the lattice table (inputs, Eq. 6 / 30)"""
+    c, w = lattice_table(lattice)
+    r = RefLBM(*grid, lattice, "BGK_T", precision=64, **kw)
+    N = r.N
+    u = np.asarray(u, float)
+    cu = c[:, :r.d] @ u[:r.d]
+    poly = 1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u[:r.d] ** 2).sum()
+    f = (w * rho * poly)[:, None] * np.ones(N)
+    g = (w * poly)[:, None] * (rho * eps)[None, :]
+    r.set_populations(np.concatenate([f.ravel(), g.ravel()]))
+    return r
+
+
+@pytest.mark.parametrize("lattice,grid,axis", [("D2Q9", (48, 4, 1), 0), ("D2Q9", (4, 48, 1), 1), ("D3Q19", (3, 4, 48), 2)])
+def test_thermal_diffusion_and_advection(lattice, grid, axis):
+    """u = 0: a sine mode of eps decays as exp(-alpha k^2 t) with alpha = (tau_e - 1/2)/3 (tau_e =
+    3 alpha + 1/2); uniform u: the mode is carried along at u (Eq. 30 has the full second-order equilibrium);
+    sum g is conserved (Eq. 27 has no source)."""
+    n = grid[axis]
+    k = 2 * np.pi / n
+    shape = (grid[2], grid[1], grid[0])
+    s = np.arange(n)
+    idx = [None] * 3; idx[2 - axis] = slice(None)
+    mode = np.broadcast_to(np.sin(k * s)[tuple(idx)], shape).ravel()
+    tau_e = 0.8
+    r = thermal_setup(lattice, grid, (0, 0, 0), 1.0 + 0.1 * mode, tau=(0.9, 0.9), tau_c=tau_e)
+    e0 = r.get_macros()["C"]
+    assert np.allclose(e0, 1.0 + 0.1 * mode, atol=1e-15)
+    _, g0 = r.split_populations(r.get_populations())
+    r.step(200)
+    e1 = r.get_macros()["C"]
+    amp = ((e1 - 1.0) * mode).sum() / (mode ** 2).sum()
+    alpha = (tau_e - 0.5) / 3
+    assert abs(amp / (0.1 * np.exp(-alpha * k * k * 200)) - 1) < 2e-3
+    _, g1 = r.split_populations(r.get_populations())
+    assert abs(g1.sum() - g0.sum()) < 1e-12 * g0.sum()
+    # advection
+    U = [0.0, 0.0, 0.0]; U[axis] = 0.05
+    r = thermal_setup(lattice, grid, U, 1.0 + 0.1 * mode, tau=(0.9, 0.9), tau_c=tau_e)
+    r.step(240)                                  # shift by 12 cells
+    e2 = r.get_macros()["C"] - 1.0
+    cosm = np.broadcast_to(np.cos(k * s)[tuple(idx)], shape).ravel()
+    phase = np.arctan2(-(e2 * cosm).sum(), (e2 * mode).sum())
+    assert abs(phase / (k * 0.05 * 240) - 1) < 5e-3
+
+
+def test_thermal_uniform_state_and_init():
+    r = RefLBM(5, 4, 3, "D3Q19", "BGK_T", precision=64, tau=(0.7, 0.7), tau_c=0.9, rho_init=(1.3, 1.0), c_init=0.75,
+               bc=(0, 0, 1), force=(1e-6, 0.0, 0.0))
+    r.init_from_seed(0)
+    assert np.allclose(r.get_macros()["C"], 0.75, atol=1e-15)
+    r.step(50)
+    m = r.get_macros()
+    assert np.abs(m["C"] - 0.75).max() < 1e-13          # a uniform temperature stays uniform, also in a driven channel
+    assert np.abs(m["u"][0]).max() > 1e-5
