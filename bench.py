@@ -65,7 +65,7 @@ def ncu_traffic(workload):
 def shape_of(cfg):
     S = 2 if cfg["model"] in ("SC2", "SC2_ADE") else 1
     Q = 19 if cfg["lattice"] == "D3Q19" else 9
-    Qs = (7 if cfg["lattice"] == "D3Q19" else 5) if cfg["model"] == "SC2_ADE" else 0
+    Qs = (7 if cfg["lattice"] == "D3Q19" else 5) if cfg["model"] == "SC2_ADE" else (Q if cfg["model"] == "BGK_T" else 0)
     B = 8 if cfg["params"]["precision"] == 64 else 4
     N = cfg["grid"][0] * cfg["grid"][1] * cfg["grid"][2]
     sc = cfg["model"] != "BGK"
@@ -360,6 +360,7 @@ EXTRAS = [
     ("cfg3", dict(bc=(0, 1, 0), force=(0.0, -1e-5, 0.0), G_ads=(0.0, 0.0)), (1200, 400, 1), 500, 50, None,
      "Rayleigh-Taylor-shaped: walls in y + body force"),
     ("cfg3", dict(forcing=1), (8192, 8192, 1), 50, 5, None, "velocity-shift forcing scheme (Eq. 16-19)"),
+    ("cfgT", dict(), (256, 256, 256), 200, 20, None, "BGK + internal-energy lattice (IEDDF, Eq. 27-30)"),
 ]
 
 

@@ -47,7 +47,11 @@ enum { LBM_D2Q9 = 0, LBM_D3Q19 = 1 };
 
 /* model: BGK single phase; Shan-Chen one component (Eq. 11); Shan-Chen two components (Eq. 13);
  * two components + scalar lattice with reaction source (Eq. 34-36) */
-enum { LBM_BGK = 0, LBM_SC1 = 1, LBM_SC2 = 2, LBM_SC2_ADE = 3 };
+enum { LBM_BGK = 0, LBM_SC1 = 1, LBM_SC2 = 2, LBM_SC2_ADE = 3,
+       /* BGK + internal-energy lattice g_i on the flow lattice (IEDDF), Eq. 27-30:
+        * tau_c is its relaxation time tau_e = 3 alpha + 1/2, c_init the initial internal energy, the C output of
+        * lbm_get_macros the internal energy eps = sum_i g_i / rho; populations: f (Q*N) then g (Q*N) */
+       LBM_BGK_T = 4 };
 
 /* initial condition kinds of lbm_init_from_seed */
 enum { LBM_INIT_REST = 0, LBM_INIT_TAYLOR_GREEN = 1, LBM_INIT_DROPLET = 2,

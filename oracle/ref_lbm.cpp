@@ -173,7 +173,7 @@ struct Sim : ref_ctx {
         double w0s = pp.w0_scalar > 0.0 ? pp.w0_scalar : (lattice == REF_D3Q19 ? 0.25 : 0.4);
         Ls = make_scalar_lattice(lattice, w0s);
         S = (model == REF_SC2 || model == REF_SC2_ADE) ? 2 : 1;
-        has_sc = (model != REF_BGK);
+        has_sc = (model == REF_SC1 || model == REF_SC2 || model == REF_SC2_ADE);
         has_walls = pp.bc[0] || pp.bc[1] || pp.bc[2];
         moving_walls = false;
         for (int a = 0; a < 3; ++a)

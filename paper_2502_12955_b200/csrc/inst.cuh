@@ -80,6 +80,13 @@ struct Launch {
                 else if (forced) step3<M_BGK, w, true>(p, parity, st);
                 else step3<M_BGK, w, false>(p, parity, st);
             });
+        } else if (model == M_BGK_T) {
+            if (forced == 2) return cudaErrorInvalidValue;
+            ok = with_int<3>(wmode, [&](auto W) {
+                constexpr int w = decltype(W)::value;
+                if (forced) step3<M_BGK_T, w, true>(p, parity, st);
+                else step3<M_BGK_T, w, false>(p, parity, st);
+            });
         } else {
             ok = with_sc_model(model, [&](auto M) {
                 with_int<3>(wmode, [&](auto W) {
@@ -105,6 +112,7 @@ struct Launch {
         R *r = (R*)rho, *uu = (R*)u, *ph = (R*)phi, *c = (R*)C, *f = (R*)F;
         if (wmode < 0 || wmode > 2) return cudaErrorInvalidValue;
         if (model == M_BGK) macros2<M_BGK>(p, parity, wmode, r, uu, ph, c, f, st);
+        else if (model == M_BGK_T) macros2<M_BGK_T>(p, parity, wmode, r, uu, ph, c, f, st);
         else if (!with_sc_model(model, [&](auto M) { macros2<decltype(M)::value>(p, parity, wmode, r, uu, ph, c, f, st); }))
             return cudaErrorInvalidValue;
         return cudaGetLastError();
@@ -132,6 +140,11 @@ struct Launch {
             if (to_canonical) permute2<LS, true>(p, parity, wmode, p.h, ch, 1, st);
             else permute2<LS, false>(p, parity, wmode, p.h, ch, 1, st);
         }
+        if (model == M_BGK_T) {     // the internal-energy lattice lives on the flow lattice
+            R* ch = cf + (size_t)S * L::Q * (size_t)p.N;
+            if (to_canonical) permute2<L, true>(p, parity, wmode, p.h, ch, 1, st);
+            else permute2<L, false>(p, parity, wmode, p.h, ch, 1, st);
+        }
         return cudaGetLastError();
     }
 
@@ -143,6 +156,7 @@ struct Launch {
         case M_SC1: k_init<R, L, M_SC1><<<g, block_for(p), 0, st>>>(p, *ia); break;
         case M_SC2: k_init<R, L, M_SC2><<<g, block_for(p), 0, st>>>(p, *ia); break;
         case M_SC2_ADE: k_init<R, L, M_SC2_ADE><<<g, block_for(p), 0, st>>>(p, *ia); break;
+        case M_BGK_T: k_init<R, L, M_BGK_T><<<g, block_for(p), 0, st>>>(p, *ia); break;
         default: return cudaErrorInvalidValue;
         }
         return cudaGetLastError();

@@ -24,7 +24,7 @@
 
 namespace lbm {
 
-enum { M_BGK = 0, M_SC1 = 1, M_SC2 = 2, M_SC2_ADE = 3 };
+enum { M_BGK = 0, M_SC1 = 1, M_SC2 = 2, M_SC2_ADE = 3, M_BGK_T = 4 };
 enum { I_REST = 0, I_TAYLOR_GREEN = 1, I_DROPLET = 2, I_UNIFORM_NOISE = 3, I_RANDOM_DROPLETS = 4 };
 
 constexpr int BLOCK = 256;   // largest block any kernel is launched with; the launchers pick blockDim.x (inst.cuh)
@@ -60,8 +60,10 @@ struct InitArgs {
 
 template <int MODEL> struct ModelTraits {
     static constexpr int S = (MODEL == M_SC2 || MODEL == M_SC2_ADE) ? 2 : 1;
-    static constexpr bool SC = MODEL != M_BGK;
+    static constexpr bool SC = MODEL == M_SC1 || MODEL == M_SC2 || MODEL == M_SC2_ADE;
     static constexpr bool SCALAR = MODEL == M_SC2_ADE;
+    // internal-energy lattice g_i on the flow lattice (IEDDF, Eq. 27-30), stored in KP::h
+    static constexpr bool THERMAL = MODEL == M_BGK_T;
 };
 
 // ------------------------------------------------------------------------------------------
@@ -543,6 +545,8 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     });
     R hl[LS::Q];
     if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
+    R gl[Q];
+    if constexpr (MT::THERMAL) load_pops<L, PARITY, WALLS>(p.h, nb, N, gl);
 
     CellMacro<R, L, MODEL> m;
     cell_macros<R, L, MODEL, FORCED, COH>(p, nb, fl, m);
@@ -580,6 +584,14 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     if constexpr (MT::SCALAR) {
         collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
         store_pops<LS, PARITY, WALLS>(p.h, ns, N, hl);
+    }
+    if constexpr (MT::THERMAL) {
+        // Eq. 27 with g^eq = w_i (rho eps) [1 + 3 cu + 4.5 cu^2 - 1.5 u.u] (Eq. 30), rho eps = sum_i g_i (Eq. 29):
+        // the LBGK relaxation of Eq. 6 with sum g in place of rho and tau_e in place of tau; reflected at walls
+        R E = gl[0];
+        static_for<1, Q>([&](auto ic) { E = E + gl[decltype(ic)::value]; });
+        collide<R, L, false>(gl, E, m.u, m.F[0], p.omega_c, p.cf[0]);
+        store_pops<L, PARITY, WALLS>(p.h, ns, N, gl);
     }
 }
 
@@ -650,6 +662,15 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
             R C = hl[0];
             static_for<1, LS::Q>([&](auto ic) { C = C + hl[decltype(ic)::value]; });
             C_o[cell] = C;
+        }
+    }
+    if constexpr (MT::THERMAL) {
+        if (C_o) {      // internal energy eps = sum_i g_i / rho, Eq. 29
+            R gl[Q];
+            load_pops<L, PARITY, WALLS>(p.h, nb, N, gl);
+            R E = gl[0];
+            static_for<1, Q>([&](auto ic) { E = E + gl[decltype(ic)::value]; });
+            C_o[cell] = E * m.inv_rho;
         }
     }
     if (F_o)
@@ -788,6 +809,14 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
             const R cu = dotc<LS, i>(u);
             const R wsi = i == 0 ? p.ws0 : p.ws1;
             p.h[(size_t)i * N + cell] = (wsi * (R)c0) * ((R)1 + p.inv_cs2g * cu);
+        });
+    }
+    if constexpr (MT::THERMAL) {     // g_i = g^eq(rho eps, u), eps = c_init: Eq. 30
+        const R rhoE = (R)r0[0] * (R)c0;
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            const R cu = dotc<L, i>(u);
+            p.h[(size_t)i * N + cell] = ((R)L::w(i) * rhoE) * ((base + (R)3 * cu) + ((R)4.5 * cu) * cu);
         });
     }
 }

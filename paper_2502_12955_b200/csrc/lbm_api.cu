@@ -49,7 +49,7 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (nx < 1 || ny < 1 || nz < 1) return "grid extents must be >= 1";
     if (lattice != LBM_D2Q9 && lattice != LBM_D3Q19) return "unknown lattice";
     if (lattice == LBM_D2Q9 && nz != 1) return "D2Q9 needs nz == 1";
-    if (model < LBM_BGK || model > LBM_SC2_ADE) return "unknown model";
+    if (model < LBM_BGK || model > LBM_BGK_T) return "unknown model";
     if (p->precision != 32 && p->precision != 64) return "precision must be 32 or 64";
     if (p->forcing != 0 && p->forcing != 1) return "forcing must be 0 (Guo) or 1 (Shan-Chen velocity shift)";
     if (p->psi_kind != 0 && p->psi_kind != 1) return "psi_kind must be 0 or 1";
@@ -60,7 +60,8 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     const int S = (model == LBM_SC2 || model == LBM_SC2_ADE) ? 2 : 1;
     for (int s = 0; s < S; ++s)
         if (!(p->tau[s] > 0.5)) return "tau must exceed 0.5";
-    if (model == LBM_SC2_ADE && !(p->tau_c > 0.5)) return "tau_c must exceed 0.5";
+    if ((model == LBM_SC2_ADE || model == LBM_BGK_T) && !(p->tau_c > 0.5)) return "tau_c must exceed 0.5";
+    if (model == LBM_BGK_T && p->forcing != 0) return "LBM_BGK_T runs with Guo forcing only";
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != 0 && p->bc[a] != 1) return "bc must be 0 (periodic) or 1 (bounce-back walls)";
     }
@@ -78,8 +79,9 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
         sh->d = lattice == LBM_D3Q19 ? 3 : 2;
         sh->Q = lattice == LBM_D3Q19 ? 19 : 9;
         sh->Qs = lattice == LBM_D3Q19 ? 7 : 5;
-        sh->sc = model != LBM_BGK;
-        sh->scalar = model == LBM_SC2_ADE;
+        if (model == LBM_BGK_T) sh->Qs = sh->Q;            // second lattice = internal-energy lattice on the flow lattice
+        sh->sc = model == LBM_SC1 || model == LBM_SC2 || model == LBM_SC2_ADE;
+        sh->scalar = model == LBM_SC2_ADE || model == LBM_BGK_T;     // has a second lattice (KP::h) of Qs values per cell
         sh->N = (size_t)nx * ny * nz;
         sh->B = p->precision == 64 ? 8 : 4;
         sh->f_bytes = align_up((size_t)S * sh->Q * sh->N * sh->B, 256);
@@ -170,7 +172,7 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     k.omega_c = (R)(1.0 / p.tau_c);
     k.inv_cs2g = (R)((double)c->sh.d / (1.0 - w0s));
     k.ws0 = (R)w0s;
-    k.ws1 = (R)((1.0 - w0s) / (double)(c->sh.Qs - 1));
+    k.ws1 = (R)((1.0 - w0s) / (double)((c->lattice == LBM_D3Q19 ? 7 : 5) - 1));
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
             for (int b = 0; b < 3; ++b) k.wall_u[a][sd][b] = (R)p.wall_u[a][sd][b];
@@ -653,6 +655,7 @@ int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
     if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
     if (c->sh.sc && c->walls) return fail(LBM_EINVAL, "Shan-Chen models between walls run on LBM_PATH_REGISTER only");
     if (c->moving) return fail(LBM_EINVAL, "moving walls run on LBM_PATH_REGISTER only");
+    if (c->model == LBM_BGK_T) return fail(LBM_EINVAL, "LBM_BGK_T runs on LBM_PATH_REGISTER only");
     if (c->kp64.mask) return fail(LBM_EINVAL, "a solid-node mask runs on LBM_PATH_REGISTER only");
     if (path == LBM_PATH_WAVEFRONT) {
         if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");

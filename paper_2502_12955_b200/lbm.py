@@ -12,9 +12,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liblbm.so")
 
 D2Q9, D3Q19 = 0, 1
-BGK, SC1, SC2, SC2_ADE = 0, 1, 2, 3
+BGK, SC1, SC2, SC2_ADE, BGK_T = 0, 1, 2, 3, 4
 LATTICES = {"D2Q9": D2Q9, "D3Q19": D3Q19}
-MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE}
+MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE, "BGK_T": BGK_T}
 INITS = {"REST": 0, "TAYLOR_GREEN": 1, "DROPLET": 2, "UNIFORM_NOISE": 3, "RANDOM_DROPLETS": 4}
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 PATHS = {"register": 0, "pipeline": 1, "wavefront": 2}
@@ -188,7 +188,7 @@ class LBM:
         self.d = 3 if self.lattice == D3Q19 else 2
         self.Q = 19 if self.lattice == D3Q19 else 9
         self.Qs = 7 if self.lattice == D3Q19 else 5
-        self.has_scalar = self.model == SC2_ADE
+        self.has_scalar = self.model in (SC2_ADE, BGK_T)      # a second lattice with a C / eps output
         self.N = self.nx * self.ny * self.nz
         self.h = None
         self.device = torch.device(device)

@@ -81,6 +81,11 @@ SMALL = [
     ("cfg5", (33, 17, 9), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
     ("cfg3", (16, 8, 1), dict(precision=32)),
+    # internal-energy lattice (model BGK_T, Eq. 27-30)
+    ("cfgT", (9, 6, 7), {}),
+    ("cfgT", (33, 5, 4), dict(precision=32, bc=(1, 0, 1))),
+    ("cfgT2", (33, 17, 1), {}),
+    ("cfgT2", (8, 9, 1), dict(bc=(0, 1, 0), force=(1e-5, 0.0, 0.0))),
     # moving-wall bounce-back (Couette, Eq. 41)
     ("cfg4", (5, 4, 7), dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, -0.01, 0.0)})),
     ("cfg4", (6, 5, 4), dict(bc=(1, 1, 1), wall_u={(0, 0): (0.0, 0.01, 0.02), (1, 1): (0.01, 0.0, -0.01), (2, 0): (0.02, 0.01, 0.0)}, precision=32)),
@@ -467,6 +472,7 @@ MASK_CASES = [
     ("cfg4", (12, 6, 5), dict(bc=(0, 0, 0), precision=32)),
     ("cfg4", (7, 6, 5), dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, 0.0, 0.0)})),
     ("cfg2", (16, 12, 1), dict(radius=4.0, G_ads=(-0.3, 0.0))),
+    ("cfgT", (9, 8, 6), {}),
     ("cfg3", (14, 11, 1), dict(G_ads=(-0.2, 0.3))),
     ("cfg5", (10, 8, 6), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, G_ads=(0.2, -0.2))),
     ("cfg5", (8, 7, 6), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, forcing=1, bc=(0, 1, 0), precision=64, tau=(0.9, 1.2))),

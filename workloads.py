@@ -30,6 +30,13 @@ CONFIGS = {
                  params=dict(precision=32, tau=(1.0, 1.0), tau_c=0.8, psi_kind=1, G=G12, k_react=1e-3,
                              init_kind="RANDOM_DROPLETS", rho_in=1.9, rho_out=0.1, c_init=1.0, width=3.0,
                              rmin=10.0, rmax=30.0, vol_frac=0.05)),
+    # beyond BASELINE.json: BGK + internal-energy lattice (IEDDF, Eq. 27-30), 3D channel / 2D box
+    "cfgT": dict(grid=(64, 64, 64), lattice="D3Q19", model="BGK_T", steps=1000,
+                 params=dict(precision=64, tau=(0.9, 0.9), tau_c=0.8, force=(1e-6, 0.0, 0.0), bc=(0, 0, 1),
+                             init_kind="TAYLOR_GREEN", u0=0.02, rho_init=(1.0, 1.0), c_init=0.5)),
+    "cfgT2": dict(grid=(128, 128, 1), lattice="D2Q9", model="BGK_T", steps=1000,
+                  params=dict(precision=64, tau=(0.8, 0.8), tau_c=0.7, init_kind="TAYLOR_GREEN", u0=0.03,
+                              rho_init=(1.0, 1.0), c_init=1.5)),
 }
 
 
