@@ -6,11 +6,15 @@
  * "PAPER.md:<line>" + equation):
  *   - LBGK collision with Guo forcing on D2Q9 / D3Q19 populations
  *         Eq. 3-8, Eq. 15, Eq. 20-23
+ *     or with the Shan-Chen velocity-shift forcing scheme, Eq. 16-19
  *   - Shan-Chen pseudopotential interaction force, one or two components
  *         Eq. 10-11, Eq. 13, Eq. 24
+ *     with solid nodes left out of the sums (Eq. 12) and the fluid-solid adhesion force (Eq. 14)
  *   - an advection-diffusion scalar lattice D2Q5 / D3Q7 with a first-order interface reaction
  *     source, Eq. 34-36; source term and D3Q7: DESIGN.md readings R6, R8
- *   - periodic boundaries and halfway bounce-back walls
+ *   - an internal-energy lattice on the flow lattice (IEDDF), Eq. 27-30
+ *   - periodic boundaries, halfway bounce-back walls at rest or moving (Couette
+ *     flow Eq. 41) and halfway bounce-back on the solid nodes of a mask
  * Every step of that path runs in CUDA kernels; there is no CPU fallback.  If no CUDA device
  * is usable, lbm_create returns NULL and lbm_last_error() says why.
  *
