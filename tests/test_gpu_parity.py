@@ -543,3 +543,73 @@ def test_masked_graph_replay_and_mass(gpu):
     assert np.array_equal(fr, fd)
     fluid = np.tile(m.ravel() == 0, 9)
     assert abs(fd[fluid].sum() - (m == 0).sum()) < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------------
+# the BASELINE.json configurations at their full sizes and step counts, checked by what the method fixes
+# (closed forms and invariants; R15: field parity with the oracle is at 1000 steps, see above)
+# ------------------------------------------------------------------------------------------------------
+def test_cfg2_laplace_law_full_run(gpu):
+    """configs[1] as stated: 256x256, R in {20, 30, 40, 50}, 20000 steps each: the pressure jump of the relaxed
+    droplet, p = rho/3 + (G/6) psi^2, times the MEASURED radius is the same constant for every droplet
+    (Laplace law dp = gamma / R: PAPER.md:636-676); mass conserved to round-off."""
+    res = []
+    for R in (20.0, 30.0, 40.0, 50.0):
+        cfg = workloads.config("cfg2", radius=R)
+        dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+        dev.init_from_seed(2)
+        m0 = dev.get_macros(u=False, phi=False)["rho"].sum().item()
+        dev.step(20000)
+        mac = dev.get_macros(phi=False)
+        rho = mac["rho"][0].cpu().numpy().reshape(256, 256)
+        assert abs(rho.sum() / m0 - 1) < 1e-10
+        psi = 1 - np.exp(-rho)
+        p = rho / 3 + (-5.0 / 6) * psi ** 2
+        rin, rout = rho[128, 128], rho[0, 0]
+        assert rin > 1.8 and rout < 0.2
+        reff = np.sqrt(((rho - rout) / (rin - rout)).sum() / np.pi)
+        res.append((1 / reff, p[128, 128] - p[0, 0]))
+        assert mac["u"].abs().max().item() < 0.02
+    inv_r, dp = np.array(res).T
+    gamma = dp / inv_r
+    assert (dp > 0).all() and (np.diff(dp) < 0).all()
+    assert gamma[1:].max() / gamma[1:].min() - 1 < 0.03        # the three larger droplets
+    assert gamma.max() / gamma.min() - 1 < 0.10                # all four (the smallest shrinks to R_eff ~ 8)
+
+
+def test_cfg3_full_run_mass_and_demixing(gpu):
+    """configs[2] as stated: 512x512, 10000 steps of spinodal decomposition: per-component mass conserved to
+    round-off, the mixture has separated into A-rich and B-rich domains, everything finite."""
+    cfg = workloads.config("cfg3")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(3)
+    m0 = dev.get_macros(u=False, phi=False)["rho"].sum(1).cpu().numpy()
+    dev.step(10000)
+    mac = dev.get_macros()
+    m1 = mac["rho"].sum(1).cpu().numpy()
+    assert np.abs(m1 / m0 - 1).max() < 1e-10
+    phi = mac["phi"].cpu().numpy()
+    assert np.isfinite(phi).all() and bool(torch.isfinite(mac["u"]).all().item())
+    assert (phi > 0.5).mean() > 0.2 and (phi < -0.5).mean() > 0.2       # two phases, each a sizeable share of the box
+    assert abs(phi.mean()) < 0.05                                        # symmetric mixture
+
+
+def test_cfg5_full_run_invariants(gpu):
+    """configs[4] as stated: 512^3, fp32, 2000 steps: masses of A and B conserved (fp32 populations, fp64 sums),
+    total C decreasing and bounded below by C0 (1 - k)^t (the reaction factor 4 rhoA rhoB / rho^2 is <= 1), no NaN."""
+    cfg = workloads.config("cfg5")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(42)
+    m = dev.get_macros(u=False, phi=False)
+    m0 = m["rho"].double().sum(1).cpu().numpy()
+    c0 = m["C"].double().sum().item()
+    del m
+    dev.step(2000)
+    m = dev.get_macros(phi=False)
+    assert bool(torch.isfinite(m["u"]).all().item()) and bool(torch.isfinite(m["rho"]).all().item())
+    m1 = m["rho"].double().sum(1).cpu().numpy()
+    c1 = m["C"].double().sum().item()
+    assert np.abs(m1 / m0 - 1).max() <= 1e-3
+    assert c0 * (1 - 1e-3) ** 2000 * (1 - 1e-4) <= c1 < c0
+    del m, dev
+    torch.cuda.empty_cache()
