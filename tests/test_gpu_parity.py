@@ -613,3 +613,25 @@ def test_cfg5_full_run_invariants(gpu):
     assert c0 * (1 - 1e-3) ** 2000 * (1 - 1e-4) <= c1 < c0
     del m, dev
     torch.cuda.empty_cache()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("LBM_LONG"), reason="9 min on a B200: set LBM_LONG=1")
+def test_cfg4_full_size_steady_state(gpu):
+    """configs[3] 'run to steady state' at the full 256^3 (700 000 steps, fp64): the Poiseuille profile with the
+    halfway-bounce-back slip term, u_x(z) = g/(2 nu) (z+1/2)(H-z-1/2) + g/(8 nu) (16 (tau-1/2)^2/3 - 1)."""
+    cfg = workloads.config("cfg4")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(0)
+    for _ in range(70):
+        dev.step(10000)
+        dev.synchronize()
+    nz, tau, g = 256, 0.9, 1e-6
+    nu = (tau - 0.5) / 3
+    u = dev.get_macros(phi=False)["u"].reshape(3, nz, -1)
+    z = np.arange(nz)
+    exact = g / (2 * nu) * (z + 0.5) * (nz - z - 0.5) + g / (8 * nu) * (16 * (tau - 0.5) ** 2 / 3 - 1)
+    ux = u[0].cpu().numpy()
+    err = np.abs(ux - exact[:, None]).max() / exact.max()
+    print("cfg4 256^3 steady state: max |u_x - exact| / u_max = %.3e" % err)
+    assert err < 1e-5
+    assert u[1:].abs().max().item() < 1e-9 * exact.max()
