@@ -151,6 +151,7 @@ struct Sim : ref_ctx {
     R omega[2], cf[2], tau_r[2], omega_c, inv_cs2g;
     R G[2][2], G_ads[2], rho0_psi, force[3], k_react;
     R wall_u[3][2][3];
+    R psi_wall;            /* psi(rho_s) of Eq. 12 (single component), 0 when rho_wall = 0 */
     bool moving_walls;
     bool has_walls;
 
@@ -198,6 +199,7 @@ struct Sim : ref_ctx {
         omega_c = (R)(1.0 / pp.tau_c);                     /* Eq. 34 */
         inv_cs2g = (R)((double)d / (1.0 - w0s));           /* 1/c_{s,g}^2, Eq. 35, DESIGN R6 */
         rho0_psi = (R)pp.rho0_psi;
+        psi_wall = pp.rho_wall > 0.0 ? psi_of((R)pp.rho_wall) : (R)0;
         for (int a = 0; a < 3; ++a) force[a] = (R)pp.force[a];
         k_react = (R)pp.k_react;
         f.assign((size_t)S * Q * N, (R)0); fnew = f;
@@ -312,6 +314,9 @@ struct Sim : ref_ctx {
                                 Fa = -(psi[(size_t)s * N + cell] * t);
                                 /* fluid-solid adhesion, Eq. 14: -G_ads rho^s sum_i w_i s c_i */
                                 if (has_walls || has_mask) Fa = Fa + (-((G_ads[s] * rho[(size_t)s * N + cell]) * adh[a]));
+                                /* solid term of Eq. 12, one component: -G psi(x) sum_solid w_i psi(rho_s) c_i */
+                                if ((has_walls || has_mask) && S == 1 && p.rho_wall > 0.0)
+                                    Fa = Fa + (-((G[0][0] * psi[cell]) * (psi_wall * adh[a])));
                             }
                             /* constant body-force density; split by mass fraction for S=2 (DESIGN R5) */
                             R Fext = (S == 1) ? force[a] : force[a] * (rho[(size_t)s * N + cell] * inv_rho);

@@ -50,6 +50,7 @@ typedef struct ref_params {
     double   c_init;
     double   rho_in, rho_out, radius, width, noise_amp, u0, rmin, rmax, vol_frac;
     double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14; solid = beyond a wall */
+    double   rho_wall;      /* SC1: density rho_s of the solid nodes in Eq. 12; 0: no such term */
     double   wall_u[3][2][3]; /* velocity of the wall at the low / high face of each wall axis (moving-wall bounce-back) */
 } ref_params;
 

@@ -1035,3 +1035,25 @@ def test_thermal_uniform_state_and_init():
     m = r.get_macros()
     assert np.abs(m["C"] - 0.75).max() < 1e-13          # a uniform temperature stays uniform, also in a driven channel
     assert np.abs(m["u"][0]).max() > 1e-5
+
+
+def test_single_component_solid_term_of_eq12():
+    """Eq. 12: next to a solid node the single-component force gains -G psi(x) sum_solid w_i psi(rho_s) c_i.
+    Uniform fluid next to a flat wall with inward normal n: sum_fluid w_i c_i = +n/6, sum_solid w_i c_i = -n/6, so the
+    fluid part is -G psi^2 n/6 and the solid part +G psi psi(rho_s) n/6; with rho_s equal to the fluid density the two cancel (the wall looks like more
+    of the same fluid), and a denser / lighter virtual wall attracts / repels (G < 0)."""
+    G, rho = -5.0, 0.7
+    def wall_force(rho_wall):
+        r = RefLBM(4, 6, 1, "D2Q9", "SC1", precision=64, tau=(1.0, 1.0), psi_kind=0, rho0_psi=1.0, G=((G, 0), (0, 0)),
+                   bc=(0, 1, 0), init_kind="REST", rho_init=(rho, 1.0), rho_wall=rho_wall)
+        r.init_from_seed(0)
+        return r.get_force().reshape(1, 2, 6, 4)
+    psi = 1 - np.exp(-rho)
+    F0 = wall_force(0.0)
+    assert np.allclose(F0[0, 1, 0], -G * psi * psi / 6.0, rtol=1e-13) and np.abs(F0[0, 1, 2:4]).max() < 1e-16
+    Fs = wall_force(rho)
+    assert np.abs(Fs).max() < 1e-15                              # same density: no net force anywhere
+    Fd = wall_force(2.0)
+    psw = 1 - np.exp(-2.0)
+    assert np.allclose(Fd[0, 1, 0], -G * psi * (psi - psw) / 6.0, rtol=1e-13)
+    assert Fd[0, 1, 0, 0] < 0 < Fd[0, 1, -1, 0]                  # denser wall attracts the fluid (towards y = -1/2 and y = ny - 1/2)
