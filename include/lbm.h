@@ -90,6 +90,8 @@ typedef struct lbm_params {
     double   rmin, rmax, vol_frac;  /* RANDOM_DROPLETS: radius range and target volume fraction */
     double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14:
                                F_ads = -G_ads rho sum_i w_i s(x + c_i) c_i; < 0 wetting, > 0 non-wetting */
+    double   rho_wall;      /* LBM_SC1: density rho_s of the solid nodes in Eq. 12: adds
+                               -G psi(x) sum_solid w_i psi(rho_s) c_i; 0: no such term */
     double   wall_u[3][2][3];  /* [axis][0 low face, 1 high face][component]: velocity of that wall (used where
                                bc[axis] == 1).  A population reflected by a moving wall loses
                                2 w_i rho (c_i . u_w) / c_s^2 (Couette flow Eq. 41).  LBM_BGK with

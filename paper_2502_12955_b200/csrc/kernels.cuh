@@ -43,6 +43,8 @@ struct KP {
     R ws0, ws1;               // scalar-lattice weights
     R G[2][2];
     R G_ads[2];               // fluid-solid adhesion, Eq. 14
+    R psi_wall;               // psi(rho_s) of the solid nodes in Eq. 12 (one component); used when solid_term != 0
+    int solid_term;
     R wall_u[3][2][3];        // velocity of the wall at the low / high face of each axis (moving-wall bounce-back)
     const unsigned char* mask;  // solid-node mask (N bytes, non-zero = solid) or nullptr; read by the WALLS == 2 variants
     R rho0_psi;
@@ -320,6 +322,8 @@ __device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L
                     Fa = -(psi_own[s] * t);
                     // fluid-solid adhesion at bounce-back walls, Eq. 14
                     if constexpr (ADH) Fa = Fa + (-((p.G_ads[s] * m.rho[s]) * adh[a]));
+                    // solid term of Eq. 12, one component: -G psi(x) sum_solid w_i psi(rho_s) c_i
+                    if constexpr (ADH && S == 1) { if (p.solid_term) Fa = Fa + (-((p.G[0][0] * psi_own[0]) * (p.psi_wall * adh[a]))); }
                 }
                 // constant body-force density, split by mass fraction for S = 2 (R5)
                 R Fext;

@@ -68,6 +68,7 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (lattice == LBM_D2Q9 && p->bc[2] != 0) return "2D: bc[2] must be 0";
     if (model != LBM_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) return "rho0_psi must be > 0";
     if (p->w0_scalar < 0.0 || p->w0_scalar >= 1.0) return "w0_scalar must lie in [0, 1)";
+    if (p->rho_wall < 0.0) return "rho_wall must be >= 0";
     if (p->init_kind < LBM_INIT_REST || p->init_kind > LBM_INIT_RANDOM_DROPLETS) return "unknown init_kind";
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
@@ -177,6 +178,11 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
         for (int sd = 0; sd < 2; ++sd)
             for (int b = 0; b < 3; ++b) k.wall_u[a][sd][b] = (R)p.wall_u[a][sd][b];
     k.mask = nullptr;
+    k.solid_term = p.rho_wall > 0.0 ? 1 : 0;
+    {   // psi(rho_s) in the context precision, the same expression as psi_of in the kernels
+        const R rw = (R)p.rho_wall, r0 = (R)p.rho0_psi;
+        k.psi_wall = p.rho_wall > 0.0 ? (p.psi_kind == 1 ? rw : r0 * ((R)1 - std::exp(-(rw / r0)))) : (R)0;
+    }
     k.rho0_psi = (R)p.rho0_psi;
     k.k_react = (R)p.k_react;
 }

@@ -92,6 +92,7 @@ SMALL = [
     ("cfg1", (9, 6, 1), dict(bc=(0, 1, 0), wall_u={(1, 0): (-0.01, 0.0, 0.0), (1, 1): (0.03, 0.0, 0.0)})),
     # Shan-Chen models between bounce-back walls: fluid-only stencil + adhesion force (Eq. 11-12, 14)
     ("cfg2", (33, 17, 1), dict(radius=5.0, bc=(0, 1, 0), G_ads=(-0.4, 0.0))),
+    ("cfg2", (17, 12, 1), dict(radius=4.0, bc=(1, 1, 0), rho_wall=1.2)),
     ("cfg3", (16, 9, 1), dict(bc=(1, 1, 0), G_ads=(-0.2, 0.3), force=(1e-5, -2e-5, 0.0))),
     ("cfg3", (9, 12, 1), dict(bc=(0, 1, 0), G_ads=(0.25, -0.25), forcing=1, tau=(0.8, 1.2))),
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 0, 1), G_ads=(-0.3, 0.3))),
