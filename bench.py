@@ -387,9 +387,13 @@ def main():
 
     import torch
     import paper_2502_12955_b200 as lbm
+    from paper_2502_12955_b200 import build as _build
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
-        from paper_2502_12955_b200 import build as _build
         _build.build()                                        # no-op when liblbm.so is up to date (needs nvcc otherwise)
+    else:
+        t_wait = time.time()
+        while not _build.up_to_date() and time.time() - t_wait < 900:
+            time.sleep(1.0)                                   # rank 0 is building
     lbm.lib()                                                 # fails loudly when liblbm.so is missing
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
