@@ -74,12 +74,29 @@ struct Launch {
                 }
             });
         } else if (model == M_BGK) {
-            ok = with_int<3>(wmode, [&](auto W) {
-                constexpr int w = decltype(W)::value;
-                if (forced == 2) step3<M_BGK, w, true, true>(p, parity, st);
-                else if (forced) step3<M_BGK, w, true>(p, parity, st);
-                else step3<M_BGK, w, false>(p, parity, st);
-            });
+            bool v2 = false;
+            if constexpr (sizeof(R) == 4) {
+                if (forced != 2 && wmode <= 1 && p.bc[0] == 0 && p.nx % 2 == 0 && p.nx >= 64) {
+                    // two cells per thread, vector accesses for the unshifted slots (k_step_v2); 128 threads = 256 cells of a row
+                    int thr = 128;
+                    while (thr > 32 && thr >= p.nx) thr /= 2;
+                    const dim3 g((unsigned)((p.nx / 2 + thr - 1) / thr), (unsigned)p.ny, (unsigned)p.nz);
+                    ok = with_int<2>(wmode, [&](auto W) {
+                        with_int<2>(parity, [&](auto P) {
+                            if (forced) k_step_v2<R, L, decltype(P)::value, decltype(W)::value, true><<<g, thr, 0, st>>>(p);
+                            else k_step_v2<R, L, decltype(P)::value, decltype(W)::value, false><<<g, thr, 0, st>>>(p);
+                        });
+                    });
+                    v2 = true;
+                }
+            }
+            if (!v2)
+                ok = with_int<3>(wmode, [&](auto W) {
+                    constexpr int w = decltype(W)::value;
+                    if (forced == 2) step3<M_BGK, w, true, true>(p, parity, st);
+                    else if (forced) step3<M_BGK, w, true>(p, parity, st);
+                    else step3<M_BGK, w, false>(p, parity, st);
+                });
         } else if (model == M_BGK_T) {
             if (forced == 2) return cudaErrorInvalidValue;
             ok = with_int<3>(wmode, [&](auto W) {

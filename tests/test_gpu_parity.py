@@ -83,6 +83,12 @@ SMALL = [
     ("cfg5", (33, 17, 9), dict(rmin=2.0, rmax=4.0, vol_frac=0.1)),
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7)),
     ("cfg3", (16, 8, 1), dict(precision=32)),
+    # fp32 BGK with an even nx >= 64 and periodic x: the two-cells-per-thread kernel (k_step_v2)
+    ("cfg4", (64, 5, 6), dict(precision=32)),
+    ("cfg4", (258, 4, 3), dict(precision=32, bc=(0, 1, 1), force=(1e-6, 2e-6, -1e-6))),
+    ("cfg4", (130, 6, 5), dict(precision=32, bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.03)),
+    ("cfg1", (260, 9, 1), dict(precision=32)),
+    ("cfg1", (66, 7, 1), dict(precision=32, bc=(0, 1, 0), force=(2e-5, 1e-5, 0.0))),
     # internal-energy lattice (model BGK_T, Eq. 27-30)
     ("cfgT", (9, 6, 7), {}),
     ("cfgT", (33, 5, 4), dict(precision=32, bc=(1, 0, 1))),
