@@ -1057,3 +1057,145 @@ def test_single_component_solid_term_of_eq12():
     psw = 1 - np.exp(-2.0)
     assert np.allclose(Fd[0, 1, 0], -G * psi * (psi - psw) / 6.0, rtol=1e-13)
     assert Fd[0, 1, 0, 0] < 0 < Fd[0, 1, -1, 0]                  # denser wall attracts the fluid (towards y = -1/2 and y = ny - 1/2)
+
+
+# ----------------------------------------------------------------------------------------------
+# Pins added in round 2 for the five terms the round-1 judge could mutate with every pin green.
+# Mutations of oracle/ref_lbm.cpp that each of these must kill (tests/test_oracle_mutations.py applies
+# them to a copy of the oracle and checks that the named test fails):
+#   (i)   body-force split for S = 2 (R5): `force[a] * (rho^s * inv_rho)` -> `force[a]`, or the OTHER
+#         component's mass fraction                      -> test_two_component_body_force_split
+#   (ii)  velocity-dependent half of Eq. 22: F_i -> 3 w_i c_i.F   -> test_guo_term_second_moment
+#   (iii) reflected scalar population at a wall / solid node dropped -> test_scalar_conserved_between_walls_and_around_a_mask
+#   (iv)  phi = (rhoA - rhoB)/(rhoA + rhoB): sign flip    -> test_phi_output
+#   (v)   exp(-rho/rho0) -> exp(-rho) in Eq. 10           -> test_pseudopotential_with_rho0_not_one
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lattice,grid,force,tau", [("D2Q9", (5, 4, 1), (3e-5, -2e-5, 0.0), (0.8, 0.8)),
+                                                    ("D3Q19", (3, 4, 3), (1e-5, 2e-5, -3e-5), (0.7, 1.3))])
+def test_two_component_body_force_split(lattice, grid, force, tau):
+    """S = 2, no interaction (G = 0), uniform densities in a periodic box, uniform body-force density F
+    (gravity "combined with F^SC(sigma)" in Eq. 20-23; reading R5): the components share F by mass
+    fraction, F^sigma = F rho^sigma / rho, so the momentum of component sigma grows by exactly F rho^sigma/rho
+    per cell per step, the total by exactly F (not 2 F), and u^b = F (t + 1/2) / rho (Eq. 20)."""
+    rA, rB = 1.25, 0.5
+    r = RefLBM(*grid, lattice, "SC2", precision=64, tau=tau, psi_kind=1, G=((0, 0), (0, 0)), force=force,
+               init_kind="REST", rho_init=(rA, rB))
+    r.init_from_seed(0)
+    c, _ = lattice_table(lattice)
+    done = 0
+    for t in (0, 1, 6, 33):
+        r.step(t - done)
+        done = t
+        m = r.get_macros()
+        f, _ = r.split_populations(r.get_populations())
+        F = r.get_force()
+        for a in range(r.d):
+            jA = (c[:, a, None] * f[0]).sum(0)
+            jB = (c[:, a, None] * f[1]).sum(0)
+            assert np.allclose(jA, force[a] * t * rA / (rA + rB), rtol=1e-10, atol=1e-19)
+            assert np.allclose(jB, force[a] * t * rB / (rA + rB), rtol=1e-10, atol=1e-19)
+            assert np.allclose(jA + jB, force[a] * t, rtol=1e-10, atol=1e-19)
+            assert np.allclose(m["u"][a], force[a] * (t + 0.5) / (rA + rB), rtol=1e-11, atol=1e-19)
+            assert np.allclose(F[0, a], force[a] * rA / (rA + rB), rtol=1e-13, atol=0)
+            assert np.allclose(F[1, a], force[a] * rB / (rA + rB), rtol=1e-13, atol=0)
+        assert np.abs(m["rho"][0] - rA).max() < 1e-13 and np.abs(m["rho"][1] - rB).max() < 1e-13
+
+
+@pytest.mark.parametrize("lattice,grid,u0,force", [("D2Q9", (4, 3, 1), (0.04, -0.03, 0.0), (2e-3, 1e-3, 0.0)),
+                                                   ("D3Q19", (3, 2, 4), (0.03, 0.02, -0.05), (1e-3, -2e-3, 1.5e-3))])
+def test_guo_term_second_moment(lattice, grid, u0, force):
+    """Uniform (rho, u0) with a uniform force in a periodic box stays uniform, so streaming changes nothing and the
+    second moment P_ab = sum_i c_a c_b f_i obeys the closed recurrence of Eq. 15:
+        P' = P - (P - P_eq)/tau + (1 - 1/(2 tau)) (u_a F_b + F_a u_b),
+    with P_eq = rho u_a u_b + rho c_s^2 delta_ab (second moment of Eq. 6), u = (j + F/2)/rho (Eq. 20)
+    and j(t) = j(0) + t F.  The source term is the second moment of the Guo term Eq. 22:
+    sum_i c_a c_b F_i = u_a F_b + F_a u_b; it comes entirely from the -3 u.F + 9 (c.u)(c.F) part."""
+    tau, rho = 0.83, 1.1
+    d = 3 if lattice == "D3Q19" else 2
+    r = RefLBM(*grid, lattice, "BGK", precision=64, tau=(tau, tau), force=force, init_kind="REST", rho_init=(rho, rho))
+    c, w = lattice_table(lattice)
+    u = np.array(u0[:d])
+    cu = c[:, :d] @ u
+    feq = w * rho * (1 + 3 * cu + 4.5 * cu ** 2 - 1.5 * (u @ u))          # an input state, built from the tables
+    r.set_populations(np.repeat(feq[:, None], r.N, axis=1).ravel())
+    F = np.array(force[:d])
+    P = np.einsum("i,ia,ib->ab", feq, c[:, :d], c[:, :d])
+    j = rho * u
+    for t in range(1, 41):
+        ub = (j + 0.5 * F) / rho
+        Peq = rho * np.outer(ub, ub) + rho / 3.0 * np.eye(d)
+        P = P - (P - Peq) / tau + (1 - 0.5 / tau) * (np.outer(ub, F) + np.outer(F, ub))
+        j = j + F
+        r.step(1)
+        f, _ = r.split_populations(r.get_populations())
+        Pn = np.einsum("in,ia,ib->abn", f[0], c[:, :d], c[:, :d])
+        assert np.abs(Pn - P[:, :, None]).max() < 1e-14, t
+    # the source is not negligible at this tolerance: without it P would be off by ~ t u F
+    assert np.abs(np.outer(u, F)).max() * 40 > 1e-4
+
+
+@pytest.mark.parametrize("lattice,grid,bc,masked", [("D2Q9", (10, 9, 1), (0, 1, 0), False), ("D2Q9", (9, 8, 1), (1, 1, 0), True),
+                                                    ("D3Q19", (6, 5, 7), (0, 0, 1), False), ("D3Q19", (6, 6, 5), (0, 1, 0), True)])
+def test_scalar_conserved_between_walls_and_around_a_mask(lattice, grid, bc, masked):
+    """k = 0: the scalar lattice only relaxes and streams (Eq. 34), and walls / solid nodes reflect
+    every population that would leave ("simple Bounce Back"), so sum_x C is invariant to round-off
+    although C is advected by a non-trivial demixing flow."""
+    r = noise_cfg("SC2_ADE", lattice, grid, bc=bc, tau=(0.9, 1.1), k_react=0.0, init_kind="DROPLET", rho_in=1.3,
+                  rho_out=0.5, radius=2.5, width=2.0, c_init=0.7, noise_amp=0.02, G_ads=(-0.1, 0.1))
+    solid = np.zeros(r.N, bool)
+    if masked:
+        rng = np.random.default_rng(4)
+        solid = rng.random(r.N) < 0.15
+        r.set_mask(solid.astype(np.uint8))
+    r.init_from_seed(9)
+    C0 = r.get_macros()["C"]
+    assert C0[~solid].max() - C0[~solid].min() > 0.3             # a non-uniform scalar field
+    tot0 = C0[~solid].sum()
+    for _ in range(4):
+        r.step(60)
+        m = r.get_macros()
+        assert abs(m["C"][~solid].sum() - tot0) <= 1e-13 * tot0
+    assert np.abs(m["u"]).max() > 1e-4                           # ... carried by a flow that is not at rest
+    assert np.abs(m["C"] - C0)[~solid].max() > 1e-3
+
+
+def test_phi_output():
+    """lbm_get_macros' phi: S = 2 -> (rhoA - rhoB)/(rhoA + rhoB) (order parameter of the two-component runs,
+    PAPER.md:584-676), sign and value on a hand-built two-cell state; S = 1 -> psi(rho) of Eq. 10."""
+    c, w = lattice_table("D2Q9")
+    r = RefLBM(2, 1, 1, "D2Q9", "SC2", precision=64, tau=(1.0, 1.0), psi_kind=1, G=((0, 0), (0, 0)))
+    rA, rB = np.array([1.5, 0.2]), np.array([0.5, 1.0])
+    r.set_populations(np.concatenate([np.outer(w, rA).ravel(), np.outer(w, rB).ravel()]))
+    m = r.get_macros()
+    assert np.allclose(m["phi"], [0.5, -2.0 / 3.0], rtol=1e-15, atol=0)
+    assert np.allclose(m["rho"], [rA, rB], rtol=1e-15)
+    r1 = RefLBM(2, 1, 1, "D2Q9", "SC1", precision=64, tau=(1.0, 1.0), psi_kind=0, rho0_psi=1.0, G=((0, 0), (0, 0)))
+    r1.set_populations(np.outer(w, rA).ravel())
+    assert np.allclose(r1.get_macros()["phi"], 1.0 - np.exp(-rA), rtol=1e-15, atol=0)
+
+
+def test_pseudopotential_with_rho0_not_one():
+    """Eq. 10 (PAPER.md:122): psi = rho0 (1 - exp(-rho/rho0)); psi -> rho for rho << rho0 and psi -> rho0 for
+    rho >> rho0.  rho0 = 2: values through the phi output, and the force against the literal pair
+    sum of Eq. 9 with that psi."""
+    c, w = lattice_table("D2Q9")
+    rho0 = 2.0
+    nx, ny = 6, 5
+    r = RefLBM(nx, ny, 1, "D2Q9", "SC1", precision=64, tau=(1.0, 1.0), psi_kind=0, rho0_psi=rho0, G=((-3.0, 0), (0, 0)))
+    rng = np.random.default_rng(2)
+    rho = rng.uniform(0.2, 3.0, nx * ny)
+    rho[0], rho[1] = 1e-6, 80.0
+    r.set_populations(np.outer(w, rho).ravel())
+    psi = r.get_macros()["phi"]
+    assert np.allclose(psi, rho0 * (1 - np.exp(-rho / rho0)), rtol=1e-14, atol=1e-15)   # 1 - exp cancels for tiny rho
+    assert abs(psi[0] / 1e-6 - 1) < 1e-6 and abs(psi[1] - rho0) < 1e-15
+    F = r.get_force().reshape(2, ny, nx)
+    P = (rho0 * (1 - np.exp(-rho / rho0))).reshape(ny, nx)
+    Fb = np.zeros((2, ny, nx))
+    for y in range(ny):
+        for x in range(nx):
+            for i in range(1, 9):
+                # Eq. 11 (PAPER.md:128): F = -G psi(x) sum_i w_i psi(x + c_i) c_i, G = -3
+                Fb[:, y, x] += 3.0 * P[y, x] * w[i] * P[(y + c[i][1]) % ny, (x + c[i][0]) % nx] * c[i][:2]
+    assert np.abs(F - Fb).max() < 1e-13 * np.abs(Fb).max()
+    assert np.abs(Fb).max() > 0.1
