@@ -20,11 +20,13 @@
  *   closed forms; equilibrium moments; rotation equivariance; lattice tables
  *   against tests/golden/.  Nothing in this file is "parity unpinned".
  *
- * Arithmetic: every operation below is a single IEEE-754 add, sub, mul, div or
- * sqrt in the context precision R (float or double), evaluated left to right
- * exactly as parenthesised; build with -ffp-contract=off so no FMA is formed.
- * Constants are formed in double from the double parameters and rounded once
- * to R (DESIGN "Arithmetic").
+ * Arithmetic ("explicit-FMA specification"): every operation
+ * below is a single IEEE-754 add, sub, mul, div or fused multiply-add in the
+ * context precision R (float or double), evaluated exactly as parenthesised.
+ * A product that feeds a sum is fused into it where -- and only where -- the code
+ * says std::fma (one rounding for a*b + c); build with -ffp-contract=off so the
+ * compiler forms no other FMA.  Constants are formed in double from the double
+ * parameters and rounded once to R.
  */
 #include "ref_lbm.h"
 
@@ -148,7 +150,9 @@ struct Sim : ref_ctx {
 
     /* constants, rounded once to R */
     R w[19], ws[7];
-    R omega[2], cf[2], tau_r[2], omega_c, inv_cs2g;
+    R omega[2], tau_r[2], omega_c, inv_cs2g;
+    R cfw[2][19];          /* (1 - 1/(2 tau^s)) w_i: prefactor of the Guo term in Eq. 15 */
+    R w6[19];              /* 6 w_i = 2 w_i / c_s^2: moving-wall bounce-back (DESIGN R24) */
     R G[2][2], G_ads[2], rho0_psi, force[3], k_react;
     R wall_u[3][2][3];
     R psi_wall;            /* psi(rho_s) of Eq. 12 (single component), 0 when rho_wall = 0 */
@@ -187,13 +191,13 @@ struct Sim : ref_ctx {
         has_thermal = (model == REF_BGK_T);
         d = L.d; Q = L.Q; Qs = Ls.Q;
         N = (size_t)nx * ny * nz;
-        for (int i = 0; i < Q; ++i) w[i] = (R)L.w[i];
+        for (int i = 0; i < Q; ++i) { w[i] = (R)L.w[i]; w6[i] = (R)(6.0 * L.w[i]); }
         for (int i = 0; i < Qs; ++i) ws[i] = (R)Ls.w[i];
         for (int s = 0; s < 2; ++s) {
             omega[s] = (R)(1.0 / pp.tau[s]);              /* 1/tau, Eq. 15 */
             tau_r[s] = (R)pp.tau[s];
             G_ads[s] = (R)pp.G_ads[s];
-            cf[s] = (R)(1.0 - 0.5 / pp.tau[s]);           /* 1 - 1/(2 tau), Eq. 15 */
+            for (int i = 0; i < Q; ++i) cfw[s][i] = (R)((1.0 - 0.5 / pp.tau[s]) * L.w[i]);   /* (1 - 1/(2 tau)) w_i, Eq. 15 */
             for (int t = 0; t < 2; ++t) G[s][t] = (R)pp.G[s][t];
         }
         omega_c = (R)(1.0 / pp.tau_c);                     /* Eq. 34 */
@@ -246,14 +250,17 @@ struct Sim : ref_ctx {
         return rho0_psi * ((R)1 - std::exp(-(r / rho0_psi)));
     }
 
-    /* Eq. 6 with c_s^2 = 1/3: w rho (1 + 3 cu + 4.5 cu^2 - 1.5 u.u) */
-    R feq(int i, R rho_s, const R* u) const {
-        R usq = (R)0, cu = (R)0;
-        for (int a = 0; a < d; ++a) usq = usq + u[a] * u[a];
-        for (int a = 0; a < d; ++a) cu = cu + (R)L.c[i][a] * u[a];
-        R base = (R)1 - (R)1.5 * usq;
-        return (w[i] * rho_s) * ((base + (R)3 * cu) + ((R)4.5 * cu) * cu);
+    /* Eq. 6 with c_s^2 = 1/3: f_i^eq = (w_i rho) e_i, e_i = 1 + 3 cu + 4.5 cu^2 - 1.5 u.u,
+     * evaluated as fma(3, cu, fma(4.5 cu, cu, fma(-1.5, u.u, 1))) */
+    R eq_poly(int i, const R* u) const {
+        R usq = u[0] * u[0];
+        for (int a = 1; a < d; ++a) usq = std::fma(u[a], u[a], usq);
+        R cu = (R)0;
+        for (int a = 0; a < d; ++a) cu = cu + (R)L.c[i][a] * u[a];      /* c = -1, 0, +1: exact products */
+        R base = std::fma((R)-1.5, usq, (R)1);
+        return std::fma((R)3, cu, std::fma((R)4.5 * cu, cu, base));
     }
+    R feq(int i, R rho_s, const R* u) const { return (w[i] * rho_s) * eq_poly(i, u); }
 
     /* ---- steps 1-4 of one update: moments, psi, force, barycentric velocity ---- */
     void moments_and_force() {
@@ -295,8 +302,8 @@ struct Sim : ref_ctx {
                                 size_t nb;
                                 /* Eq. 11 / 12 sum over FLUID neighbours only: a node beyond a wall is solid */
                                 if (!neighbour(x, y, z, L.c[i], nb)) continue;
-                                R wp = w[i] * psi[(size_t)t * N + nb];
-                                for (int a = 0; a < d; ++a) acc[t][a] = acc[t][a] + wp * (R)L.c[i][a];
+                                for (int a = 0; a < d; ++a)      /* (w_i c_ia) is +-w_i or 0: exact */
+                                    acc[t][a] = std::fma(w[i] * (R)L.c[i][a], psi[(size_t)t * N + nb], acc[t][a]);
                             }
                         if (has_walls || has_mask)
                             for (int i = 1; i < Q; ++i) {
@@ -307,20 +314,20 @@ struct Sim : ref_ctx {
                     }
                     for (int s = 0; s < S; ++s)
                         for (int a = 0; a < 3; ++a) {
-                            R Fa = (R)0;
+                            /* constant body-force density; split by mass fraction for S=2 (DESIGN R5) */
+                            R Fa = (S == 1) ? force[a] : force[a] * (rho[(size_t)s * N + cell] * inv_rho);
+                            if (a >= d) Fa = (R)0;
                             if (has_sc && a < d) {
+                                /* Eq. 11 / 13: - psi^s(x) sum_t G_st acc^t */
                                 R t = G[s][0] * acc[0][a];
-                                if (S == 2) t = t + G[s][1] * acc[1][a];
-                                Fa = -(psi[(size_t)s * N + cell] * t);
+                                if (S == 2) t = std::fma(G[s][1], acc[1][a], t);
+                                Fa = std::fma(-psi[(size_t)s * N + cell], t, Fa);
                                 /* fluid-solid adhesion, Eq. 14: -G_ads rho^s sum_i w_i s c_i */
-                                if (has_walls || has_mask) Fa = Fa + (-((G_ads[s] * rho[(size_t)s * N + cell]) * adh[a]));
+                                if (has_walls || has_mask) Fa = std::fma(-(G_ads[s] * rho[(size_t)s * N + cell]), adh[a], Fa);
                                 /* solid term of Eq. 12, one component: -G psi(x) sum_solid w_i psi(rho_s) c_i */
                                 if ((has_walls || has_mask) && S == 1 && p.rho_wall > 0.0)
-                                    Fa = Fa + (-((G[0][0] * psi[cell]) * (psi_wall * adh[a])));
+                                    Fa = std::fma(-(G[0][0] * psi[cell]), psi_wall * adh[a], Fa);
                             }
-                            /* constant body-force density; split by mass fraction for S=2 (DESIGN R5) */
-                            R Fext = (S == 1) ? force[a] : force[a] * (rho[(size_t)s * N + cell] * inv_rho);
-                            if (a < d) Fa = Fa + Fext;
                             Fv[((size_t)s * 3 + a) * N + cell] = Fa;
                         }
                     /* 4. u^b = (1/rho) sum_sigma [ j^sigma + F^sigma/2 ], Eq. 20-21 */
@@ -330,22 +337,22 @@ struct Sim : ref_ctx {
                             jt = jt + jm[((size_t)s * 3 + a) * N + cell];
                             Ft = Ft + Fv[((size_t)s * 3 + a) * N + cell];
                         }
-                        ub[(size_t)a * N + cell] = (jt + (R)0.5 * Ft) * inv_rho;
+                        ub[(size_t)a * N + cell] = std::fma((R)0.5, Ft, jt) * inv_rho;
                     }
                     /* Shan-Chen (velocity-shift) forcing scheme, p.forcing == 1: common velocity
                      * u' = sum_s (j^s / tau^s) / sum_s (rho^s / tau^s), Eq. 17, and
                      * u^eq,s = u' + tau^s F^s / rho^s, Eq. 16; rho^s u^s = j^s, Eq. 18 */
                     if (p.forcing == 1) {
                         R den = rho[cell] * omega[0];
-                        for (int s = 1; s < S; ++s) den = den + rho[(size_t)s * N + cell] * omega[s];
+                        for (int s = 1; s < S; ++s) den = std::fma(rho[(size_t)s * N + cell], omega[s], den);
                         R inv_den = (R)1 / den;
                         for (int a = 0; a < 3; ++a) {
                             R num = jm[(size_t)a * N + cell] * omega[0];
-                            for (int s = 1; s < S; ++s) num = num + jm[((size_t)s * 3 + a) * N + cell] * omega[s];
+                            for (int s = 1; s < S; ++s) num = std::fma(jm[((size_t)s * 3 + a) * N + cell], omega[s], num);
                             R up = num * inv_den;
                             for (int s = 0; s < S; ++s) {
                                 R inv_rs = (R)1 / rho[(size_t)s * N + cell];
-                                ueq[((size_t)s * 3 + a) * N + cell] = up + (tau_r[s] * Fv[((size_t)s * 3 + a) * N + cell]) * inv_rs;
+                                ueq[((size_t)s * 3 + a) * N + cell] = std::fma(tau_r[s] * Fv[((size_t)s * 3 + a) * N + cell], inv_rs, up);
                             }
                         }
                     }
@@ -371,8 +378,9 @@ struct Sim : ref_ctx {
                     for (int s = 0; s < S; ++s) {
                         R Fs[3] = {Fv[((size_t)s * 3 + 0) * N + cell], Fv[((size_t)s * 3 + 1) * N + cell],
                                    Fv[((size_t)s * 3 + 2) * N + cell]};
-                        R uF = (R)0;
-                        for (int a = 0; a < d; ++a) uF = uF + u[a] * Fs[a];
+                        R uF = u[0] * Fs[0];
+                        for (int a = 1; a < d; ++a) uF = std::fma(u[a], Fs[a], uF);
+                        R m3uF = (R)-3 * uF;
                         R rho_s = rho[(size_t)s * N + cell];
                         /* velocity-shift scheme: equilibrium at u^eq,s, no forcing term F_i */
                         R us[3] = {u[0], u[1], u[2]};
@@ -380,14 +388,19 @@ struct Sim : ref_ctx {
                             for (int a = 0; a < 3; ++a) us[a] = ueq[((size_t)s * 3 + a) * N + cell];
                         for (int i = 0; i < Q; ++i) {
                             R fi = F_(f, s, i, cell);
-                            R fe = feq(i, rho_s, us);
-                            R cu = (R)0, cF = (R)0;
-                            for (int a = 0; a < d; ++a) cu = cu + (R)L.c[i][a] * u[a];
-                            for (int a = 0; a < d; ++a) cF = cF + (R)L.c[i][a] * Fs[a];
-                            /* F_i = w_i [ (c_i - u).F / c_s^2 + (c_i.u)(c_i.F) / c_s^4 ], Eq. 22 */
-                            R Fi = w[i] * ((R)3 * (cF - uF) + ((R)9 * cu) * cF);
-                            R fstar = (fi - omega[s] * (fi - fe)) + cf[s] * Fi;
-                            if (p.forcing == 1) fstar = fi - omega[s] * (fi - fe);
+                            /* f_i - f_i^eq with one rounding: f^eq = (w_i rho^s) e_i, Eq. 6 */
+                            R dneq = std::fma(-(w[i] * rho_s), eq_poly(i, us), fi);
+                            /* f_i - (f_i - f_i^eq)/tau, Eq. 15 */
+                            R fstar = std::fma(-omega[s], dneq, fi);
+                            if (p.forcing == 0) {
+                                R cu = (R)0, cF = (R)0;
+                                for (int a = 0; a < d; ++a) cu = cu + (R)L.c[i][a] * u[a];
+                                for (int a = 0; a < d; ++a) cF = cF + (R)L.c[i][a] * Fs[a];
+                                /* F_i / w_i = 3 (c_i.F - u.F) + 9 (c_i.u)(c_i.F), Eq. 22 with c_s^2 = 1/3 */
+                                R Fi = std::fma((R)3, cF, std::fma((R)9 * cu, cF, m3uF));
+                                /* + (1 - 1/(2 tau)) F_i, Eq. 15 */
+                                fstar = std::fma(cfw[s][i], Fi, fstar);
+                            }
                             /* 7. stream, Eq. 5; halfway bounce-back at walls */
                             size_t nb;
                             if (neighbour(x, y, z, L.c[i], nb)) F_(fnew, s, i, nb) = fstar;
@@ -399,7 +412,7 @@ struct Sim : ref_ctx {
                                     const R* uw = wall_velocity(x, y, z, L.c[i]);
                                     R cuw = (R)0;
                                     for (int a = 0; a < d; ++a) cuw = cuw + (R)L.c[i][a] * uw[a];
-                                    fstar = fstar - (((R)6 * w[i]) * rho_s) * cuw;
+                                    fstar = std::fma(-(w6[i] * rho_s), cuw, fstar);
                                 }
                                 F_(fnew, s, L.opp[i], cell) = fstar;
                             }
@@ -412,8 +425,7 @@ struct Sim : ref_ctx {
                         for (int i = 0; i < Q; ++i) E = E + H_(g, i, cell);
                         for (int i = 0; i < Q; ++i) {
                             R gi = H_(g, i, cell);
-                            R ge = feq(i, E, u);
-                            R gstar = gi - omega_c * (gi - ge);
+                            R gstar = std::fma(-omega_c, std::fma(-(w[i] * E), eq_poly(i, u), gi), gi);
                             size_t nb;
                             if (neighbour(x, y, z, L.c[i], nb)) H_(gnew, i, nb) = gstar;
                             else H_(gnew, L.opp[i], cell) = gstar;     /* adiabatic wall: plain reflection */
@@ -431,8 +443,9 @@ struct Sim : ref_ctx {
                             R hi = H_(h, i, cell);
                             R cu = (R)0;
                             for (int a = 0; a < d; ++a) cu = cu + (R)Ls.c[i][a] * u[a];
-                            R he = (ws[i] * C) * ((R)1 + inv_cs2g * cu);
-                            R hstar = (hi - omega_c * (hi - he)) + ws[i] * Rsrc;
+                            /* h_i - h_i^eq, h^eq = (w_i C)(1 + c_i.u / c_sg^2), Eq. 35; relaxation Eq. 34; source w_i R (R8) */
+                            R dneq = std::fma(-(ws[i] * C), std::fma(inv_cs2g, cu, (R)1), hi);
+                            R hstar = std::fma(ws[i], Rsrc, std::fma(-omega_c, dneq, hi));
                             size_t nb;
                             if (neighbour(x, y, z, Ls.c[i], nb)) H_(hnew, i, nb) = hstar;
                             else H_(hnew, Ls.opp[i], cell) = hstar;
@@ -556,7 +569,7 @@ struct Sim : ref_ctx {
                         for (int i = 0; i < Qs; ++i) {
                             R cu = (R)0;
                             for (int a = 0; a < d; ++a) cu = cu + (R)Ls.c[i][a] * u[a];
-                            H_(h, i, cell) = (ws[i] * (R)c0) * ((R)1 + inv_cs2g * cu);
+                            H_(h, i, cell) = (ws[i] * (R)c0) * std::fma(inv_cs2g, cu, (R)1);
                         }
                     if (has_thermal)      /* g_i = g^eq(rho eps, u), eps = c_init */
                         for (int i = 0; i < Q; ++i) H_(g, i, cell) = feq(i, (R)r0[0] * (R)c0, u);
