@@ -83,8 +83,8 @@ struct Launch {
                     const dim3 g((unsigned)((p.nx / 2 + thr - 1) / thr), (unsigned)p.ny, (unsigned)p.nz);
                     ok = with_int<2>(wmode, [&](auto W) {
                         with_int<2>(parity, [&](auto P) {
-                            if (forced) k_step_v2<R, L, decltype(P)::value, decltype(W)::value, true><<<g, thr, 0, st>>>(p);
-                            else k_step_v2<R, L, decltype(P)::value, decltype(W)::value, false><<<g, thr, 0, st>>>(p);
+                            if (forced) k_step_v2<L, decltype(P)::value, decltype(W)::value, true><<<g, thr, 0, st>>>(p);
+                            else k_step_v2<L, decltype(P)::value, decltype(W)::value, false><<<g, thr, 0, st>>>(p);
                         });
                     });
                     v2 = true;

@@ -13,14 +13,16 @@
 // read, slot sets of different cells are disjoint, so a step needs no barrier and no second copy.
 // Eq. 5 and halfway bounce-back are both encoded in P_i.
 //
-// Arithmetic: every floating-point operation is a single IEEE-754 add/sub/mul/div in the context
-// precision R, in the order written (the files are compiled with --fmad=false, default
-// -prec-div=true); DESIGN.md "Arithmetic" lists the expression tree.
+// Arithmetic: the explicit-FMA expression tree of DESIGN.md section 5.  Every operation is a single IEEE-754
+// add/sub/mul/div or, where the code says vfma, ONE fused multiply-add, in the context precision (the files are
+// compiled with --fmad=false, default -prec-div=true, so nvcc forms no other FMA).  The per-cell code is generic in
+// the value type V (vec.cuh): a scalar per thread, or two fp32 cells per thread in packed f32x2 instructions.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "lattice.cuh"
+#include "vec.cuh"
 
 namespace lbm {
 
@@ -37,7 +39,8 @@ struct KP {
     int nx, ny, nz, N;
     int bc[3];
     int psi_kind;
-    R omega[2], cf[2];        // 1/tau, 1 - 1/(2 tau): Eq. 15
+    R omega[2];               // 1/tau: Eq. 15
+    R cfw[2][3];              // (1 - 1/(2 tau)) w_i per weight class (rest, axis, diagonal): prefactor of the Guo term, Eq. 15
     R tau[2];                 // tau itself (velocity-shift forcing, Eq. 16)
     R omega_c, inv_cs2g;      // 1/tau_c (Eq. 34), 1/c_{s,g}^2 = d/(1-w0) (Eq. 35, R6)
     R ws0, ws1;               // scalar-lattice weights
@@ -168,21 +171,29 @@ __device__ __forceinline__ R* slot_of(R* base, const NB& nb, size_t N) {
     }
 }
 
-// sum_a c_{I,a} v_a in axis order, skipping the zero components (adding +-0 changes nothing)
-template <class L, int I, class R>
-__device__ __forceinline__ R dotc(const R* v) {
-    constexpr int c0 = L::c(I, 0), c1 = L::c(I, 1), c2 = L::c(I, 2);
-    R r = (R)0;
-    if constexpr (c0 != 0) r = c0 > 0 ? v[0] : -v[0];
-    if constexpr (c1 != 0) {
-        if constexpr (c0 == 0) r = c1 > 0 ? v[1] : -v[1];
-        else r = c1 > 0 ? r + v[1] : r - v[1];
+// sum_a c_{I,a} v_a in axis order, skipping the zero components (adding +-0 changes nothing).  (-x) + y is written
+// y - x and (-x) - y as -(x + y): the same bits (negation is exact, addition commutes), one instruction less.
+template <class L, int I, class V>
+__device__ __forceinline__ V dotc(const V* v) {
+    constexpr int c0 = L::c(I, 0), c1 = L::c(I, 1), c2 = L::D == 3 ? L::c(I, 2) : 0;
+    constexpr int nnz = (c0 != 0) + (c1 != 0) + (c2 != 0);
+    static_assert(nnz <= 2, "lattice velocities with at most two non-zero components");
+    if constexpr (nnz == 0) {
+        return vconst<V>(0.0);
+    } else {
+        constexpr int a = c0 != 0 ? 0 : (c1 != 0 ? 1 : 2);
+        constexpr int sa = a == 0 ? c0 : (a == 1 ? c1 : c2);
+        if constexpr (nnz == 1) {
+            if constexpr (sa > 0) return v[a]; else return -v[a];
+        } else {
+            constexpr int b = (a == 0 && c1 != 0) ? 1 : 2;
+            constexpr int sb = b == 1 ? c1 : c2;
+            if constexpr (sa > 0 && sb > 0) return v[a] + v[b];
+            else if constexpr (sa > 0) return v[a] - v[b];
+            else if constexpr (sb > 0) return v[b] - v[a];
+            else return -(v[a] + v[b]);
+        }
     }
-    if constexpr (L::D == 3 && c2 != 0) {
-        if constexpr (c0 == 0 && c1 == 0) r = c2 > 0 ? v[2] : -v[2];
-        else r = c2 > 0 ? r + v[2] : r - v[2];
-    }
-    return r;
 }
 
 template <class L>
@@ -209,13 +220,6 @@ __device__ __forceinline__ void moments(const R* fl, R& rho, R* j) {
     });
 }
 
-// Eq. 10 / 24 or psi = rho (R3)
-template <class R>
-__device__ __forceinline__ R psi_of(R rho, int kind, R rho0) {
-    if (kind == 1) return rho;
-    return rho0 * ((R)1 - exp(-(rho / rho0)));
-}
-
 template <class L, int PARITY, int WALLS, class R, class NB>
 __device__ __forceinline__ void load_pops(R* __restrict__ base, const NB& nb, size_t N, R* fl) {
     static_for<0, L::Q>([&](auto ic) {
@@ -240,6 +244,7 @@ __device__ __forceinline__ R load_psi(const R* q) {
     if constexpr (COH) return __ldcg(q); else return __ldg(q);
 }
 
+// acc[t][a] = fma(c_{i,a} w_i, psi^t(x + c_i), acc[t][a]) in index order from zero (row a3).
 // Neighbours beyond a bounce-back wall are solid nodes: they are left out of the sum (Eq. 11-12: sum over FLUID
 // neighbours; adding an exact zero instead of skipping changes no bit).
 template <class L, int S, bool COH, class R, class NB>
@@ -251,15 +256,12 @@ __device__ __forceinline__ void sc_stencil(const R* __restrict__ psi, const NB& 
         static_for<1, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-            R wp = (R)L::w(i) * load_psi<COH>(ps + ((unsigned)nb.template row<CY, CZ>() + (unsigned)nb.template col<CX>()));
-            if (nb.template outside<CX, CY, CZ>()) wp = (R)0;
+            R pv = load_psi<COH>(ps + ((unsigned)nb.template row<CY, CZ>() + (unsigned)nb.template col<CX>()));
+            if (nb.template outside<CX, CY, CZ>()) pv = (R)0;       // fma(w, 0, acc) = acc: the term is left out
             static_for<0, L::D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
                 constexpr int c = L::c(i, a);
-                if constexpr (c != 0) {
-                    if constexpr (first_nonzero<L>(i, a)) acc[t][a] = c > 0 ? wp : -wp;
-                    else acc[t][a] = c > 0 ? acc[t][a] + wp : acc[t][a] - wp;
-                }
+                if constexpr (c != 0) acc[t][a] = vfma((R)(c * L::w(i)), pv, acc[t][a]);
             });
         });
     });
@@ -294,53 +296,56 @@ struct CellMacro {
     R inv_rho;
 };
 
-// steps a1, a3 (given the stencil sums), a4: moments, force, barycentric velocity.
+// steps a1, a3 (given the stencil sums), a4: moments, force, barycentric velocity (rows a1-a4).
 // acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a} and psi_own[s] = psi^s(x) are read only for Shan-Chen models.
-template <class R, class L, int MODEL, bool FORCED, bool ADH = false>
-__device__ __forceinline__ void cell_macros_core(const KP<R>& p, const R (*fl)[L::Q], const R (*acc)[3], const R* psi_own,
-                                                 CellMacro<R, L, MODEL>& m, const R* adh = nullptr) {
+// V: value type (scalar, or two fp32 cells), T: its scalar type.
+template <class V, class L, int MODEL, bool FORCED, bool ADH = false, class T>
+__device__ __forceinline__ void cell_macros_core(const KP<T>& p, const V (*fl)[L::Q], const V (*acc)[3], const V* psi_own,
+                                                 CellMacro<V, L, MODEL>& m, const V* adh = nullptr) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
-    R (&j)[S][3] = m.j;
+    V (&j)[S][3] = m.j;
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
-        j[s][0] = j[s][1] = j[s][2] = (R)0;
+        j[s][0] = j[s][1] = j[s][2] = vconst<V>(0.0);
         moments<L>(fl[s], m.rho[s], j[s]);
     });
-    R rho_t = m.rho[0];
+    V rho_t = m.rho[0];
     if constexpr (S == 2) rho_t = rho_t + m.rho[1];
-    m.inv_rho = (R)1 / rho_t;
+    m.inv_rho = vrecip(rho_t);
     if constexpr (FORCED) {
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
             static_for<0, D>([&](auto ac) {
                 constexpr int a = decltype(ac)::value;
-                R Fa = (R)0;
-                if constexpr (SC) {
-                    R t = p.G[s][0] * acc[0][a];
-                    if constexpr (S == 2) t = t + p.G[s][1] * acc[1][a];
-                    Fa = -(psi_own[s] * t);
-                    // fluid-solid adhesion at bounce-back walls, Eq. 14 (PAPER.md:141)
-                    if constexpr (ADH) Fa = Fa + (-((p.G_ads[s] * m.rho[s]) * adh[a]));
-                    // solid term of Eq. 12 (PAPER.md:132), one component: -G psi(x) sum_solid w_i psi(rho_s) c_i
-                    if constexpr (ADH && S == 1) { if (p.solid_term) Fa = Fa + (-((p.G[0][0] * psi_own[0]) * (p.psi_wall * adh[a]))); }
-                }
                 // constant body-force density, split by mass fraction for S = 2 (R5)
-                R Fext;
-                if constexpr (S == 1) Fext = p.force[a]; else Fext = p.force[a] * (m.rho[s] * m.inv_rho);
-                m.F[s][a] = Fa + Fext;
+                V Fa = vbcast<V>(p.force[a]);
+                if constexpr (S == 2) Fa = Fa * (m.rho[s] * m.inv_rho);
+                if constexpr (SC) {
+                    // Eq. 11 / 13: - psi^s(x) sum_t G_st acc^t
+                    V t = vbcast<V>(p.G[s][0]) * acc[0][a];
+                    if constexpr (S == 2) t = vfma(vbcast<V>(p.G[s][1]), acc[1][a], t);
+                    Fa = vfma(-psi_own[s], t, Fa);
+                    // fluid-solid adhesion at bounce-back walls, Eq. 14 (PAPER.md:141)
+                    if constexpr (ADH) Fa = vfma(-(vbcast<V>(p.G_ads[s]) * m.rho[s]), adh[a], Fa);
+                    // solid term of Eq. 12 (PAPER.md:132), one component: -G psi(x) sum_solid w_i psi(rho_s) c_i
+                    if constexpr (ADH && S == 1) {
+                        if (p.solid_term) Fa = vfma(-(vbcast<V>(p.G[0][0]) * psi_own[0]), vbcast<V>(p.psi_wall) * adh[a], Fa);
+                    }
+                }
+                m.F[s][a] = Fa;
             });
         });
     }
     // u^b = (1/rho) sum_sigma [ j^sigma + F^sigma / 2 ]: Eq. 20-21
     static_for<0, D>([&](auto ac) {
         constexpr int a = decltype(ac)::value;
-        R jt = j[0][a];
+        V jt = j[0][a];
         if constexpr (S == 2) jt = jt + j[1][a];
         if constexpr (FORCED) {
-            R Ft = m.F[0][a];
+            V Ft = m.F[0][a];
             if constexpr (S == 2) Ft = Ft + m.F[1][a];
-            m.u[a] = (jt + (R)0.5 * Ft) * m.inv_rho;
+            m.u[a] = vfma(vconst<V>(0.5), Ft, jt) * m.inv_rho;
         } else {
             m.u[a] = jt * m.inv_rho;
         }
@@ -366,28 +371,31 @@ __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const 
     cell_macros_core<R, L, MODEL, FORCED, ADH>(p, fl, acc, psi_own, m, adh);
 }
 
-// step a5 for one component: f* = f - (f - f^eq)/tau + (1 - 1/(2 tau)) F_i
-// Eq. 15, Eq. 6 with c_s^2 = 1/3, Eq. 22.
-// Opposite directions share c.u, c.F and the even terms (exactly: negation is exact).
-template <class R, class L, bool FORCED>
-__device__ __forceinline__ void collide(R* fl, R rho_s, const R* u, const R* Fs, R omega, R cfs) {
+// step a5 for one component: e_i = fma(3, cu, fma(4.5 cu, cu, base)), f^eq = (w rho) e_i (Eq. 6,
+// PAPER.md:95, c_s^2 = 1/3); d = fma(-(w rho), e_i, f) = f - f^eq; f* = fma(-omega, d, f) (Eq. 15);
+// Guo term (Eq. 22): Phi_i = fma(3, cF, fma(9 cu, cF, -3 u.F)), f* = fma((1 - 1/(2 tau)) w_i, Phi_i, f*).
+// Opposite directions share cu, cF and the even terms (exactly: negation is exact).
+// nomega = -1/tau; cfw[k] = (1 - 1/(2 tau)) w of weight class k (read only when FORCED).
+template <class V, class L, bool FORCED>
+__device__ __forceinline__ void collide(V* fl, V rho_s, const V* u, const V* Fs, V nomega, const V* cfw) {
     constexpr int D = L::D;
-    R usq = u[0] * u[0];
-    usq = usq + u[1] * u[1];
-    if constexpr (D == 3) usq = usq + u[2] * u[2];
-    const R base = (R)1 - (R)1.5 * usq;
-    R uF = (R)0;
+    V usq = u[0] * u[0];
+    usq = vfma(u[1], u[1], usq);
+    if constexpr (D == 3) usq = vfma(u[2], u[2], usq);
+    const V base = vfma(vconst<V>(-1.5), usq, vconst<V>(1.0));
+    V m3uF = vconst<V>(0.0);
     if constexpr (FORCED) {
-        uF = u[0] * Fs[0];
-        uF = uF + u[1] * Fs[1];
-        if constexpr (D == 3) uF = uF + u[2] * Fs[2];
+        V uF = u[0] * Fs[0];
+        uF = vfma(u[1], Fs[1], uF);
+        if constexpr (D == 3) uF = vfma(u[2], Fs[2], uF);
+        m3uF = vconst<V>(-3.0) * uF;
     }
-    const R W[3] = {(R)L::w(0), (R)L::w(1), (R)L::w(L::Q - 1)};
-    const R wr[3] = {W[0] * rho_s, W[1] * rho_s, W[2] * rho_s};
-    {   // rest population: c = 0
-        const R fe = wr[0] * base;
-        R fs = fl[0] - omega * (fl[0] - fe);
-        if constexpr (FORCED) fs = fs + cfs * (W[0] * ((R)3 * (-uF)));
+    // -(w rho) per weight class
+    const V nwr[3] = {vconst<V>(-L::w(0)) * rho_s, vconst<V>(-L::w(1)) * rho_s, vconst<V>(-L::w(L::Q - 1)) * rho_s};
+    const V c3 = vconst<V>(3.0), cm3 = vconst<V>(-3.0);
+    {   // rest population: c = 0, e_0 = base, Phi_0 = -3 u.F
+        V fs = vfma(nomega, vfma(nwr[0], base, fl[0]), fl[0]);
+        if constexpr (FORCED) fs = vfma(cfw[0], m3uF, fs);
         fl[0] = fs;
     }
     static_for<1, L::Q>([&](auto ic) {
@@ -395,20 +403,17 @@ __device__ __forceinline__ void collide(R* fl, R rho_s, const R* u, const R* Fs,
         constexpr int o = L::opp(i);
         if constexpr (i < o) {
             constexpr int k = L::wclass(i);
-            const R cu = dotc<L, i>(u);
-            const R t3 = (R)3 * cu;
-            const R q = ((R)4.5 * cu) * cu;
-            const R fe_i = wr[k] * ((base + t3) + q);
-            const R fe_o = wr[k] * ((base - t3) + q);
-            R fs_i = fl[i] - omega * (fl[i] - fe_i);
-            R fs_o = fl[o] - omega * (fl[o] - fe_o);
+            const V cu = dotc<L, i>(u);
+            const V bq = vfma(vconst<V>(4.5) * cu, cu, base);
+            const V e_i = vfma(c3, cu, bq);
+            const V e_o = vfma(cm3, cu, bq);
+            V fs_i = vfma(nomega, vfma(nwr[k], e_i, fl[i]), fl[i]);
+            V fs_o = vfma(nomega, vfma(nwr[k], e_o, fl[o]), fl[o]);
             if constexpr (FORCED) {
-                const R cF = dotc<L, i>(Fs);
-                const R g = ((R)9 * cu) * cF;
-                const R Fi_i = W[k] * ((R)3 * (cF - uF) + g);
-                const R Fi_o = W[k] * ((R)3 * ((-cF) - uF) + g);
-                fs_i = fs_i + cfs * Fi_i;
-                fs_o = fs_o + cfs * Fi_o;
+                const V cF = dotc<L, i>(Fs);
+                const V A = vfma(vconst<V>(9.0) * cu, cF, m3uF);
+                fs_i = vfma(cfw[k], vfma(c3, cF, A), fs_i);
+                fs_o = vfma(cfw[k], vfma(cm3, cF, A), fs_o);
             }
             fl[i] = fs_i;
             fl[o] = fs_o;
@@ -416,27 +421,36 @@ __device__ __forceinline__ void collide(R* fl, R rho_s, const R* u, const R* Fs,
     });
 }
 
-// step a6: scalar lattice, Eq. 34-36 + source w_i R, R = -k C 4 rhoA rhoB/(rhoA+rhoB)^2 (R8)
-template <class R, class LS>
-__device__ __forceinline__ void collide_scalar(const KP<R>& p, R* hl, R rA, R rB, R inv_rho, const R* u) {
-    R C = hl[0];
+// step a6: scalar lattice, Eq. 34-36 + source w_i R, R = -k C 4 rhoA rhoB/(rhoA+rhoB)^2 (R8):
+// d = fma(-(w C), fma(1/c_sg^2, c.u, 1), h) = h - h^eq;  h* = fma(w, R, fma(-omega_c, d, h))
+template <class V, class LS, class T>
+__device__ __forceinline__ void collide_scalar(const KP<T>& p, V* hl, V rA, V rB, V inv_rho, const V* u) {
+    V C = hl[0];
     static_for<1, LS::Q>([&](auto ic) { C = C + hl[decltype(ic)::value]; });
-    const R chi = ((R)4 * (rA * inv_rho)) * (rB * inv_rho);
-    const R Rsrc = -((p.k_react * C) * chi);
-    const R wC0 = p.ws0 * C, wC1 = p.ws1 * C;
-    const R s0 = p.ws0 * Rsrc, s1 = p.ws1 * Rsrc;
-    hl[0] = (hl[0] - p.omega_c * (hl[0] - wC0)) + s0;
+    const V chi = (vconst<V>(4.0) * (rA * inv_rho)) * (rB * inv_rho);
+    const V Rsrc = -((vbcast<V>(p.k_react) * C) * chi);
+    const V nwC0 = vbcast<V>(-p.ws0) * C, nwC1 = vbcast<V>(-p.ws1) * C;
+    const V w0 = vbcast<V>(p.ws0), w1 = vbcast<V>(p.ws1), nomc = vbcast<V>(-p.omega_c);
+    const V inv = vbcast<V>(p.inv_cs2g), ninv = vbcast<V>(-p.inv_cs2g), one = vconst<V>(1.0);
+    hl[0] = vfma(w0, Rsrc, vfma(nomc, hl[0] + nwC0, hl[0]));       // c = 0: h^eq = (w_0 C) * 1 exactly
     static_for<1, LS::Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         constexpr int o = LS::opp(i);
         if constexpr (i < o) {
-            const R m = p.inv_cs2g * dotc<LS, i>(u);
-            const R he_i = wC1 * ((R)1 + m);
-            const R he_o = wC1 * ((R)1 - m);
-            hl[i] = (hl[i] - p.omega_c * (hl[i] - he_i)) + s1;
-            hl[o] = (hl[o] - p.omega_c * (hl[o] - he_o)) + s1;
+            const V m = dotc<LS, i>(u);
+            const V d_i = vfma(nwC1, vfma(inv, m, one), hl[i]);
+            const V d_o = vfma(nwC1, vfma(ninv, m, one), hl[o]);
+            hl[i] = vfma(w1, Rsrc, vfma(nomc, d_i, hl[i]));
+            hl[o] = vfma(w1, Rsrc, vfma(nomc, d_o, hl[o]));
         }
     });
+}
+
+// step a5 for component s with the constants of the context (KP): -omega^s and (1 - 1/(2 tau^s)) w_k
+template <class V, class L, bool FORCED, int s, class T>
+__device__ __forceinline__ void collide_component(const KP<T>& p, V* fl, V rho_s, const V* u, const V* Fs) {
+    const V cfw[3] = {vbcast<V>(p.cfw[s][0]), vbcast<V>(p.cfw[s][1]), vbcast<V>(p.cfw[s][2])};
+    collide<V, L, FORCED>(fl, rho_s, u, Fs, vbcast<V>(-p.omega[s]), cfw);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -499,7 +513,7 @@ __device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl
     asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
-        collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+        collide_component<R, L, FORCED, s>(p, fl[s], m.rho[s], m.u, m.F[s]);
         store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
     });
     if constexpr (MT::SCALAR) {
@@ -526,7 +540,7 @@ __device__ __forceinline__ void moving_wall_correction(const KP<R>& p, const NB&
             if constexpr (CZ != 0) { if (!found && (CZ < 0 ? nb.lo[2] : nb.hi[2])) { uw = p.wall_u[2][CZ < 0 ? 0 : 1]; found = true; } }
             const R u3[3] = {uw[0], uw[1], uw[2]};
             const R cuw = dotc<L, k>(u3);
-            fl[k] = fl[k] - (((R)6 * (R)L::w(k)) * rho_s) * cuw;
+            fl[k] = vfma(-((R)(6.0 * L::w(k)) * rho_s), cuw, fl[k]);
         }
     });
 }
@@ -560,18 +574,18 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     R ueq[S][3];
     if constexpr (VSHIFT) {
         R den = m.rho[0] * p.omega[0];
-        if constexpr (S == 2) den = den + m.rho[1] * p.omega[1];
-        const R inv_den = (R)1 / den;
+        if constexpr (S == 2) den = vfma(m.rho[1], p.omega[1], den);
+        const R inv_den = vrecip(den);
         R inv_rs[S];
-        static_for<0, S>([&](auto sc) { inv_rs[decltype(sc)::value] = (R)1 / m.rho[decltype(sc)::value]; });
+        static_for<0, S>([&](auto sc) { inv_rs[decltype(sc)::value] = vrecip(m.rho[decltype(sc)::value]); });
         static_for<0, L::D>([&](auto ac) {
             constexpr int a = decltype(ac)::value;
             R num = m.j[0][a] * p.omega[0];
-            if constexpr (S == 2) num = num + m.j[1][a] * p.omega[1];
+            if constexpr (S == 2) num = vfma(m.j[1][a], p.omega[1], num);
             const R up = num * inv_den;
             static_for<0, S>([&](auto sc) {
                 constexpr int s = decltype(sc)::value;
-                ueq[s][a] = up + (p.tau[s] * m.F[s][a]) * inv_rs[s];
+                ueq[s][a] = vfma(p.tau[s] * m.F[s][a], inv_rs[s], up);
             });
         });
     }
@@ -580,8 +594,8 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
-        if constexpr (VSHIFT) collide<R, L, false>(fl[s], m.rho[s], ueq[s], m.F[s], p.omega[s], p.cf[s]);
-        else collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+        if constexpr (VSHIFT) collide_component<R, L, false, s>(p, fl[s], m.rho[s], ueq[s], m.F[s]);
+        else collide_component<R, L, FORCED, s>(p, fl[s], m.rho[s], m.u, m.F[s]);
         if constexpr (MOVING && WALLS) moving_wall_correction<L>(p, nb, m.rho[s], fl[s]);
         store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
     });
@@ -594,7 +608,7 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
         // the LBGK relaxation of Eq. 6 with sum g in place of rho and tau_e in place of tau; reflected at walls
         R E = gl[0];
         static_for<1, Q>([&](auto ic) { E = E + gl[decltype(ic)::value]; });
-        collide<R, L, false>(gl, E, m.u, m.F[0], p.omega_c, p.cf[0]);
+        collide<R, L, false>(gl, E, m.u, m.F[0], -p.omega_c, (const R*)nullptr);
         store_pops<L, PARITY, WALLS>(p.h, ns, N, gl);
     }
 }
@@ -623,54 +637,42 @@ __global__ void __launch_bounds__(StepBounds<R, MODEL, L::Q>::THREADS, StepBound
 }
 
 // ------------------------------------------------------------------------------------------
-// fused BGK step, TWO cells (x, x+1) per thread: slots that are not shifted in x (all of them at even parity,
-// those with c_x = 0 at odd parity) are moved as one 2-element vector per thread, the others element-wise.
-// Same per-cell arithmetic as k_step.  Needs an even nx and periodic x (the launcher checks).  Used for fp32 BGK,
-// where k_step is limited by instruction issue: cfg4 fp32 41.4 -> 43.4 GLUPS (1.02 of the measured copy peak);
-// measured with 64 / 128 threads and 4 / 5 / 6 / 8 blocks per SM: 128 threads and 6 blocks are the optimum.  In
-// fp64 the 2 x 19 doubles per thread spill and the single-cell kernel is at the copy peak anyway.
+// fused fp32 BGK step, TWO cells (x, x+1) per thread in packed f32x2 arithmetic (V = F2: one FADD2 / FMUL2 / FFMA2
+// per operation of the expression tree for both cells).  Slots that are not shifted in x (all of them at even
+// parity, those with c_x = 0 at odd parity) are moved as one 8-byte access per thread -- the loaded register pair IS
+// the packed operand -- the others element-wise.  Same per-cell arithmetic as k_step, bit for bit.  Needs an even nx
+// and periodic x (the launcher checks).  k_step in fp32 is limited by instruction issue; in fp64 there is no packed
+// arithmetic and the single-cell kernel is at the copy peak anyway.
 // ------------------------------------------------------------------------------------------
-template <class R> struct Vec2;
-template <> struct Vec2<float> { using type = float2; };
-template <> struct Vec2<double> { using type = double2; };
-
-template <class R, class L, int PARITY, int WALLS, bool FORCED>
-__global__ void __launch_bounds__(128, 6) k_step_v2(const __grid_constant__ KP<R> p) {
-    using V = typename Vec2<R>::type;
+template <class L, int PARITY, int WALLS, bool FORCED>
+__global__ void __launch_bounds__(128, 6) k_step_v2(const __grid_constant__ KP<float> p) {
     constexpr int Q = L::Q;
     const int x = 2 * (int)(blockIdx.x * blockDim.x + threadIdx.x), y = (int)blockIdx.y, z = (int)blockIdx.z;
     if (x >= p.nx) return;
     const size_t N = (size_t)p.N;
     const Nbr<L::D, WALLS> na(p, x, y, z), nbb(p, x + 1, y, z);
-    R fa[1][Q], fb[1][Q];
+    F2 f2[1][Q];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        R* pa = slot_of<L, PARITY, WALLS, i>(p.f, na, N);
-        if constexpr (PARITY == 0 || L::c(i, 0) == 0) {
-            const V v = *reinterpret_cast<const V*>(pa);
-            fa[0][i] = v.x; fb[0][i] = v.y;
-        } else {
-            fa[0][i] = *pa;
-            fb[0][i] = *slot_of<L, PARITY, WALLS, i>(p.f, nbb, N);
-        }
+        float* pa = slot_of<L, PARITY, WALLS, i>(p.f, na, N);
+        if constexpr (PARITY == 0 || L::c(i, 0) == 0) f2[0][i].v = *reinterpret_cast<const unsigned long long*>(pa);
+        else f2[0][i] = pack2(*pa, *slot_of<L, PARITY, WALLS, i>(p.f, nbb, N));
     });
-    CellMacro<R, L, M_BGK> ma, mb;
-    cell_macros_core<R, L, M_BGK, FORCED>(p, fa, nullptr, nullptr, ma);
-    cell_macros_core<R, L, M_BGK, FORCED>(p, fb, nullptr, nullptr, mb);
-    collide<R, L, FORCED>(fa[0], ma.rho[0], ma.u, ma.F[0], p.omega[0], p.cf[0]);
-    collide<R, L, FORCED>(fb[0], mb.rho[0], mb.u, mb.F[0], p.omega[0], p.cf[0]);
+    CellMacro<F2, L, M_BGK> m;
+    cell_macros_core<F2, L, M_BGK, FORCED>(p, f2, (const F2(*)[3])nullptr, (const F2*)nullptr, m);
+    collide_component<F2, L, FORCED, 0>(p, f2[0], m.rho[0], m.u, m.F[0]);
     Nbr<L::D, WALLS> sa = na, sb = nbb;
     asm volatile("" : "+r"(sa.xx[0]), "+r"(sa.xx[1]), "+r"(sa.xx[2]), "+r"(sb.xx[0]), "+r"(sb.xx[1]), "+r"(sb.xx[2]));
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        R* pa = slot_of<L, PARITY, WALLS, i>(p.f, sa, N);
+        float* pa = slot_of<L, PARITY, WALLS, i>(p.f, sa, N);
         if constexpr (PARITY == 0 || L::c(i, 0) == 0) {
-            V v;
-            v.x = fa[0][L::opp(i)]; v.y = fb[0][L::opp(i)];
-            *reinterpret_cast<V*>(pa) = v;
+            *reinterpret_cast<unsigned long long*>(pa) = f2[0][L::opp(i)].v;
         } else {
-            *pa = fa[0][L::opp(i)];
-            *slot_of<L, PARITY, WALLS, i>(p.f, sb, N) = fb[0][L::opp(i)];
+            float lo, hi;
+            unpack2(f2[0][L::opp(i)], lo, hi);
+            *pa = lo;
+            *slot_of<L, PARITY, WALLS, i>(p.f, sb, N) = hi;
         }
     });
 }
@@ -847,9 +849,9 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
     // populations = equilibrium at (rho, u), no non-equilibrium part (R10)
     const R u[3] = {(R)u0[0], (R)u0[1], (R)u0[2]};
     R usq = u[0] * u[0];
-    usq = usq + u[1] * u[1];
-    if constexpr (D == 3) usq = usq + u[2] * u[2];
-    const R base = (R)1 - (R)1.5 * usq;
+    usq = vfma(u[1], u[1], usq);
+    if constexpr (D == 3) usq = vfma(u[2], u[2], usq);
+    const R base = vfma((R)-1.5, usq, (R)1);
     static_for<0, S>([&](auto sc) {
         constexpr int s = decltype(sc)::value;
         const R rho_s = (R)r0[s];
@@ -857,7 +859,7 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const R cu = dotc<L, i>(u);
-            fb[(size_t)i * N + cell] = ((R)L::w(i) * rho_s) * ((base + (R)3 * cu) + ((R)4.5 * cu) * cu);
+            fb[(size_t)i * N + cell] = ((R)L::w(i) * rho_s) * vfma((R)3, cu, vfma((R)4.5 * cu, cu, base));
         });
     });
     if constexpr (MT::SCALAR) {
@@ -865,7 +867,7 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
             constexpr int i = decltype(ic)::value;
             const R cu = dotc<LS, i>(u);
             const R wsi = i == 0 ? p.ws0 : p.ws1;
-            p.h[(size_t)i * N + cell] = (wsi * (R)c0) * ((R)1 + p.inv_cs2g * cu);
+            p.h[(size_t)i * N + cell] = (wsi * (R)c0) * vfma(p.inv_cs2g, cu, (R)1);
         });
     }
     if constexpr (MT::THERMAL) {     // g_i = g^eq(rho eps, u), eps = c_init: Eq. 30
@@ -873,7 +875,7 @@ __global__ void __launch_bounds__(BLOCK) k_init(const __grid_constant__ KP<R> p,
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const R cu = dotc<L, i>(u);
-            p.h[(size_t)i * N + cell] = ((R)L::w(i) * rhoE) * ((base + (R)3 * cu) + ((R)4.5 * cu) * cu);
+            p.h[(size_t)i * N + cell] = ((R)L::w(i) * rhoE) * vfma((R)3, cu, vfma((R)4.5 * cu, cu, base));
         });
     }
 }

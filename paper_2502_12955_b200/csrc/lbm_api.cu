@@ -164,7 +164,11 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     // constants are formed in double and rounded once to R
     for (int s = 0; s < 2; ++s) {
         k.omega[s] = (R)(1.0 / p.tau[s]);
-        k.cf[s] = (R)(1.0 - 0.5 / p.tau[s]);
+        // (1 - 1/(2 tau)) w per weight class (rest, axis, diagonal), formed in double from the double weights
+        const double wc[3] = {c->lattice == LBM_D3Q19 ? lbm::D3Q19::w(0) : lbm::D2Q9::w(0),
+                              c->lattice == LBM_D3Q19 ? lbm::D3Q19::w(1) : lbm::D2Q9::w(1),
+                              c->lattice == LBM_D3Q19 ? lbm::D3Q19::w(18) : lbm::D2Q9::w(8)};
+        for (int kc = 0; kc < 3; ++kc) k.cfw[s][kc] = (R)((1.0 - 0.5 / p.tau[s]) * wc[kc]);
         k.tau[s] = (R)p.tau[s];
         for (int t = 0; t < 2; ++t) k.G[s][t] = (R)p.G[s][t];
         k.G_ads[s] = (R)p.G_ads[s];

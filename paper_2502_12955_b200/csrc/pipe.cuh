@@ -343,14 +343,11 @@ struct Pipe {
                 static_for<1, Q>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
                     constexpr int CX = L::c(i, 0), CY = L::c(i, 1), CZ = L::c(i, 2);
-                    const R wp = (R)L::w(i) * sb[T::psi_row(tt, CY, CZ) * RS + CX];
+                    const R pv = sb[T::psi_row(tt, CY, CZ) * RS + CX];
                     static_for<0, D>([&](auto ac) {
                         constexpr int a = decltype(ac)::value;
                         constexpr int c = L::c(i, a);
-                        if constexpr (c != 0) {
-                            if constexpr (first_nonzero<L>(i, a)) acc[tt][a] = c > 0 ? wp : -wp;
-                            else acc[tt][a] = c > 0 ? acc[tt][a] + wp : acc[tt][a] - wp;
-                        }
+                        if constexpr (c != 0) acc[tt][a] = vfma((R)(c * L::w(i)), pv, acc[tt][a]);
                     });
                 });
                 psi_own[tt] = sb[T::psi_row(tt, 0, 0) * RS];
@@ -366,7 +363,7 @@ struct Pipe {
         col[2] = (unsigned)(x == p.nx - 1 ? 0 : x + 1);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
-            collide<R, L, FORCED>(fl[s], m.rho[s], m.u, m.F[s], p.omega[s], p.cf[s]);
+            collide_component<R, L, FORCED, s>(p, fl[s], m.rho[s], m.u, m.F[s]);
             write_pops<L, s * Q, EDGE>(tbl, col, fl[s]);
         });
         if constexpr (MT::SCALAR) {
