@@ -346,8 +346,7 @@ def run_reference(args, cfg, key):
 EXTRAS = [
     ("cfg4", dict(precision=32), None, 1000, 50),
     ("cfg5", dict(), None, 100, 10),
-    ("cfg5", dict(), None, 40, 5, ("pipeline", 0, 0), "one-launch shared-memory pipeline (DESIGN.md 6.3)"),
-    ("cfg5", dict(), None, 40, 5, ("wavefront", 0, 0), "one-launch register wavefront (DESIGN.md 6.3)"),
+    ("cfg5", dict(), None, 40, 5, ("register", 0), "two launches per step: psi pass + fused step (DESIGN.md 6.3)"),
     ("cfg1", dict(), None, 2000, 100),
     ("cfg2", dict(), None, 2000, 100),
     ("cfg3", dict(), None, 1000, 50),
@@ -373,8 +372,7 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(workloads.CONFIGS))
     ap.add_argument("--precision", type=int, default=None, choices=[32, 64])
     ap.add_argument("--grid", type=int, nargs=3, default=None, help="override the grid (profiling runs)")
-    ap.add_argument("--path", default=None, help="register | wavefront | pipeline[:rows_per_pencil:lead_rows] "
-                    "(default: the library's choice)")
+    ap.add_argument("--path", default=None, help="register | pipeline[:rows_per_pencil] (default: the library's choice)")
     ap.add_argument("--no-extras", action="store_true", help="skip per_model, e2e and cpu_baseline (profiling runs)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -418,7 +416,7 @@ def main():
     path = None
     if args.path:
         pp = args.path.split(":")
-        path = (pp[0], int(pp[1]) if len(pp) > 1 else 0, int(pp[2]) if len(pp) > 2 else 0)
+        path = (pp[0], int(pp[1]) if len(pp) > 1 else 0)
     r = time_device(cfg, args.steps, args.warmup, device, seed=replica_seed(rank), sampler=sampler, barrier=barrier,
                     path=path)
     ms = max_over_ranks(r["ms"], dist, device)

@@ -134,7 +134,7 @@ int lbm_get_force(lbm_ctx* ctx, void* F);
  * replaced, cleared (NULL) or the context is destroyed.  Solid nodes reflect populations like a wall (halfway
  * bounce-back on arbitrary nodes), are not updated, are left out of the psi stencil (Eq. 11-12,
  * PAPER.md:128-132) and act on the fluid through the adhesion force (G_ads, Eq. 14); all output fields read zero
- * there.  LBM_PATH_REGISTER only; the mask may change at even time levels only (LBM_ESTATE otherwise: at odd
+ * there.  Runs on LBM_PATH_REGISTER (the context falls back to it); the mask may change at even time levels only (LBM_ESTATE otherwise: at odd
  * levels the in-place layout depends on which neighbours reflect).  Synchronises the stream. */
 int lbm_set_mask(lbm_ctx* ctx, const unsigned char* mask);
 
@@ -151,34 +151,37 @@ int lbm_set_populations(lbm_ctx* ctx, const void* f);
 int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
                  void* rho_host, void* u_host, void* phi_host, void* C_host);
 
-/* Which kernels lbm_step launches.  All paths compute the same bits (same expression tree per cell).
- *   LBM_PATH_REGISTER   one thread per cell, populations loaded straight into registers: one launch of the
- *                       fused step kernel per time step, preceded by the psi pass for Shan-Chen models.
- *                       Works for every shape and boundary.
- *   LBM_PATH_PIPELINE   ONE persistent launch per time step: a ticket counter hands out 128-cell row segments
- *                       whose populations (and psi tile) are staged in shared memory by 16-byte asynchronous
- *                       copies, double buffered.  Shan-Chen models run psi segments (step a2) and step
- *                       segments (a1, a3-a8) in the same launch, ordered so that every psi value a step
- *                       segment needs was published by a lower ticket (Eq. 11 / 13 need psi of all neighbours
- *                       at the same time level: PAPER.md:128, 136; R9): the populations cross HBM once per
- *                       step, the second read hits L2.  Needs nx * sizeof(value) % 16 == 0 and periodic x
- *                       (LBM_EINVAL otherwise).
- *   LBM_PATH_WAVEFRONT  Shan-Chen models only: the same one-launch schedule of psi and step segments, with the
- *                       populations loaded straight into registers as on LBM_PATH_REGISTER (any nx).
- * lbm_create starts with LBM_PATH_REGISTER.
- * rows_per_pencil / lead_rows: schedule parameters of the two one-launch paths for Shan-Chen models (<= 0: defaults; DESIGN.md
- * "Wavefront").  Synchronises the stream. */
-enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1, LBM_PATH_WAVEFRONT = 2 };
-int lbm_set_path(lbm_ctx* ctx, int path, int rows_per_pencil, int lead_rows);
+/* Which kernels lbm_step launches.  Both paths compute the same bits (same expression tree per cell).
+ *   LBM_PATH_REGISTER   one thread per cell (two in fp32 BGK), populations loaded straight into registers: one launch
+ *                       of the fused step kernel per time step, preceded by the psi pass for Shan-Chen models
+ *                       (which reads the flow populations a second time).  Works for every shape and boundary.
+ *   LBM_PATH_PIPELINE   Shan-Chen models: ONE persistent, warp-specialised launch per time step (tile.cuh).  A block
+ *                       bulk-copies the populations of a 128-cell row segment into shared memory (cp.async.bulk +
+ *                       mbarrier, a ring of stages), computes and publishes its psi (step a2), keeps the tile in
+ *                       shared memory until the psi of the tiles around it has been published by their owners
+ *                       (Eq. 11 / 13 need psi of all neighbours at the same time level: PAPER.md:128, 136; R9), then
+ *                       collides and streams it (a1, a3-a8) from shared memory, two fp32 cells per thread in packed
+ *                       arithmetic: every population crosses HBM once per step in each direction.  Needs
+ *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing and no solid-node mask (LBM_EINVAL
+ *                       otherwise); walls in y / z are handled.
+ * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a Shan-Chen
+ * context with more than 2^21 cells to LBM_PATH_PIPELINE where it applies (smaller grids replay a CUDA graph of
+ * the register kernels).  lbm_set_mask falls back to LBM_PATH_REGISTER.
+ * rows_per_pencil: rows of the slower-but-one axis that are marched together along the slowest axis (<= 0:
+ * default).  Synchronises the stream. */
+enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1 };
+int lbm_set_path(lbm_ctx* ctx, int path, int rows_per_pencil);
 int lbm_get_path(const lbm_ctx* ctx);
 
-/* The row schedule of the pipelined path for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1,
- * ns = ny): *count items; if items != NULL (HOST, capacity items of 3 int32: kind 1 = psi row / 0 = step
- * row, m, s) they are written out.  Host-only, needs no GPU. */
-int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity,
-                           size_t* count);
+/* The row schedule of LBM_PATH_PIPELINE for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1, ns = ny;
+ * wrap_m / wrap_s: that axis is periodic): *count items; if items != NULL (HOST, capacity items of 3 int32: kind
+ * 0 = full life cycle of the row / 1 = psi only, m, s) they are written out; *lead_rows (optional) receives the
+ * largest distance from a full item to a later item that provides psi it needs.  Host-only, needs no GPU. */
+int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
+                      size_t* count, int* lead_rows);
 
-/* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a wait for published psi timed out). */
+/* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a bounded wait of LBM_PATH_PIPELINE
+ * timed out; lbm_run_host performs the same check before it returns). */
 int lbm_check(lbm_ctx* ctx);
 
 /* number of time steps taken since init / set_populations */

@@ -7,7 +7,7 @@
 namespace lbm {
 
 struct InitArgs;
-struct PipeArgs;
+struct TileArgs;
 
 struct Ops {
     // kp points at a KP<R> of the matching precision
@@ -19,13 +19,10 @@ struct Ops {
     cudaError_t (*permute)(const void* kp, int model, int parity, int walls, void* canon, int to_canonical,
                            cudaStream_t st);
     cudaError_t (*init)(const void* kp, int model, const InitArgs* ia, cudaStream_t st);
-    // pipelined persistent kernel (pipe.cuh); walls: bounce-back walls in y and / or z (x must be periodic)
-    cudaError_t (*pipe)(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
-                        cudaStream_t st);
-    int (*pipe_blocks)(int model, int parity, int walls, int forced);
-    // register-flavoured wavefront kernel of the Shan-Chen models (wave.cuh)
-    cudaError_t (*wave)(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st);
-    int (*wave_blocks)(int model, int parity);
+    // resident-tile persistent kernel of the Shan-Chen models (tile.cuh); walls: bounce-back walls in y and / or z
+    cudaError_t (*tile)(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st);
+    int (*tile_blocks)(int model, int parity, int walls);     // co-resident blocks on the current device
+    int (*tile_stages)();                                     // stages per block (tiles kept in shared memory)
 };
 
 const Ops* ops_f64_d2q9();

@@ -2,11 +2,16 @@
 #pragma once
 #include "dispatch.h"
 #include "kernels.cuh"
-#include "pipe.cuh"
-#include "wave.cuh"
+#include "tile.cuh"
 #include <cstdlib>
 
 namespace lbm {
+
+// stages (tiles in flight) per block of the resident-tile kernel
+#ifndef LBM_TILE_NS
+#define LBM_TILE_NS 3
+#endif
+constexpr int TILE_NS = LBM_TILE_NS;
 
 // threads per block: 128 (64 and 256 measured within 1 % for BGK, 256 slower for Shan-Chen), less for short rows
 template <class R>
@@ -179,93 +184,52 @@ struct Launch {
         return cudaGetLastError();
     }
 
-    // pipelined kernel: blocks == 0 -> only return the number of co-resident blocks through *out_blocks
-    template <int MODEL, bool WALLYZ, bool FORCED>
-    static cudaError_t pipe3(const KP<R>& p, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
-        constexpr size_t smem = pipe_smem_bytes<R, L, MODEL>();
-        auto k0 = k_pipe<R, L, MODEL, 0, WALLYZ, FORCED>;
-        auto k1 = k_pipe<R, L, MODEL, 1, WALLYZ, FORCED>;
+    // resident-tile kernel (tile.cuh): wa == nullptr -> only return the number of co-resident blocks through *out_blocks
+    template <int MODEL, bool WALLYZ>
+    static cudaError_t tile3(const KP<R>& p, int parity, const TileArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
+        using C = TileCfg<R, L, MODEL, TILE_NS>;
+        constexpr size_t smem = C::SMEM;
+        auto k0 = k_tile<R, L, MODEL, 0, WALLYZ, TILE_NS>;
+        auto k1 = k_tile<R, L, MODEL, 1, WALLYZ, TILE_NS>;
         auto k = parity ? k1 : k0;
-        static bool attr_set[2] = {false, false};
-        if (!attr_set[parity]) {
-            cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return e;
-            attr_set[parity] = true;
-        }
+        // per device and context, cheap: set on every call
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
         if (out_blocks) {
             int per_sm = 0, dev = 0, sms = 0;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PIPE_TX, smem);
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, C::THREADS, smem);
             if (e == cudaSuccess) e = cudaGetDevice(&dev);
             if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
             if (e != cudaSuccess) return e;
             *out_blocks = per_sm * sms;
             return cudaSuccess;
         }
-        k<<<blocks, PIPE_TX, smem, st>>>(p, *wa);
+        k<<<blocks, C::THREADS, smem, st>>>(p, *wa);
         return cudaGetLastError();
     }
-    static cudaError_t pipe_any(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
-                                cudaStream_t st, int* out_blocks) {
+    static cudaError_t tile_any(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st,
+                                int* out_blocks) {
         const KP<R>& p = *(const KP<R>*)kp;
-        switch (model) {
-        case M_BGK:
-            if (walls) return forced ? pipe3<M_BGK, true, true>(p, parity, wa, blocks, st, out_blocks)
-                                     : pipe3<M_BGK, true, false>(p, parity, wa, blocks, st, out_blocks);
-            return forced ? pipe3<M_BGK, false, true>(p, parity, wa, blocks, st, out_blocks)
-                          : pipe3<M_BGK, false, false>(p, parity, wa, blocks, st, out_blocks);
-        case M_SC1: return pipe3<M_SC1, false, true>(p, parity, wa, blocks, st, out_blocks);
-        case M_SC2: return pipe3<M_SC2, false, true>(p, parity, wa, blocks, st, out_blocks);
-        case M_SC2_ADE: return pipe3<M_SC2_ADE, false, true>(p, parity, wa, blocks, st, out_blocks);
-        default: return cudaErrorInvalidValue;
-        }
+        cudaError_t e = cudaErrorInvalidValue;
+        with_sc_model(model, [&](auto M) {
+            if (walls) e = tile3<decltype(M)::value, true>(p, parity, wa, blocks, st, out_blocks);
+            else e = tile3<decltype(M)::value, false>(p, parity, wa, blocks, st, out_blocks);
+        });
+        return e;
     }
-    static cudaError_t pipe(const void* kp, int model, int parity, int walls, int forced, const PipeArgs* wa, int blocks,
-                            cudaStream_t st) {
-        return pipe_any(kp, model, parity, walls, forced, wa, blocks, st, nullptr);
+    static cudaError_t tile(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st) {
+        return tile_any(kp, model, parity, walls, wa, blocks, st, nullptr);
     }
-    static int pipe_blocks(int model, int parity, int walls, int forced) {
+    static int tile_blocks(int model, int parity, int walls) {
         int b = 0;
         KP<R> dummy{};
-        if (pipe_any(&dummy, model, parity, walls, forced, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
+        if (tile_any(&dummy, model, parity, walls, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
         return b;
     }
-
-    template <int MODEL>
-    static cudaError_t wave2(const KP<R>& p, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
-        auto k = parity ? k_wave<R, L, MODEL, 1> : k_wave<R, L, MODEL, 0>;
-        if (out_blocks) {
-            int per_sm = 0, dev = 0, sms = 0;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, PIPE_TX, 0);
-            if (e == cudaSuccess) e = cudaGetDevice(&dev);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e != cudaSuccess) return e;
-            *out_blocks = per_sm * sms;
-            return cudaSuccess;
-        }
-        k<<<blocks, PIPE_TX, 0, st>>>(p, *wa);
-        return cudaGetLastError();
-    }
-    static cudaError_t wave_any(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st, int* ob) {
-        const KP<R>& p = *(const KP<R>*)kp;
-        switch (model) {
-        case M_SC1: return wave2<M_SC1>(p, parity, wa, blocks, st, ob);
-        case M_SC2: return wave2<M_SC2>(p, parity, wa, blocks, st, ob);
-        case M_SC2_ADE: return wave2<M_SC2_ADE>(p, parity, wa, blocks, st, ob);
-        default: return cudaErrorInvalidValue;
-        }
-    }
-    static cudaError_t wave(const void* kp, int model, int parity, const PipeArgs* wa, int blocks, cudaStream_t st) {
-        return wave_any(kp, model, parity, wa, blocks, st, nullptr);
-    }
-    static int wave_blocks(int model, int parity) {
-        int b = 0;
-        KP<R> dummy{};
-        if (wave_any(&dummy, model, parity, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
-        return b;
-    }
+    static int tile_stages() { return TILE_NS; }
 
     static const Ops* ops() {
-        static const Ops o = {&psi, &step, &macros, &permute, &init, &pipe, &pipe_blocks, &wave, &wave_blocks};
+        static const Ops o = {&psi, &step, &macros, &permute, &init, &tile, &tile_blocks, &tile_stages};
         return &o;
     }
 };

@@ -484,44 +484,6 @@ __global__ void __launch_bounds__(BLOCK) k_psi(const __grid_constant__ KP<R> p) 
 // ------------------------------------------------------------------------------------------
 // fused step (a1, a3-a8): one thread per cell
 // ------------------------------------------------------------------------------------------
-// first half: the populations of the cell into registers
-template <class R, class L, int MODEL, int PARITY, int WALLS, class NB>
-__device__ __forceinline__ void step_load(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
-    using MT = ModelTraits<MODEL>;
-    using LS = typename ScalarOf<L>::type;
-    constexpr int S = MT::S, Q = L::Q;
-    const size_t N = (size_t)p.N;
-    static_for<0, S>([&](auto sc) {
-        constexpr int s = decltype(sc)::value;
-        load_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, nb, N, fl[s]);
-    });
-    if constexpr (MT::SCALAR) load_pops<LS, PARITY, WALLS>(p.h, nb, N, hl);
-}
-// second half: moments, force (psi stencil), collision, stores
-template <class R, class L, int MODEL, int PARITY, int WALLS, bool FORCED, bool COH, class NB>
-__device__ __forceinline__ void step_finish(const KP<R>& p, const NB& nb, R (*fl)[L::Q], R* hl) {
-    using MT = ModelTraits<MODEL>;
-    using LS = typename ScalarOf<L>::type;
-    constexpr int S = MT::S, Q = L::Q;
-    const size_t N = (size_t)p.N;
-    CellMacro<R, L, MODEL> m;
-    cell_macros<R, L, MODEL, FORCED, COH>(p, nb, fl, m);
-
-    // the store addresses are recomputed from laundered column offsets instead of being kept in
-    // registers from the loads on
-    NB ns = nb;
-    asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
-    static_for<0, S>([&](auto sc) {
-        constexpr int s = decltype(sc)::value;
-        collide_component<R, L, FORCED, s>(p, fl[s], m.rho[s], m.u, m.F[s]);
-        store_pops<L, PARITY, WALLS>(p.f + (size_t)s * Q * N, ns, N, fl[s]);
-    });
-    if constexpr (MT::SCALAR) {
-        collide_scalar<R, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
-        store_pops<LS, PARITY, WALLS>(p.h, ns, N, hl);
-    }
-}
-
 // Moving-wall halfway bounce-back (DESIGN R24): a post-collision population f*_k that leaves the
 // cell through a wall comes back as f_opp(k) minus 2 w_k rho (c_k . u_w) / c_s^2.  It is stored exactly once (to
 // P_opp(k)(x), the cell's own slot), so the correction is applied to the register value before the stores.
@@ -545,8 +507,7 @@ __device__ __forceinline__ void moving_wall_correction(const KP<R>& p, const NB&
     });
 }
 
-// both halves for one cell (k_step).  Written out rather than calling step_load / step_finish: ptxas keeps the
-// load addresses alive across the call boundary of the split form (fp32 BGK: 40 -> 80 registers).
+// one cell of the fused step (k_step)
 template <class R, class L, int MODEL, int PARITY, int WALLS, bool FORCED, bool COH = false, bool VSHIFT = false, bool MOVING = false>
 __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     using MT = ModelTraits<MODEL>;

@@ -13,11 +13,14 @@
 
 #include "dispatch.h"
 #include "kernels.cuh"
-#include "pipe.cuh"
+#include "tile.cuh"
 
 namespace {
 
 thread_local std::string g_err;
+#ifdef LBM_TILE_TRACE
+long long* g_trace = nullptr;
+#endif
 
 int fail(int code, const std::string& msg) {
     g_err = msg;
@@ -135,17 +138,16 @@ struct lbm_ctx {
     cudaGraphExec_t graph_exec;
     cudaStream_t graph_capture_stream;
     bool graph_failed;
-    // one-launch persistent paths (pipe.cuh, wave.cuh): schedule, ticket counter, flags
-    int wave_py, wave_lead;           // schedule parameters in use
-    int wave_blocks[2];               // blocks per launch, by parity
-    lbm::PipeItem* wave_items;        // device copy of the schedule, one entry per ticket
-    long long wave_n_items;
-    int wave_nxs;
-    int* wave_flags;                  // one int per chunk, then the status word
-    size_t wave_n_chunks;
-    unsigned long long* wave_counter;
-    unsigned long long wave_base;
-    int wave_epoch;
+    // resident-tile path (tile.cuh): schedule, flags
+    int tile_py, tile_lead;           // rows per pencil in use; lead of the schedule in tickets
+    int tile_blocks;                  // blocks per launch
+    lbm::TileItem* tile_items;        // device copy of the schedule, one entry per ticket
+    long long tile_n_items;
+    int tile_nxs;
+    int* tile_flags;                  // one int per tile, then the status word
+    size_t tile_n_tiles;
+    int tile_epoch;
+    bool path_user_set;               // the caller chose the path (lbm_set_path): no automatic switch
 
     const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
     // kernel variant: 0 fully periodic, 1 bounce-back walls (bc), 2 with a solid-node mask
@@ -246,102 +248,111 @@ int run_psi(lbm_ctx* c) {
     return mark(c, 1);
 }
 
-void wave_free(lbm_ctx* c) {
-    if (c->wave_items) cudaFree(c->wave_items);
-    if (c->wave_flags) cudaFree(c->wave_flags);
-    if (c->wave_counter) cudaFree(c->wave_counter);
-    c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
+void tile_free(lbm_ctx* c) {
+    if (c->tile_items) cudaFree(c->tile_items);
+    if (c->tile_flags) cudaFree(c->tile_flags);
+    c->tile_items = nullptr; c->tile_flags = nullptr;
     c->path = LBM_PATH_REGISTER;
 }
 
-bool pipe_eligible(const lbm_ctx* c) {
-    return ((size_t)c->nx * c->sh.B) % 16 == 0 && c->p.bc[0] == 0;
+// what the resident-tile kernel handles (tile.cuh): Shan-Chen models with Guo forcing, periodic x, 16-byte aligned
+// rows, walls in y / z at rest, no solid-node mask
+const char* tile_ineligible(const lbm_ctx* c) {
+    if (!c->sh.sc) return "LBM_PATH_PIPELINE exists for the Shan-Chen models (BGK already moves the algorithmic bytes)";
+    if (c->forced == 2) return "velocity-shift forcing runs on LBM_PATH_REGISTER only";
+    if (c->kp64.mask) return "a solid-node mask runs on LBM_PATH_REGISTER only";
+    if (c->p.bc[0] != 0) return "LBM_PATH_PIPELINE needs periodic x";
+    if (((size_t)c->nx * c->sh.B) % 16 != 0) return "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes";
+    return nullptr;
 }
 
-// Switch to the pipelined path: (re)build the schedule (one entry per ticket) and the device state of the
-// ticket counter; py / lead <= 0 pick the defaults
-int path_setup(lbm_ctx* c, int path, int py, int lead) {
+// Switch to the resident-tile path: build the schedule (one entry per ticket) and the flags; py <= 0 picks the default
+int path_setup(lbm_ctx* c, int py) {
     CK(cudaStreamSynchronize(c->stream));
-    wave_free(c);
+    tile_free(c);
     const Shape& sh = c->sh;
     const int nm = sh.d == 3 ? c->ny : 1, ns = sh.d == 3 ? c->nz : c->ny;
-    const int nxs = (c->nx + lbm::PIPE_TX - 1) / lbm::PIPE_TX;
-    for (int par = 0; par < 2; ++par) {
-        c->wave_blocks[par] = path == LBM_PATH_WAVEFRONT ? c->ops->wave_blocks(c->model, par)
-                                                          : c->ops->pipe_blocks(c->model, par, c->walls, c->forced);
-        if (c->wave_blocks[par] < 1) return fail(LBM_ECUDA, "persistent kernel: occupancy query failed");
+    const bool wrap_m = sh.d == 3 ? c->p.bc[1] == 0 : true, wrap_s = sh.d == 3 ? c->p.bc[2] == 0 : c->p.bc[1] == 0;
+    const int nxs = (c->nx + lbm::TILE_TX - 1) / lbm::TILE_TX;
+    const int walls = c->bc_walls ? 1 : 0;
+    int resident = c->ops->tile_blocks(c->model, 0, walls);
+    const int r1 = c->ops->tile_blocks(c->model, 1, walls);
+    if (r1 < resident) resident = r1;
+    if (resident < 1) return fail(LBM_ECUDA, "resident-tile kernel: occupancy query failed");
+    const int stages = c->ops->tile_stages();
+    // default pencil: the psi a step waits for is about one stage of tickets ahead (tile.cuh: LEAD <= (NS - 1) * B)
+    if (py <= 0) py = resident / nxs - 2;
+    if (py < 1) py = 1;
+    if (py > nm) py = nm;
+    std::vector<lbm::TileRow> rows;
+    int blocks = 0;
+    long long lead_tickets = 0;
+    for (;;) {
+        int lead_rows = 0;
+        rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, &lead_rows);
+        const long long n_items = (long long)rows.size() * nxs;
+        blocks = (long long)resident < n_items ? resident : (int)n_items;
+        lead_tickets = ((long long)lead_rows + 1) * nxs;      // x-neighbours of the last needed row included
+        if (lead_tickets <= (long long)(stages - 1) * blocks) break;
+        if (py == 1) return fail(LBM_EINVAL, "resident-tile kernel: the grid is too wide for the pipeline depth of this device");
+        py = py / 2;
     }
-    std::vector<lbm::WaveItem> rows;
-    if (sh.sc) {
-        if (py <= 0) {
-            // a pencil plane of about 4 MB of populations: psi item and step item of a row stay close in L2
-            const double row_bytes = (double)c->nx * (double)(sh.S * sh.Q + (sh.scalar ? sh.Qs : 0)) * (double)sh.B;
-            py = (int)(4.0e6 / row_bytes);
-        }
-        if (py < 1) py = 1;
-        if (py > nm) py = nm;
-        if (lead <= 0) lead = (2 * c->wave_blocks[0] + nxs - 1) / nxs;   // psi items about two waves of blocks ahead
-        if (lead < 1) lead = 1;
-        rows = lbm::wave_schedule(nm, ns, py, lead);
-        c->wave_py = py; c->wave_lead = lead;
-    } else {
-        c->wave_py = c->wave_lead = 0;
-        rows.reserve((size_t)nm * ns);
-        for (int s = 0; s < ns; ++s)
-            for (int m = 0; m < nm; ++m) rows.push_back(lbm::WaveItem{m, s});     // step rows only
-    }
-    if ((double)rows.size() * nxs > 2.0e9) return fail(LBM_EINVAL, "pipelined path: more than 2e9 tickets");
-    std::vector<lbm::PipeItem> items;
+    if ((double)rows.size() * nxs > 2.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 2e9 tickets");
+    std::vector<lbm::TileItem> items;
     items.reserve(rows.size() * (size_t)nxs);
-    for (const lbm::WaveItem& r : rows) {
-        const int m = r.m & 0x7fffffff;
-        lbm::PipeItem it;
-        it.kind = r.m < 0 ? lbm::ITEM_PSI : lbm::ITEM_STEP;
-        it.y = sh.d == 3 ? m : r.s;
+    for (const lbm::TileRow& r : rows) {
+        lbm::TileItem it;
+        it.kind = r.kind;
+        it.y = sh.d == 3 ? r.m : r.s;
         it.z = sh.d == 3 ? r.s : 0;
         for (int xs = 0; xs < nxs; ++xs) { it.xs = xs; items.push_back(it); }
     }
-    c->wave_n_items = (long long)items.size();
-    c->wave_nxs = nxs;
-    c->wave_n_chunks = (size_t)nm * ns * nxs;
-    cudaError_t e = cudaMalloc((void**)&c->wave_items, items.size() * sizeof(lbm::PipeItem));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_flags, (c->wave_n_chunks + 1) * sizeof(int));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&c->wave_counter, sizeof(unsigned long long));
-    if (e != cudaSuccess) { cudaGetLastError(); wave_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
-    CK(cudaMemcpyAsync(c->wave_items, items.data(), items.size() * sizeof(lbm::PipeItem), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemsetAsync(c->wave_flags, 0, (c->wave_n_chunks + 1) * sizeof(int), c->stream));
-    CK(cudaMemsetAsync(c->wave_counter, 0, sizeof(unsigned long long), c->stream));
+    c->tile_py = py; c->tile_lead = (int)lead_tickets; c->tile_blocks = blocks;
+    c->tile_n_items = (long long)items.size();
+    c->tile_nxs = nxs;
+    c->tile_n_tiles = (size_t)nm * ns * nxs;
+    cudaError_t e = cudaMalloc((void**)&c->tile_items, items.size() * sizeof(lbm::TileItem));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->tile_flags, (c->tile_n_tiles + 1) * sizeof(int));
+    if (e != cudaSuccess) { cudaGetLastError(); tile_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
+    CK(cudaMemcpyAsync(c->tile_items, items.data(), items.size() * sizeof(lbm::TileItem), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemsetAsync(c->tile_flags, 0, (c->tile_n_tiles + 1) * sizeof(int), c->stream));
     CK(cudaStreamSynchronize(c->stream));   // items goes out of scope
-    c->wave_base = 0;
-    c->wave_epoch = 0;
-    c->path = path;
+    c->tile_epoch = 0;
+    c->path = LBM_PATH_PIPELINE;
     return 0;
 }
 
-int run_pipe(lbm_ctx* c) {
+int run_tile(lbm_ctx* c) {
     const int parity = (int)(c->t & 1);
-    if (c->wave_epoch == 0x7fffffff) {   // epoch wrap: clear the flags (once per 2^31 - 1 launches)
-        CK(cudaMemsetAsync(c->wave_flags, 0, c->wave_n_chunks * sizeof(int), c->stream));
-        c->wave_epoch = 0;
+    if (c->tile_epoch == 0x7fffffff) {   // epoch wrap: clear the flags (once per 2^31 - 1 launches)
+        CK(cudaMemsetAsync(c->tile_flags, 0, c->tile_n_tiles * sizeof(int), c->stream));
+        c->tile_epoch = 0;
     }
-    lbm::PipeArgs wa;
-    wa.items = c->wave_items;
-    wa.n_tickets = (unsigned)c->wave_n_items;
-    wa.nxs = c->wave_nxs;
-    wa.flags = c->wave_flags;
-    wa.counter = c->wave_counter;
-    wa.base = c->wave_base;
-    wa.epoch = ++c->wave_epoch;
-    wa.status = c->wave_flags + c->wave_n_chunks;
-    const int blocks = c->wave_blocks[parity];
+    lbm::TileArgs wa;
+    wa.items = c->tile_items;
+    wa.n_items = (unsigned)c->tile_n_items;
+    wa.nxs = c->tile_nxs;
+    wa.flags = c->tile_flags;
+    wa.epoch = ++c->tile_epoch;
+    wa.status = c->tile_flags + c->tile_n_tiles;
+#ifdef LBM_TILE_TRACE
+    if (!g_trace) { cudaMalloc((void**)&g_trace, sizeof(long long) * 10 * 4096); cudaMemset(g_trace, 0, sizeof(long long) * 10 * 4096); }
+    wa.trace = g_trace;
+#endif
     int rc = mark(c, 0);
     if (rc) return rc;
-    if (c->path == LBM_PATH_WAVEFRONT) CK(c->ops->wave(c->kp(), c->model, parity, &wa, blocks, c->stream));
-    else CK(c->ops->pipe(c->kp(), c->model, parity, c->walls, c->forced, &wa, blocks, c->stream));
-    // every block draws tickets until three of them lie past the end (pipe.cuh)
-    c->wave_base += (unsigned long long)wa.n_tickets + 3ULL * (unsigned long long)blocks;
+    CK(c->ops->tile(c->kp(), c->model, parity, c->bc_walls ? 1 : 0, &wa, c->tile_blocks, c->stream));
     c->launches++;
     return mark(c, 0);
+}
+
+// deferred device-side error of the resident-tile path (a bounded wait gave up); the stream must be idle
+int tile_status(lbm_ctx* c) {
+    if (c->path == LBM_PATH_REGISTER) return 0;
+    int st = 0;
+    CK(cudaMemcpy(&st, c->tile_flags + c->tile_n_tiles, sizeof(int), cudaMemcpyDeviceToHost));
+    if (st != 0) return fail(LBM_ECUDA, "resident-tile kernel: a wait for published psi timed out; the state is invalid");
+    return 0;
 }
 
 int ensure_scratch(lbm_ctx* c, size_t bytes) {
@@ -387,8 +398,8 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->droplets_dev = nullptr; c->scratch = nullptr; c->scratch_bytes = 0;
     c->timing = false;
     c->graph_exec = nullptr; c->graph_capture_stream = nullptr; c->graph_failed = false;
-    c->path = LBM_PATH_REGISTER; c->wave_items = nullptr; c->wave_flags = nullptr; c->wave_counter = nullptr;
-    c->wave_py = c->wave_lead = 0; c->wave_base = 0; c->wave_epoch = 0;
+    c->path = LBM_PATH_REGISTER; c->tile_items = nullptr; c->tile_flags = nullptr;
+    c->tile_py = c->tile_lead = 0; c->tile_blocks = 0; c->tile_epoch = 0; c->path_user_set = false;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
         if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
@@ -430,7 +441,7 @@ void lbm_destroy(lbm_ctx* c) {
     drop_events(c);
     if (c->droplets_dev) cudaFree(c->droplets_dev);
     if (c->scratch) cudaFree(c->scratch);
-    wave_free(c);
+    tile_free(c);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     if (c->graph_capture_stream) cudaStreamDestroy(c->graph_capture_stream);
     if (c->owns_ws && c->ws) cudaFree(c->ws);
@@ -469,6 +480,15 @@ namespace {
 constexpr int GRAPH_STEPS = 32;                 // even: a replay starts and ends at even parity
 constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far longer than a launch call
 
+// Default launch path, chosen at the first step unless the caller chose one (lbm_set_path): Shan-Chen models on
+// grids too large for the CUDA-graph replay take the resident-tile kernel where it applies (tile.cuh)
+void choose_default_path(lbm_ctx* c) {
+    if (c->path_user_set || c->path != LBM_PATH_REGISTER) return;
+    c->path_user_set = true;                    // decide once
+    if (c->sh.N <= GRAPH_MAX_CELLS || tile_ineligible(c) != nullptr) return;
+    if (path_setup(c, 0) != 0) { cudaGetLastError(); tile_free(c); }
+}
+
 // the kernels of one time step of the register path, enqueued on st (no event marks, no counters)
 int enqueue_register_step(lbm_ctx* c, int parity, cudaStream_t st) {
     if (c->sh.sc) CK(c->ops->psi(c->kp(), c->model, parity, c->wmode(), st));
@@ -501,6 +521,7 @@ int lbm_step(lbm_ctx* c, int n) {
     if (!c->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init_from_seed / lbm_set_populations");
     if (n < 0) return fail(LBM_EINVAL, "n < 0");
     DeviceGuard g(c->device);
+    if ((c->t & 1) == 0) choose_default_path(c);
     int done = 0;
     if (c->path == LBM_PATH_REGISTER && !c->timing && !c->graph_failed && c->sh.N <= GRAPH_MAX_CELLS) {
         if ((c->t & 1) && n >= GRAPH_STEPS + 1) {       // reach even parity with one ordinary step
@@ -520,8 +541,8 @@ int lbm_step(lbm_ctx* c, int n) {
     for (int k = done; k < n; ++k) {
         const int parity = (int)(c->t & 1);
         int rc;
-        if (c->path != LBM_PATH_REGISTER) {   // one persistent ticketed launch per step (pipe.cuh)
-            if ((rc = run_pipe(c))) return rc;
+        if (c->path != LBM_PATH_REGISTER) {   // one persistent launch per step (tile.cuh)
+            if ((rc = run_tile(c))) return rc;
             c->t++;
             continue;
         }
@@ -625,7 +646,7 @@ int lbm_run_host(lbm_ctx* c, const void* f_in_host, int n, void* rho_h, void* u_
         if (C_h) CK(cudaMemcpyAsync(C_h, C_d, fb, cudaMemcpyDeviceToHost, c->stream));
     }
     CK(cudaStreamSynchronize(c->stream));
-    return 0;
+    return tile_status(c);
 }
 
 int lbm_kernel_timing(lbm_ctx* c, int enable) {
@@ -654,40 +675,32 @@ int lbm_kernel_time_ms(lbm_ctx* c, int kind, double* total_ms, int64_t* launches
     return 0;
 }
 
-int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil, int lead_rows) {
+int lbm_set_path(lbm_ctx* c, int path, int rows_per_pencil) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
     DeviceGuard g(c->device);
     if (path == LBM_PATH_REGISTER) {
         CK(cudaStreamSynchronize(c->stream));
-        wave_free(c);
+        tile_free(c);
+        c->path_user_set = true;
         return 0;
     }
-    if (c->forced == 2) return fail(LBM_EINVAL, "velocity-shift forcing runs on LBM_PATH_REGISTER only");
-    if (c->sh.sc && c->walls) return fail(LBM_EINVAL, "Shan-Chen models between walls run on LBM_PATH_REGISTER only");
-    if (c->moving) return fail(LBM_EINVAL, "moving walls run on LBM_PATH_REGISTER only");
-    if (c->model == LBM_BGK_T) return fail(LBM_EINVAL, "LBM_BGK_T runs on LBM_PATH_REGISTER only");
-    if (c->kp64.mask) return fail(LBM_EINVAL, "a solid-node mask runs on LBM_PATH_REGISTER only");
-    if (path == LBM_PATH_WAVEFRONT) {
-        if (!c->sh.sc) return fail(LBM_EINVAL, "LBM_PATH_WAVEFRONT exists for the Shan-Chen models only");
-    } else if (path == LBM_PATH_PIPELINE) {
-        if (!pipe_eligible(c))
-            return fail(LBM_EINVAL, "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes and periodic x");
-    } else {
-        return fail(LBM_EINVAL, "unknown path");
-    }
-    return path_setup(c, path, rows_per_pencil, lead_rows);
+    if (path != LBM_PATH_PIPELINE) return fail(LBM_EINVAL, "unknown path");
+    if (const char* why = tile_ineligible(c)) return fail(LBM_EINVAL, why);
+    int rc = path_setup(c, rows_per_pencil);
+    if (rc == 0) c->path_user_set = true;
+    return rc;
 }
 
 int lbm_get_path(const lbm_ctx* c) { return c ? c->path : LBM_EINVAL; }
 
 int lbm_set_mask(lbm_ctx* c, const unsigned char* mask) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
-    if (mask && c->path != LBM_PATH_REGISTER) return fail(LBM_EINVAL, "a solid-node mask runs on LBM_PATH_REGISTER only");
     // at an odd time level the in-place layout depends on which neighbours reflect: the mask may only change
     // when the populations sit in their own cells
     if (c->inited && (c->t & 1)) return fail(LBM_ESTATE, "lbm_set_mask needs an even time level (lbm_time)");
     DeviceGuard g(c->device);
     CK(cudaStreamSynchronize(c->stream));
+    if (mask && c->path != LBM_PATH_REGISTER) tile_free(c);     // a solid-node mask runs on LBM_PATH_REGISTER only
     c->kp64.mask = mask;
     c->kp32.mask = mask;
     c->walls = c->bc_walls || mask != nullptr;
@@ -695,16 +708,19 @@ int lbm_set_mask(lbm_ctx* c, const unsigned char* mask) {
     return 0;
 }
 
-int lbm_wavefront_schedule(int nm, int ns, int rows_per_pencil, int lead_rows, int32_t* items, size_t capacity, size_t* count) {
+int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
+                      size_t* count, int* lead_rows) {
     if (!count) return fail(LBM_EINVAL, "count is NULL");
     if (nm < 1 || ns < 1) return fail(LBM_EINVAL, "nm and ns must be >= 1");
-    const std::vector<lbm::WaveItem> v = lbm::wave_schedule(nm, ns, rows_per_pencil, lead_rows);
+    int lead = 0;
+    const std::vector<lbm::TileRow> v = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, &lead);
     *count = v.size();
+    if (lead_rows) *lead_rows = lead;
     if (items) {
         if (capacity < v.size()) return fail(LBM_EINVAL, "capacity too small");
         for (size_t k = 0; k < v.size(); ++k) {
-            items[3 * k + 0] = v[k].m < 0 ? 1 : 0;
-            items[3 * k + 1] = v[k].m & 0x7fffffff;
+            items[3 * k + 0] = v[k].kind;
+            items[3 * k + 1] = v[k].m;
             items[3 * k + 2] = v[k].s;
         }
     }
@@ -715,13 +731,12 @@ int lbm_check(lbm_ctx* c) {
     if (!c) return fail(LBM_EINVAL, "ctx is NULL");
     DeviceGuard g(c->device);
     CK(cudaStreamSynchronize(c->stream));
-    if (c->path != LBM_PATH_REGISTER) {
-        int st = 0;
-        CK(cudaMemcpy(&st, c->wave_flags + c->wave_n_chunks, sizeof(int), cudaMemcpyDeviceToHost));
-        if (st != 0) return fail(LBM_ECUDA, "persistent kernel: a wait for published psi timed out; the state is invalid");
-    }
-    return 0;
+    return tile_status(c);
 }
+
+#ifdef LBM_TILE_TRACE
+int lbm_debug_trace(void* out) { return (int)cudaMemcpy(out, g_trace, sizeof(long long) * 10 * 4096, cudaMemcpyDeviceToHost); }
+#endif
 
 int64_t lbm_time(const lbm_ctx* c) { return c ? c->t : -1; }
 int64_t lbm_launch_count(const lbm_ctx* c) { return c ? c->launches : -1; }

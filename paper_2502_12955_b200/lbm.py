@@ -17,12 +17,12 @@ LATTICES = {"D2Q9": D2Q9, "D3Q19": D3Q19}
 MODELS = {"BGK": BGK, "SC1": SC1, "SC2": SC2, "SC2_ADE": SC2_ADE, "BGK_T": BGK_T}
 INITS = {"REST": 0, "TAYLOR_GREEN": 1, "DROPLET": 2, "UNIFORM_NOISE": 3, "RANDOM_DROPLETS": 4}
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
-PATHS = {"register": 0, "pipeline": 1, "wavefront": 2}
+PATHS = {"register": 0, "pipeline": 1}
 
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_wavefront_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_tile_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -76,10 +76,10 @@ def lib():
     L.lbm_get_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_set_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
-    L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+    L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int]
     L.lbm_get_path.argtypes = [C.c_void_p]
     L.lbm_set_mask.argtypes = [C.c_void_p, C.c_void_p]
-    L.lbm_wavefront_schedule.argtypes = [C.c_int] * 4 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
+    L.lbm_tile_schedule.argtypes = [C.c_int] * 5 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
     L.lbm_check.argtypes = [C.c_void_p]
     L.lbm_time.restype = C.c_int64
     L.lbm_time.argtypes = [C.c_void_p]
@@ -142,19 +142,21 @@ def make_params(**kw):
     return p
 
 
-def wavefront_schedule(nm, ns, rows_per_pencil, lead_rows):
-    """The wavefront kernel's row schedule as an (n, 3) int32 array of (kind, m, s); host-only call."""
+def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True):
+    """The resident-tile kernel's row schedule as an (n, 3) int32 array of (kind, m, s), and its lead in rows;
+    host-only call (kind 0: full life cycle of the row, 1: psi only)."""
     import numpy as np
     L = lib()
     n = C.c_size_t(0)
-    rc = L.lbm_wavefront_schedule(nm, ns, rows_per_pencil, lead_rows, None, 0, C.byref(n))
+    lead = C.c_int(0)
+    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), None, 0, C.byref(n), C.byref(lead))
     if rc != 0:
         raise LbmError(rc, last_error())
     out = np.zeros((n.value, 3), np.int32)
-    rc = L.lbm_wavefront_schedule(nm, ns, rows_per_pencil, lead_rows, out.ctypes.data, n.value, C.byref(n))
+    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), out.ctypes.data, n.value, C.byref(n), C.byref(lead))
     if rc != 0:
         raise LbmError(rc, last_error())
-    return out
+    return out, lead.value
 
 
 def lattice_table(lattice, kind=0):
@@ -277,10 +279,10 @@ class LBM:
         self._chk(self.L.lbm_kernel_time_ms(self.h, int(kind), C.byref(ms), C.byref(n)))
         return ms.value, n.value
 
-    def set_path(self, path, rows_per_pencil=0, lead_rows=0):
-        """which kernels step() launches: "register", "pipeline" or "wavefront" (Shan-Chen only) (include/lbm.h)"""
+    def set_path(self, path, rows_per_pencil=0):
+        """which kernels step() launches: "register" or "pipeline" (Shan-Chen models; include/lbm.h)"""
         path = PATHS[path] if isinstance(path, str) else int(path)
-        self._chk(self.L.lbm_set_path(self.h, path, int(rows_per_pencil), int(lead_rows)))
+        self._chk(self.L.lbm_set_path(self.h, path, int(rows_per_pencil)))
 
     def set_mask(self, mask):
         """solid-node mask (N values, non-zero = solid; any array-like or tensor) or None; kept alive here"""

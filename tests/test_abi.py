@@ -152,29 +152,41 @@ def test_product_path_never_touches_the_oracle():
             assert "liblbm" not in text and "kernels.cuh" not in text and "import paper_2502_12955_b200" not in text, f
 
 
-@pytest.mark.parametrize("nm,ns,py,lead", [(1, 1, 1, 0), (1, 7, 1, 1), (1, 64, 1, 5), (5, 4, 2, 3), (8, 8, 3, 0),
-                                           (8, 8, 8, 100), (2, 2, 1, 1), (3, 1, 2, 1), (16, 9, 5, 7), (6, 5, 100, 2)])
-def test_wavefront_schedule_is_valid(nm, ns, py, lead):
-    """Host logic of the wavefront kernel (wave_schedule.h): every row has exactly one psi item and one
-    step item, and every psi row a step row needs (itself and its 8 neighbours, periodic wrap) comes
-    EARLIER in the list -- the rule that makes the in-kernel waits deadlock-free and the results equal
-    to the two-pass order (psi of the whole field, then the step: DESIGN.md R9)."""
+@pytest.mark.parametrize("nm,ns,py", [(1, 1, 1), (1, 7, 1), (1, 64, 1), (5, 4, 2), (8, 8, 3), (8, 8, 8), (2, 2, 1), (3, 1, 2),
+                                      (16, 9, 5), (6, 5, 100), (40, 12, 7)])
+@pytest.mark.parametrize("wrap_m,wrap_s", [(True, True), (False, True), (True, False), (False, False)])
+def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s):
+    """Host logic of the resident-tile kernel (tile_schedule.h).  Every row has exactly one FULL item (load, psi,
+    wait, step), in pencil order.  The step of a FULL item needs psi of the 3 x 3 rows around it (periodic wrap or
+    wall): each of them is computed by some item (PSI_ONLY, or its own FULL item), and the FIRST such item lies at
+    most `lead` items after the FULL item -- the number the kernel's pipeline depth has to cover for its bounded
+    waits to be deadlock-free; the results equal the two-pass order (psi of the whole field, then
+    the step: R9).  PSI_ONLY items re-read a row: they must stay a small fraction."""
     import paper_2502_12955_b200 as pkg
-    it = pkg.lbm.wavefront_schedule(nm, ns, py, lead)
-    assert it.shape == (2 * nm * ns, 3)
-    pos_psi, pos_step = {}, {}
+    it, lead = pkg.lbm.tile_schedule(nm, ns, py, wrap_m, wrap_s)
+    first = {}
+    full_pos = {}
     for k, (kind, m, s) in enumerate(it.tolist()):
-        assert 0 <= m < nm and 0 <= s < ns
-        d = pos_psi if kind == 1 else pos_step
-        assert (m, s) not in d
-        d[(m, s)] = k
-    assert len(pos_psi) == nm * ns and len(pos_step) == nm * ns
-    for (m, s), k in pos_step.items():
+        assert kind in (0, 1) and 0 <= m < nm and 0 <= s < ns
+        first.setdefault((m, s), k)
+        if kind == 0:
+            assert (m, s) not in full_pos
+            full_pos[(m, s)] = k
+    assert len(full_pos) == nm * ns
+    worst = 0
+    for (m, s), k in full_pos.items():
         for dm in (-1, 0, 1):
             for ds in (-1, 0, 1):
-                assert pos_psi[((m + dm) % nm, (s + ds) % ns)] < k
-    # step rows march through pencils of py rows along s
-    steps = [(m, s) for kind, m, s in it.tolist() if kind == 0]
+                mm, ss = m + dm, s + ds
+                if (not wrap_m and not 0 <= mm < nm) or (not wrap_s and not 0 <= ss < ns):
+                    continue
+                worst = max(worst, first[(mm % nm, ss % ns)] - k)
+    assert worst == lead
     p = max(1, min(py, nm))
-    expect = [(m, s) for m0 in range(0, nm, p) for s in range(ns) for m in range(m0, min(m0 + p, nm))]
-    assert steps == expect
+    # one plane of the pencil and its two edge rows; at the start of a pencil also the wrapped plane's PSI_ONLY items
+    assert lead <= 2 * p + 8
+    fulls = [(m, s) for kind, m, s in it.tolist() if kind == 0]
+    assert fulls == [(m, s) for m0 in range(0, nm, p) for s in range(ns) for m in range(m0, min(m0 + p, nm))]
+    n_psi_only = len(it) - nm * ns
+    pencils = -(-nm // p)
+    assert n_psi_only <= pencils * (2 * ns + 2 * (p + 2)) + 2
