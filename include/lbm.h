@@ -156,12 +156,13 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *                       of the fused step kernel per time step, preceded by the psi pass for Shan-Chen models
  *                       (which reads the flow populations a second time).  Works for every shape and boundary.
  *   LBM_PATH_PIPELINE   Shan-Chen models: ONE persistent, warp-specialised launch per time step (tile.cuh).  A block
- *                       bulk-copies the populations of a 128-cell row segment into shared memory (cp.async.bulk +
- *                       mbarrier, a ring of stages), computes and publishes its psi (step a2), keeps the tile in
- *                       shared memory until the psi of the tiles around it has been published by their owners
- *                       (Eq. 11 / 13 need psi of all neighbours at the same time level: PAPER.md:128, 136; R9), then
- *                       collides and streams it (a1, a3-a8) from shared memory, two fp32 cells per thread in packed
- *                       arithmetic: every population crosses HBM once per step in each direction.  Needs
+ *                       copies the populations of a 128-cell row segment and the psi rows around it into shared
+ *                       memory (cp.async + mbarrier, a ring of stages) and collides and streams it (a1, a3-a8) from
+ *                       there, two fp32 cells per thread in packed arithmetic; psi of the NEXT time level (step a2;
+ *                       Eq. 11 / 13 need psi of all neighbours at one time level: PAPER.md:128, 136; R9) is formed by
+ *                       trailing psi warps of the same launch as soon as the step of the tiles around a tile is
+ *                       complete, from populations still in L2, into a second psi buffer (allocated by the library,
+ *                       S * N values): every population crosses HBM once per step in each direction.  Needs
  *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing and no solid-node mask (LBM_EINVAL
  *                       otherwise); walls in y / z are handled.
  * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a Shan-Chen
@@ -174,11 +175,12 @@ int lbm_set_path(lbm_ctx* ctx, int path, int rows_per_pencil);
 int lbm_get_path(const lbm_ctx* ctx);
 
 /* The row schedule of LBM_PATH_PIPELINE for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1, ns = ny;
- * wrap_m / wrap_s: that axis is periodic): *count items; if items != NULL (HOST, capacity items of 3 int32: kind
- * 0 = full life cycle of the row / 1 = psi only, m, s) they are written out; *lead_rows (optional) receives the
- * largest distance from a full item to a later item that provides psi it needs.  Host-only, needs no GPU. */
+ * wrap_m / wrap_s: that axis is periodic): *count = 2 * nm * ns items; if items != NULL (HOST, capacity items of 3
+ * int32: kind 0 = step of the row / 1 = psi of the next time level of the row, m, s) they are written out: every
+ * step row in pencil order, followed by the psi rows whose last dependency it is.  *deferred_rows (optional)
+ * receives the number of psi rows that wait for another pencil (re-read from HBM).  Host-only, needs no GPU. */
 int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
-                      size_t* count, int* lead_rows);
+                      size_t* count, int* deferred_rows);
 
 /* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a bounded wait of LBM_PATH_PIPELINE
  * timed out; lbm_run_host performs the same check before it returns). */

@@ -22,7 +22,7 @@ struct Ops {
     // resident-tile persistent kernel of the Shan-Chen models (tile.cuh); walls: bounce-back walls in y and / or z
     cudaError_t (*tile)(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st);
     int (*tile_blocks)(int model, int parity, int walls);     // co-resident blocks on the current device
-    int (*tile_stages)();                                     // stages per block (tiles kept in shared memory)
+    int (*tile_tx)();                                         // cells per tile
 };
 
 const Ops* ops_f64_d2q9();

@@ -7,12 +7,6 @@
 
 namespace lbm {
 
-// stages (tiles in flight) per block of the resident-tile kernel
-#ifndef LBM_TILE_NS
-#define LBM_TILE_NS 3
-#endif
-constexpr int TILE_NS = LBM_TILE_NS;
-
 // threads per block: 128 (64 and 256 measured within 1 % for BGK, 256 slower for Shan-Chen), less for short rows
 template <class R>
 inline int block_for(const KP<R>& p) {
@@ -187,10 +181,10 @@ struct Launch {
     // resident-tile kernel (tile.cuh): wa == nullptr -> only return the number of co-resident blocks through *out_blocks
     template <int MODEL, bool WALLYZ>
     static cudaError_t tile3(const KP<R>& p, int parity, const TileArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
-        using C = TileCfg<R, L, MODEL, TILE_NS>;
+        using C = TileCfg<R, L, MODEL>;
         constexpr size_t smem = C::SMEM;
-        auto k0 = k_tile<R, L, MODEL, 0, WALLYZ, TILE_NS>;
-        auto k1 = k_tile<R, L, MODEL, 1, WALLYZ, TILE_NS>;
+        auto k0 = k_tile<R, L, MODEL, 0, WALLYZ>;
+        auto k1 = k_tile<R, L, MODEL, 1, WALLYZ>;
         auto k = parity ? k1 : k0;
         // per device and context, cheap: set on every call
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -226,10 +220,10 @@ struct Launch {
         if (tile_any(&dummy, model, parity, walls, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
         return b;
     }
-    static int tile_stages() { return TILE_NS; }
+    static int tile_tx() { return TILE_ROW_BYTES / (int)sizeof(R); }
 
     static const Ops* ops() {
-        static const Ops o = {&psi, &step, &macros, &permute, &init, &tile, &tile_blocks, &tile_stages};
+        static const Ops o = {&psi, &step, &macros, &permute, &init, &tile, &tile_blocks, &tile_tx};
         return &o;
     }
 };

@@ -296,20 +296,26 @@ struct CellMacro {
     R inv_rho;
 };
 
-// steps a1, a3 (given the stencil sums), a4: moments, force, barycentric velocity (rows a1-a4).
+// step a1: rho^s, j^s of every component (row a1)
+template <class V, class L, int MODEL>
+__device__ __forceinline__ void cell_moments(const V (*fl)[L::Q], CellMacro<V, L, MODEL>& m) {
+    constexpr int S = ModelTraits<MODEL>::S;
+    static_for<0, S>([&](auto sc) {
+        constexpr int s = decltype(sc)::value;
+        m.j[s][0] = m.j[s][1] = m.j[s][2] = vconst<V>(0.0);
+        moments<L>(fl[s], m.rho[s], m.j[s]);
+    });
+}
+
+// steps a3 (given the stencil sums), a4: force, barycentric velocity from the moments in m (rows a3-a4).
 // acc[t][a] = sum_{i>=1} w_i psi^t(x + c_i) c_{i,a} and psi_own[s] = psi^s(x) are read only for Shan-Chen models.
 // V: value type (scalar, or two fp32 cells), T: its scalar type.
 template <class V, class L, int MODEL, bool FORCED, bool ADH = false, class T>
-__device__ __forceinline__ void cell_macros_core(const KP<T>& p, const V (*fl)[L::Q], const V (*acc)[3], const V* psi_own,
-                                                 CellMacro<V, L, MODEL>& m, const V* adh = nullptr) {
+__device__ __forceinline__ void cell_force_velocity(const KP<T>& p, const V (*acc)[3], const V* psi_own,
+                                                    CellMacro<V, L, MODEL>& m, const V* adh = nullptr) {
     constexpr int S = ModelTraits<MODEL>::S, D = L::D;
     constexpr bool SC = ModelTraits<MODEL>::SC;
     V (&j)[S][3] = m.j;
-    static_for<0, S>([&](auto sc) {
-        constexpr int s = decltype(sc)::value;
-        j[s][0] = j[s][1] = j[s][2] = vconst<V>(0.0);
-        moments<L>(fl[s], m.rho[s], j[s]);
-    });
     V rho_t = m.rho[0];
     if constexpr (S == 2) rho_t = rho_t + m.rho[1];
     m.inv_rho = vrecip(rho_t);
@@ -350,6 +356,14 @@ __device__ __forceinline__ void cell_macros_core(const KP<T>& p, const V (*fl)[L
             m.u[a] = jt * m.inv_rho;
         }
     });
+}
+
+// steps a1, a3 (given the stencil sums), a4 from the populations of the cell
+template <class V, class L, int MODEL, bool FORCED, bool ADH = false, class T>
+__device__ __forceinline__ void cell_macros_core(const KP<T>& p, const V (*fl)[L::Q], const V (*acc)[3], const V* psi_own,
+                                                 CellMacro<V, L, MODEL>& m, const V* adh = nullptr) {
+    cell_moments<V, L, MODEL>(fl, m);
+    cell_force_velocity<V, L, MODEL, FORCED, ADH>(p, acc, psi_own, m, adh);
 }
 
 // steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field in global memory

@@ -17,6 +17,11 @@
 
 namespace {
 
+// rows per pencil of the resident-tile schedule unless the caller chooses (lbm_set_path)
+#ifndef LBM_TILE_DEFAULT_PY
+#define LBM_TILE_DEFAULT_PY 32
+#endif
+
 thread_local std::string g_err;
 #ifdef LBM_TILE_TRACE
 long long* g_trace = nullptr;
@@ -138,11 +143,14 @@ struct lbm_ctx {
     cudaGraphExec_t graph_exec;
     cudaStream_t graph_capture_stream;
     bool graph_failed;
-    // resident-tile path (tile.cuh): schedule, flags
-    int tile_py, tile_lead;           // rows per pencil in use; lead of the schedule in tickets
+    // resident-tile path (tile.cuh): schedule, flags, second psi buffer
+    int tile_py;                      // rows per pencil in use
     int tile_blocks;                  // blocks per launch
-    lbm::TileItem* tile_items;        // device copy of the schedule, one entry per ticket
-    long long tile_n_items;
+    lbm::TileItem* tile_items;        // device copy of the schedule: the STEP tickets, then the PSI tickets
+    long long tile_n_items;           // tiles = STEP tickets = PSI tickets
+    void* psi_ws;                     // the psi buffer inside the workspace
+    void* psi_alt;                    // the psi buffer the resident-tile kernel writes psi(t + 1) to (swapped with psi after every launch)
+    int64_t psi_t;                    // time level of the values in psi (-1: none)
     int tile_nxs;
     int* tile_flags;                  // one int per tile, then the status word
     size_t tile_n_tiles;
@@ -245,13 +253,26 @@ int run_psi(lbm_ctx* c) {
     if (rc) return rc;
     CK(c->ops->psi(c->kp(), c->model, (int)(c->t & 1), c->wmode(), c->stream));
     c->launches++;
+    c->psi_t = c->t;
     return mark(c, 1);
+}
+
+void set_psi(lbm_ctx* c, void* psi) {
+    c->psi = psi;
+    c->kp64.psi = (double*)psi;
+    c->kp32.psi = (float*)psi;
 }
 
 void tile_free(lbm_ctx* c) {
     if (c->tile_items) cudaFree(c->tile_items);
     if (c->tile_flags) cudaFree(c->tile_flags);
-    c->tile_items = nullptr; c->tile_flags = nullptr;
+    if (c->psi_alt) {
+        // psi and psi_alt swap after every launch: free whichever of the two is not the workspace buffer
+        void* extra = c->psi == c->psi_ws ? c->psi_alt : c->psi;
+        if (c->psi != c->psi_ws) { set_psi(c, c->psi_ws); c->psi_t = -1; }
+        cudaFree(extra);
+    }
+    c->tile_items = nullptr; c->tile_flags = nullptr; c->psi_alt = nullptr;
     c->path = LBM_PATH_REGISTER;
 }
 
@@ -266,53 +287,49 @@ const char* tile_ineligible(const lbm_ctx* c) {
     return nullptr;
 }
 
-// Switch to the resident-tile path: build the schedule (one entry per ticket) and the flags; py <= 0 picks the default
+// Switch to the resident-tile path: build the schedule (one STEP and one PSI entry per tile), the flags and the
+// second psi buffer; py <= 0 picks the default
 int path_setup(lbm_ctx* c, int py) {
     CK(cudaStreamSynchronize(c->stream));
     tile_free(c);
     const Shape& sh = c->sh;
     const int nm = sh.d == 3 ? c->ny : 1, ns = sh.d == 3 ? c->nz : c->ny;
     const bool wrap_m = sh.d == 3 ? c->p.bc[1] == 0 : true, wrap_s = sh.d == 3 ? c->p.bc[2] == 0 : c->p.bc[1] == 0;
-    const int nxs = (c->nx + lbm::TILE_TX - 1) / lbm::TILE_TX;
+    const int tx = c->ops->tile_tx();
+    const int nxs = (c->nx + tx - 1) / tx;
     const int walls = c->bc_walls ? 1 : 0;
     int resident = c->ops->tile_blocks(c->model, 0, walls);
     const int r1 = c->ops->tile_blocks(c->model, 1, walls);
     if (r1 < resident) resident = r1;
     if (resident < 1) return fail(LBM_ECUDA, "resident-tile kernel: occupancy query failed");
-    const int stages = c->ops->tile_stages();
-    // default pencil: the psi a step waits for is about one stage of tickets ahead (tile.cuh: LEAD <= (NS - 1) * B)
-    if (py <= 0) py = resident / nxs - 2;
+    // default pencil: one plane of the pencil (what the psi pass trails the step by) stays far below the L2 capacity
+    if (py <= 0) py = LBM_TILE_DEFAULT_PY;
     if (py < 1) py = 1;
     if (py > nm) py = nm;
-    std::vector<lbm::TileRow> rows;
-    int blocks = 0;
-    long long lead_tickets = 0;
-    for (;;) {
-        int lead_rows = 0;
-        rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, &lead_rows);
-        const long long n_items = (long long)rows.size() * nxs;
-        blocks = (long long)resident < n_items ? resident : (int)n_items;
-        lead_tickets = ((long long)lead_rows + 1) * nxs;      // x-neighbours of the last needed row included
-        if (lead_tickets <= (long long)(stages - 1) * blocks) break;
-        if (py == 1) return fail(LBM_EINVAL, "resident-tile kernel: the grid is too wide for the pipeline depth of this device");
-        py = py / 2;
-    }
-    if ((double)rows.size() * nxs > 2.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 2e9 tickets");
-    std::vector<lbm::TileItem> items;
-    items.reserve(rows.size() * (size_t)nxs);
+    const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, nullptr);
+    const size_t n_tiles = (size_t)nm * ns * nxs;
+    if ((double)n_tiles > 2.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 2e9 tiles");
+    std::vector<lbm::TileItem> items(2 * n_tiles);
+    size_t k_step = 0, k_psi = n_tiles;
     for (const lbm::TileRow& r : rows) {
         lbm::TileItem it;
-        it.kind = r.kind;
         it.y = sh.d == 3 ? r.m : r.s;
         it.z = sh.d == 3 ? r.s : 0;
-        for (int xs = 0; xs < nxs; ++xs) { it.xs = xs; items.push_back(it); }
+        it.pad = 0;
+        for (int xs = 0; xs < nxs; ++xs) {
+            it.xs = xs;
+            if (r.kind == lbm::TILE_STEP) items[k_step++] = it; else items[k_psi++] = it;
+        }
     }
-    c->tile_py = py; c->tile_lead = (int)lead_tickets; c->tile_blocks = blocks;
-    c->tile_n_items = (long long)items.size();
+    if (k_step != n_tiles || k_psi != 2 * n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
+    c->tile_py = py;
+    c->tile_blocks = (long long)resident < (long long)n_tiles ? resident : (int)n_tiles;
+    c->tile_n_items = (long long)n_tiles;
     c->tile_nxs = nxs;
-    c->tile_n_tiles = (size_t)nm * ns * nxs;
+    c->tile_n_tiles = n_tiles;
     cudaError_t e = cudaMalloc((void**)&c->tile_items, items.size() * sizeof(lbm::TileItem));
     if (e == cudaSuccess) e = cudaMalloc((void**)&c->tile_flags, (c->tile_n_tiles + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&c->psi_alt, sh.psi_bytes);
     if (e != cudaSuccess) { cudaGetLastError(); tile_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
     CK(cudaMemcpyAsync(c->tile_items, items.data(), items.size() * sizeof(lbm::TileItem), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemsetAsync(c->tile_flags, 0, (c->tile_n_tiles + 1) * sizeof(int), c->stream));
@@ -324,25 +341,37 @@ int path_setup(lbm_ctx* c, int py) {
 
 int run_tile(lbm_ctx* c) {
     const int parity = (int)(c->t & 1);
+    if (c->psi_t != c->t) {              // first step on this path (or after new populations): psi(t) by the psi pass
+        int rc = run_psi(c);
+        if (rc) return rc;
+    }
     if (c->tile_epoch == 0x7fffffff) {   // epoch wrap: clear the flags (once per 2^31 - 1 launches)
         CK(cudaMemsetAsync(c->tile_flags, 0, c->tile_n_tiles * sizeof(int), c->stream));
         c->tile_epoch = 0;
     }
     lbm::TileArgs wa;
-    wa.items = c->tile_items;
+    wa.step_items = c->tile_items;
+    wa.psi_items = c->tile_items + c->tile_n_items;
     wa.n_items = (unsigned)c->tile_n_items;
     wa.nxs = c->tile_nxs;
     wa.flags = c->tile_flags;
     wa.epoch = ++c->tile_epoch;
     wa.status = c->tile_flags + c->tile_n_tiles;
+    wa.psi_out = c->psi_alt;
 #ifdef LBM_TILE_TRACE
-    if (!g_trace) { cudaMalloc((void**)&g_trace, sizeof(long long) * 10 * 4096); cudaMemset(g_trace, 0, sizeof(long long) * 10 * 4096); }
+    if (!g_trace) cudaMalloc((void**)&g_trace, sizeof(long long) * (10 * 4096 + 2 * 160 * 1024));
+    cudaMemsetAsync(g_trace, 0, sizeof(long long) * (10 * 4096 + 2 * 160 * 1024), c->stream);
     wa.trace = g_trace;
 #endif
     int rc = mark(c, 0);
     if (rc) return rc;
     CK(c->ops->tile(c->kp(), c->model, parity, c->bc_walls ? 1 : 0, &wa, c->tile_blocks, c->stream));
     c->launches++;
+    // the launch has written psi(t + 1) to psi_alt: it is the current buffer from now on
+    void* cur = c->psi;
+    set_psi(c, c->psi_alt);
+    c->psi_alt = cur;
+    c->psi_t = c->t + 1;
     return mark(c, 0);
 }
 
@@ -351,7 +380,9 @@ int tile_status(lbm_ctx* c) {
     if (c->path == LBM_PATH_REGISTER) return 0;
     int st = 0;
     CK(cudaMemcpy(&st, c->tile_flags + c->tile_n_tiles, sizeof(int), cudaMemcpyDeviceToHost));
-    if (st != 0) return fail(LBM_ECUDA, "resident-tile kernel: a wait for published psi timed out; the state is invalid");
+    if (st != 0)
+        return fail(LBM_ECUDA, "resident-tile kernel: a bounded wait timed out (bits: 1 stage load, 2 free stage, 4 publisher, 8 flags of the "
+                               "tiles around a psi tile): " + std::to_string(st) + "; the state is invalid");
     return 0;
 }
 
@@ -399,7 +430,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->timing = false;
     c->graph_exec = nullptr; c->graph_capture_stream = nullptr; c->graph_failed = false;
     c->path = LBM_PATH_REGISTER; c->tile_items = nullptr; c->tile_flags = nullptr;
-    c->tile_py = c->tile_lead = 0; c->tile_blocks = 0; c->tile_epoch = 0; c->path_user_set = false;
+    c->tile_py = 0; c->tile_blocks = 0; c->tile_epoch = 0; c->path_user_set = false;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
         if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
@@ -418,6 +449,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->f = c->ws;
     c->h = sh.scalar ? c->ws + sh.f_bytes : nullptr;
     c->psi = sh.sc ? c->ws + sh.f_bytes + sh.h_bytes : nullptr;
+    c->psi_ws = c->psi; c->psi_alt = nullptr; c->psi_t = -1;
     c->bc_walls = p->bc[0] || p->bc[1] || p->bc[2];
     c->walls = c->bc_walls;
     c->moving = false;
@@ -473,6 +505,7 @@ int lbm_init_from_seed(lbm_ctx* c, uint64_t seed) {
     c->launches++;
     c->inited = true;
     c->t = 0;
+    c->psi_t = -1;
     return 0;
 }
 
@@ -564,7 +597,7 @@ int lbm_get_macros(lbm_ctx* c, void* rho, void* u, void* phi, void* C) {
     if (!c->inited) return fail(LBM_ESTATE, "lbm_get_macros before init");
     if (C && !c->sh.scalar) return fail(LBM_EINVAL, "model has no scalar lattice");
     DeviceGuard g(c->device);
-    if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
+    if (c->sh.sc && c->psi_t != c->t) { int rc = run_psi(c); if (rc) return rc; }
     CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->wmode(), rho, u, phi, C, nullptr, c->stream));
     c->launches++;
     return 0;
@@ -575,7 +608,7 @@ int lbm_get_force(lbm_ctx* c, void* F) {
     if (!c->inited) return fail(LBM_ESTATE, "lbm_get_force before init");
     if (!F) return fail(LBM_EINVAL, "F is NULL");
     DeviceGuard g(c->device);
-    if (c->sh.sc) { int rc = run_psi(c); if (rc) return rc; }
+    if (c->sh.sc && c->psi_t != c->t) { int rc = run_psi(c); if (rc) return rc; }
     CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->wmode(), nullptr, nullptr, nullptr, nullptr, F, c->stream));
     c->launches++;
     return 0;
@@ -609,6 +642,7 @@ int lbm_set_populations(lbm_ctx* c, const void* f) {
     if (c->sh.scalar) CK(cudaMemcpyAsync(c->h, (const char*)f + nf, nh, cudaMemcpyDeviceToDevice, c->stream));
     c->inited = true;
     c->t = 0;
+    c->psi_t = -1;
     return 0;
 }
 
@@ -624,6 +658,7 @@ int lbm_run_host(lbm_ctx* c, const void* f_in_host, int n, void* rho_h, void* u_
         if (sh.scalar) CK(cudaMemcpyAsync(c->h, (const char*)f_in_host + nf, nh, cudaMemcpyHostToDevice, c->stream));
         c->inited = true;
         c->t = 0;
+        c->psi_t = -1;
     }
     if (!c->inited) return fail(LBM_ESTATE, "lbm_run_host without populations");
     int rc = lbm_step(c, n);
@@ -703,19 +738,20 @@ int lbm_set_mask(lbm_ctx* c, const unsigned char* mask) {
     if (mask && c->path != LBM_PATH_REGISTER) tile_free(c);     // a solid-node mask runs on LBM_PATH_REGISTER only
     c->kp64.mask = mask;
     c->kp32.mask = mask;
+    c->psi_t = -1;
     c->walls = c->bc_walls || mask != nullptr;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // the graph holds the old parameters
     return 0;
 }
 
 int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
-                      size_t* count, int* lead_rows) {
+                      size_t* count, int* deferred_rows) {
     if (!count) return fail(LBM_EINVAL, "count is NULL");
     if (nm < 1 || ns < 1) return fail(LBM_EINVAL, "nm and ns must be >= 1");
-    int lead = 0;
-    const std::vector<lbm::TileRow> v = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, &lead);
+    int deferred = 0;
+    const std::vector<lbm::TileRow> v = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, &deferred);
     *count = v.size();
-    if (lead_rows) *lead_rows = lead;
+    if (deferred_rows) *deferred_rows = deferred;
     if (items) {
         if (capacity < v.size()) return fail(LBM_EINVAL, "capacity too small");
         for (size_t k = 0; k < v.size(); ++k) {
@@ -735,7 +771,15 @@ int lbm_check(lbm_ctx* c) {
 }
 
 #ifdef LBM_TILE_TRACE
+int lbm_debug_flags(lbm_ctx* c, int* out, size_t cap, int* epoch, int* blocks) {
+    cudaDeviceSynchronize();
+    *epoch = c->tile_epoch; *blocks = c->tile_blocks;
+    size_t n = c->tile_n_tiles + 1 < cap ? c->tile_n_tiles + 1 : cap;
+    cudaMemcpy(out, c->tile_flags, n * sizeof(int), cudaMemcpyDeviceToHost);
+    return (int)n;
+}
 int lbm_debug_trace(void* out) { return (int)cudaMemcpy(out, g_trace, sizeof(long long) * 10 * 4096, cudaMemcpyDeviceToHost); }
+int lbm_debug_marks(void* out) { return (int)cudaMemcpy(out, g_trace + 10 * 4096, sizeof(long long) * 2 * 160 * 1024, cudaMemcpyDeviceToHost); }
 #endif
 
 int64_t lbm_time(const lbm_ctx* c) { return c ? c->t : -1; }

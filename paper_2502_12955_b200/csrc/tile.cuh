@@ -1,31 +1,30 @@
 // Resident-tile kernel of the Shan-Chen models (sm_100a): ONE persistent, warp-specialised launch per time step in
-// which every population crosses HBM once in each direction and is read from L2 once.
+// which every population crosses HBM once in each direction.
 //
 // The problem: Eq. 11 / 13 need psi(x + c_i, t) of all neighbours before cell x
-// is collided (R9), and with in-place streaming a cell's populations can only be read before its own step
-// overwrites them.  Two launches (k_psi, k_step) read the flow populations twice from HBM.  Here a block keeps the
-// populations of a tile of TILE_TX cells of one x-row in SHARED MEMORY between the two uses:
+// is collided (R9), and rho(x, t + 1) = sum_i f*_i(x - c_i, t) (Eq. 5 / 7) needs the step of all neighbours.  Two
+// launches per time step (k_psi, k_step) read the flow populations twice from HBM.  Here the psi pass of time level
+// t + 1 TRAILS the step of time level t inside the same launch, a few rows behind it, so that it reads the
+// populations the step has just written while they are still in L2 (126 MB):
 //
-//   producer warp   bulk-copies (cp.async.bulk -> UBLKCP, completion on an mbarrier) the S*Q + Q_s slot rows P_i(x) of
-//                   the tile into the next free stage of a ring of NS stages; at odd parity a row comes from the
+//   producer warp   copies (16-byte cp.async, LDGSTS.128) the S*Q + Q_s slot rows P_i(x) of a 128-cell tile and the
+//                   psi(t) rows around it (3 x 3 rows per component, with a one-cell halo in x) into the next free
+//                   stage of a ring of NS shared-memory stages; at odd parity a population row comes from the
 //                   neighbour row (y - c_y, z - c_z) and is shifted by -c_x, so it is the aligned segment plus the
-//                   16-byte piece left or right of it.  One lane issues a row: no registers, no per-cell instructions.
-//   psi warp        step a2: rho^sigma in index order (Eq. 7 / 18) from the stage, psi^sigma (Eq. 10 / 24 or psi = rho)
-//                   to global memory, then publishes the tile's flag (st.release.gpu, launch epoch).
-//   halo warp       waits (ld.acquire.gpu) for the flags of the up to 27 tiles around the tile -- published by the
-//                   blocks that own them -- and copies the psi rows with their one-cell halo from L2 (cp.async.cg, never a stale L1 line) into one of TILE_NHB
-//                   shared-memory halo buffers, without waiting for the copies.
-//   step warps      steps a1, a3-a8: populations from the stage, psi stencil from the halo buffer, collide, store to
-//                   the global slots the rows came from; in fp32 every thread owns TWO cells and runs the packed
-//                   f32x2 instantiation (V = F2) of the cell arithmetic.
+//                   16-byte piece left or right of it.  No registers, no per-cell instructions.
+//   step warps      steps a1, a3-a8 from the stage: moments, psi stencil, force, collide, store to the global slots
+//                   the rows came from; in fp32 every thread owns TWO cells and runs the packed f32x2 instantiation
+//                   (V = F2) of the cell arithmetic.  They never wait for another block.
+//   publisher warp  once all step warps have stored a tile: fence, then the tile's flag (launch epoch) in global memory.
+//   psi warps       step a2 for t + 1: wait (acquire) for the flags of the up to 27 tiles around a tile, then rho^sigma
+//                   in index order (Eq. 7 / 18) from the slots of the NEXT parity (ld.global.cg: L2, never a stale L1
+//                   line) and psi^sigma (Eq. 10 / 24 or psi = rho) to the second psi buffer, which the next launch reads.
 //
-// Work distribution is static: block b owns the tickets b, b + B, b + 2B, ... of the host-built schedule
-// (tile_schedule.h; one ticket = one tile), so every warp knows its items without communication.  Deadlock freedom:
-// producer and psi warp never wait for another block (only for free stages and landed copies), the step of the
-// globally lowest unreleased ticket g needs psi of tickets <= g + LEAD only, and every block keeps NS stages, i.e.
-// its next NS tickets, loaded: with LEAD <= (NS - 1) * B all those tickets are in a stage, their psi gets published,
-// and ticket g proceeds.  The host checks that inequality (lbm_set_path) and launches at most as many blocks as
-// are co-resident.  Every wait is bounded (clock64); a timeout sets *status and gives up instead of hanging the GPU.
+// Work distribution is static: block b owns the STEP tickets b, b + B, ... and psi worker w the PSI tickets w, w + W,
+// ... of the host-built lists (tile_schedule.h; one ticket = one tile).  Deadlock freedom: producer, step warps and
+// publisher wait only inside their block (free stage, landed copy, stored tile); only the psi warps wait for other
+// blocks, and nothing waits for a psi warp.  The host launches at most as many blocks as are co-resident.  Every
+// wait is bounded (clock64); a timeout sets *status and gives up instead of hanging the GPU.
 //
 // Requirements (else the two-launch path runs): periodic x, nx * sizeof(R) a multiple of 16 bytes, no solid mask,
 // Guo forcing.  Walls in y / z are uniform per row and handled here: rows beyond a wall are redirected to the
@@ -36,39 +35,37 @@
 
 namespace lbm {
 
-constexpr int TILE_TX = 128;          // cells per tile
-// how the producer warp moves a row: 16-byte cp.async (LDGSTS.128) per lane, or one cp.async.bulk (UBLKCP) per row.
-// The bulk form is the measured-and-rejected alternative (the per-SM request rate of 512-byte bulk
-// copies bounds the kernel at about 1 TB/s); build with -DLBM_TILE_BULK=1 to reproduce it.
-#ifndef LBM_TILE_BULK
-#define LBM_TILE_BULK 0
+constexpr int TILE_ROW_BYTES = 1024;  // bytes of one row segment of a tile: 256 fp32 / 128 fp64 cells (one bulk copy)
+constexpr int TILE_PROD_WARPS = 2;    // producer warps per block (each issues the bulk copies of half the rows)
+// psi warps per block.  With two teams of four step warps, two producers and the publisher that makes 15 warps = 480
+// threads of up to 136 registers: 16 warps of 128 registers would claim the whole register file of the SM, and a
+// launch of one such block per SM was observed NOT to be fully co-resident (the psi warps then wait for tiles of a
+// block that has not started).
+#ifndef LBM_TILE_PSIW
+#define LBM_TILE_PSIW 4
 #endif
-constexpr bool TILE_BULK = LBM_TILE_BULK != 0;
-constexpr int TILE_AUX_WARPS = 3;     // producer, psi, halo
-#ifndef LBM_TILE_NHB
-#define LBM_TILE_NHB 3
-#endif
-constexpr int TILE_NHB = LBM_TILE_NHB;   // psi halo buffers per block (the halo warp runs that many tiles ahead of the step warps)
 
 struct TileItem {
-    int kind, xs, y, z;               // TILE_FULL / TILE_PSI_ONLY, x-segment, row
+    int xs, y, z, pad;                // x-segment, row
 };
 
 struct TileArgs {
-    const TileItem* items;            // the schedule of one time step, one entry per ticket (device)
-    unsigned n_items;
+    const TileItem* step_items;       // the STEP tickets of one time step (device)
+    const TileItem* psi_items;        // the PSI tickets, in the order they become ready
+    unsigned n_items;                 // tiles = STEP tickets = PSI tickets
     int nxs;                          // tiles per row
-    int* flags;                       // one per tile (z, y, xs): launch epoch of the last published psi
+    int* flags;                       // one per tile (z, y, xs): launch epoch of the last completed step
     int epoch;                        // > 0, differs from every earlier launch since the flags were cleared
     int* status;                      // set to 1 if a wait timed out
+    void* psi_out;                    // psi(t + 1): S * N values, not the buffer KP::psi points at
 #ifdef LBM_TILE_TRACE
     long long* trace;
 #endif
 };
 
 #ifdef LBM_TILE_TRACE
-// developer trace: time stamps of block 0's roles per item (0 issue, 1 full seen by psi, 2 psi published, 3 flags ok,
-// 4 halo issued, 5 step start, 6 step end, 7 empty seen by the producer)
+// developer trace: time stamps of block 0's roles per ticket (0 copies issued, 1 stage full seen by the step warps,
+// 2 flag published, 3 flags seen by psi warp 0, 4 psi stored, 5 step start, 6 step end, 7 free stage seen by the producer)
 __device__ __forceinline__ void tile_trace(long long* buf, int what, unsigned n) {
     if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && n < 4096) {
         long long t;
@@ -77,39 +74,39 @@ __device__ __forceinline__ void tile_trace(long long* buf, int what, unsigned n)
     }
 }
 #define TILE_TRACE(what, n) tile_trace(w.trace, what, n)
+// per block and ticket marks: 0 stepped (count of warps), 1 published
+#define TILE_MARK(kind, n, v) do { if ((n) < 1024) atomicAdd((unsigned long long*)&w.trace[10 * 4096 + ((kind) * 160 + blockIdx.x) * 1024 + (n)], (unsigned long long)(v)); } while (0)
 #else
+#define TILE_MARK(kind, n, v)
 #define TILE_TRACE(what, n)
 #endif
 
 // ---- PTX helpers ----
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+// (LDG.STRONG.GPU + CCTL.IVALL: no MEMBAR, unlike a relaxed load followed by fence.acq_rel.gpu, which waits for the
+// warp's own outstanding stores)
 __device__ __forceinline__ int ld_acquire(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ int ld_relaxed(const int* p) {
-    int v;
-    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
+__device__ __forceinline__ void st_relaxed(int* p, int v) {
+    asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
-__device__ __forceinline__ void st_release(int* p, int v) {
-    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-__device__ __forceinline__ int4 ld_cg16(const void* p) {
-    int4 v;
-    asm volatile("ld.global.cg.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+__device__ __forceinline__ unsigned ld_acquire_cta_shared(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
     return v;
+}
+__device__ __forceinline__ void st_release_cta_shared(unsigned* p, unsigned v) {
+    asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 // (the suspend-time hint lets a waiting warp sleep in hardware instead of spinning on its scheduler's issue slots)
 constexpr unsigned TILE_SUSPEND_NS = 20000u;
@@ -127,14 +124,24 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long* bar, unsigned 
     return ok != 0;
 }
 constexpr long long TILE_TIMEOUT_CYCLES = 6000000000LL;     // ~3 s: far beyond any legitimate wait
-// bounded wait for the phase with the given parity; false (and *status = 1) on timeout
-__device__ __forceinline__ bool mbar_wait(unsigned long long* bar, unsigned parity, int* status) {
+// bounded wait for the phase with the given parity; false (and *status |= code) on timeout
+__device__ __forceinline__ bool mbar_wait(unsigned long long* bar, unsigned parity, int* status, int code) {
     if (mbar_try_wait(bar, parity)) return true;
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { *status = 1; return false; }
+        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(status, code); return false; }
     }
     return true;
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// global -> shared bulk copy by the TMA unit (bytes a multiple of 16, both addresses 16-byte aligned), completion
+// counted as transaction bytes on bar
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
 }
 // 16-byte asynchronous copy global -> shared (LDGSTS.128, L2 only) and its completion on an mbarrier: the barrier
 // receives one arrival from the executing thread once all its earlier cp.async have landed (.noinc: the arrival is
@@ -142,16 +149,14 @@ __device__ __forceinline__ bool mbar_wait(unsigned long long* bar, unsigned pari
 // (no "memory" clobber: ordinary loads of the row tables may be scheduled across the copies; ordering against the
 // consumers comes from the mbarrier operations, which do clobber memory)
 __device__ __forceinline__ void cp_async16(unsigned dst, const void* src) {
+#ifdef LBM_TILE_CA
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+#else
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
+#endif
 }
 __device__ __forceinline__ void cp_async_arrive(unsigned long long* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-// global -> shared bulk copy (bytes a multiple of 16, both addresses 16-byte aligned), completion counted on bar
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
-                 "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
 }
 
 // stores through an address read from shared memory: say "global" (a generic ST would check the address space)
@@ -171,14 +176,9 @@ __device__ __forceinline__ int c_runtime(int i) {
     constexpr unsigned long long pk = packed_axis<LL>(A);
     return (int)((pk >> (2 * i)) & 3ULL) - 1;
 }
-template <class LL>
-__host__ __device__ constexpr int count_x_shifted() {
-    int n = 0;
-    for (int i = 0; i < LL::Q; ++i) n += LL::c(i, 0) != 0;
-    return n;
-}
 
-template <class R, class L, int MODEL, int NS>
+// One block per SM (__launch_bounds__(THREADS, 1)): the stages fill the shared memory, the warps the register file.
+template <class R, class L, int MODEL>
 struct TileCfg {
     using MT = ModelTraits<MODEL>;
     using LS = typename ScalarOf<L>::type;
@@ -187,51 +187,61 @@ struct TileCfg {
     static constexpr int CPT = PACK ? 2 : 1;
     static constexpr int S = MT::S, Q = L::Q, D = L::D;
     static constexpr int B = (int)sizeof(R);
+    static constexpr int TX = TILE_ROW_BYTES / B;                // cells per tile
     static constexpr int H = 16 / B;                             // elements per 16-byte piece = halo width
-    static constexpr int RS = TILE_TX + 2 * H;                   // elements per shared-memory row: [piece | segment | piece]
+    static constexpr int RS = TX + 2 * H;                        // elements per shared-memory row: [piece | segment | piece]
     static constexpr int NF = S * Q;
     static constexpr int NH = MT::SCALAR ? LS::Q : 0;
     static constexpr int NPOPS = NF + NH;
     static constexpr int NPSI = D == 3 ? 9 : 3;                  // psi rows (dy, dz) per component
     static constexpr int NP = S * NPSI;
-    static constexpr int STEP_THREADS = TILE_TX / CPT;
+    static constexpr int NROWS = NPOPS + NP;                     // rows of a stage: populations, then psi
+    static constexpr int STEP_THREADS = TX / CPT;
     static constexpr int STEP_WARPS = STEP_THREADS / 32;
-    static constexpr int THREADS = 32 * TILE_AUX_WARPS + STEP_THREADS;
-    static constexpr size_t STAGE_BYTES = (size_t)NPOPS * RS * B;
-    static constexpr size_t HALO_BYTES = (size_t)NP * RS * B;
-    static constexpr size_t ROWPTR_BYTES = (size_t)NS * NPOPS * sizeof(unsigned long long);
+    // Two teams of step warps work on two stages at a time (two warps per scheduler hide each other's latencies):
+    // 512 threads of at most 128 registers.  The step role of the D3Q19 models in fp64 needs more registers (19
+    // doubles per component and thread): one team, 256 threads.
+    static constexpr bool HEAVY = B == 8 && Q > 9;
+    static constexpr int TEAMS = HEAVY ? 1 : 2;
+    static constexpr int PSI_WARPS = HEAVY ? 1 : LBM_TILE_PSIW;
+    static constexpr int AUX_WARPS = PSI_WARPS + 1 + TILE_PROD_WARPS;      // psi, publisher, producers
+    static constexpr int THREADS = 32 * AUX_WARPS + TEAMS * STEP_THREADS;
+    static constexpr size_t STAGE_BYTES = (size_t)NROWS * RS * B;
+    static constexpr int NS = (215 * 1024) / STAGE_BYTES >= 6 ? 6 : (int)((215 * 1024) / STAGE_BYTES);   // stages
+    static constexpr size_t ROWPTR_BYTES = (size_t)NS * 64 * sizeof(unsigned long long);    // pointers of the (up to 64) rows of a stage
     static constexpr size_t ROWSX_BYTES = ((size_t)NS * NPOPS * sizeof(int) + 15) / 16 * 16;
-    static constexpr int NBAR = 3 * NS + 2 * TILE_NHB;
-    static constexpr size_t SMEM = NS * STAGE_BYTES + TILE_NHB * HALO_BYTES + ROWPTR_BYTES + ROWSX_BYTES + NBAR * 8;
-    __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
+    static constexpr int NBAR = 2 * NS;
+    static constexpr size_t SMEM = NS * STAGE_BYTES + ROWPTR_BYTES + ROWSX_BYTES + NBAR * 8 + 32;
+    static_assert(NROWS <= 32 * TILE_PROD_WARPS, "one row per producer lane");
+    static_assert(TEAMS * STEP_WARPS <= 8, "done counters");
+    static_assert(NS >= 2 && SMEM <= 227 * 1024, "shared memory");
+    __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return NPOPS + t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLYZ, int NS>
+template <class R, class L, int MODEL, int PARITY, bool WALLYZ>
 struct Tile {
-    using C = TileCfg<R, L, MODEL, NS>;
+    using C = TileCfg<R, L, MODEL>;
     using MT = typename C::MT;
     using LS = typename C::LS;
     using V = typename C::V;
     static constexpr int S = C::S, Q = C::Q, D = C::D, B = C::B, H = C::H, RS = C::RS, NF = C::NF, NPOPS = C::NPOPS, CPT = C::CPT;
+    static constexpr int NROWS = C::NROWS, NS = C::NS, TILE_TX = C::TX, TILE_PSI_WARPS = C::PSI_WARPS;
 
     const KP<R>& p;
     const TileArgs& w;
-    R* stages;                          // [NS][NPOPS][RS]
-    R* halo;                            // [TILE_NHB][NP][RS]
-    unsigned long long* rowptr;         // [NS][NPOPS]: global address of element x = 0 of the row staged there
+    R* stages;                          // [NS][NROWS][RS]
+    unsigned long long* rowptr;         // [NS][64]: global address of element x = 0 of the row staged there (0: none)
     int* rowsx;                         // [NS][NPOPS]: its x-shift (-1, 0, +1): cell x reads position H + (x - x0) + shift
-    unsigned long long *full, *psi_done, *empty, *halo_full, *halo_empty;
+    unsigned long long *full, *empty;
+    unsigned* done;                     // [TEAMS * STEP_WARPS]: tickets of its team that step warp k has stored
 
     __device__ __forceinline__ Tile(const KP<R>& kp, const TileArgs& wa, unsigned char* smem) : p(kp), w(wa) {
         stages = (R*)smem;
-        halo = (R*)(smem + NS * C::STAGE_BYTES);
-        rowptr = (unsigned long long*)(smem + NS * C::STAGE_BYTES + TILE_NHB * C::HALO_BYTES);
+        rowptr = (unsigned long long*)(smem + NS * C::STAGE_BYTES);
         rowsx = (int*)((unsigned char*)rowptr + C::ROWPTR_BYTES);
         full = (unsigned long long*)((unsigned char*)rowsx + C::ROWSX_BYTES);
-        psi_done = full + NS;
-        empty = psi_done + NS;
-        halo_full = empty + NS;
-        halo_empty = halo_full + TILE_NHB;
+        empty = full + NS;
+        done = (unsigned*)(empty + NS);
     }
     static __device__ __forceinline__ int wrap(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
     __device__ __forceinline__ bool wall_y() const { return WALLYZ && p.bc[1]; }
@@ -241,13 +251,22 @@ struct Tile {
         if constexpr (!WALLYZ) return false;
         return (wall_y() && (y + dy < 0 || y + dy >= p.ny)) || (wall_z() && (z + dz < 0 || z + dz >= p.nz));
     }
-    __device__ __forceinline__ TileItem item_of(unsigned ticket) const {
-        const int4 v = __ldg((const int4*)(w.items + ticket));
+    __device__ __forceinline__ bool edge_row(int y, int z) const {
+        return WALLYZ && ((wall_y() && (y == 0 || y == p.ny - 1)) || (wall_z() && (z == 0 || z == p.nz - 1)));
+    }
+    static __device__ __forceinline__ TileItem item_of(const TileItem* items, unsigned ticket) {
+        const int4 v = __ldg((const int4*)(items + ticket));
         return TileItem{v.x, v.y, v.z, v.w};
+    }
+    __device__ __forceinline__ int* flag_of(int xs, int y, int z) const {
+        const int nm = D == 3 ? p.ny : 1;
+        const int ms = D == 3 ? y : 0, ss = D == 3 ? z : y;
+        return w.flags + ((size_t)ss * nm + ms) * w.nxs + xs;
     }
 
     // ---------------- producer ----------------
-    // row r of a stage for an item at (y, z): slot array, source row, x-shift
+    // population row r of an item at (y, z) at the parity PAR: slot array, source row, x-shift
+    template <int PAR>
     __device__ __forceinline__ void row_source(int r, int y, int z, unsigned long long& base, int& sx) const {
         const size_t N = (size_t)p.N;
         int i, c0, c1, c2, op;
@@ -264,88 +283,80 @@ struct Tile {
         }
         int slot = i, yy = y, zz = z;
         sx = 0;
-        if (PARITY == 1 && i != 0 && !crosses(y, z, -c1, -c2)) {
+        if (PAR == 1 && i != 0 && !crosses(y, z, -c1, -c2)) {
             // P_i(x) = slot opp(i) of cell x - c_i; beyond a bounce-back wall: slot i of x itself
             slot = op; yy = wrap(y - c1, p.ny); zz = D == 3 ? wrap(z - c2, p.nz) : 0; sx = -c0;
         }
         base = (unsigned long long)(arr + (size_t)slot * N + ((size_t)zz * p.ny + yy) * (size_t)p.nx);
     }
-    __device__ __forceinline__ void produce(unsigned n_mine, unsigned b0, unsigned stride) const {
+    // producer warp `pwid` looks after the rows r = 32 * pwid + lane of every stage
+    __device__ __forceinline__ void produce(int pwid, unsigned n_mine, unsigned b0, unsigned stride) const {
         const int lane = (int)(threadIdx.x & 31);
+        const int r = 32 * pwid + lane;
+        const size_t N = (size_t)p.N;
+        // where row r comes from relative to the item's row.  nbr: element 0 of row (0, 0) of the source array / slot;
+        // own: the same for the cell's own slot (a population row that would cross a wall; a psi row is left out)
+        const R* nbr = nullptr;
+        const R* own = nullptr;
+        int dy = 0, dz = 0, sx0 = 0;
+        if (r < NPOPS) {
+            int i, c0, c1, c2, op;
+            const R* arr;
+            if (r < NF) {
+                const int s = r / Q;
+                i = r - s * Q;
+                arr = p.f + (size_t)s * Q * N;
+                c0 = c_runtime<L, 0>(i); c1 = c_runtime<L, 1>(i); c2 = D == 3 ? c_runtime<L, 2>(i) : 0; op = L::opp(i);
+            } else {
+                i = r - NF;
+                arr = p.h;
+                c0 = c_runtime<LS, 0>(i); c1 = c_runtime<LS, 1>(i); c2 = D == 3 ? c_runtime<LS, 2>(i) : 0; op = LS::opp(i);
+            }
+            own = arr + (size_t)i * N;
+            nbr = own;
+            if (PARITY == 1 && i != 0) {       // P_i(x) = slot opp(i) of cell x - c_i; beyond a wall: slot i of x itself
+                nbr = arr + (size_t)op * N; dy = -c1; dz = -c2; sx0 = -c0;
+            }
+        } else if (r < NROWS) {
+            const int q0 = r - NPOPS, t = q0 / C::NPSI, q = q0 - t * C::NPSI;
+            dy = D == 3 ? q % 3 - 1 : q - 1; dz = D == 3 ? q / 3 - 1 : 0;
+            nbr = p.psi + (size_t)t * N;
+        }
         for (unsigned n = 0; n < n_mine; ++n) {
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
-            const TileItem it = item_of(b0 + n * stride);
-            if (!mbar_wait(&empty[stage], ph ^ 1u, w.status)) return;
-            TILE_TRACE(7, n);
+            const TileItem it = item_of(w.step_items, b0 + n * stride);
+            if (!mbar_wait(&empty[stage], ph ^ 1u, w.status, 2)) return;
+            if (pwid == 0) TILE_TRACE(7, n);
             const int x0 = it.xs * TILE_TX;
             const int len = min(TILE_TX, p.nx - x0);
-            const int nrows = it.kind == TILE_PSI_ONLY ? NF : NPOPS;
-            // bytes this stage will receive: nrows segments plus one 16-byte piece per x-shifted row
-            unsigned long long base[2] = {0, 0};
-            int sx[2] = {0, 0};
-            unsigned pieces = 0;
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                const int r = lane + 32 * k;
-                if (r < nrows) {
-                    row_source(r, it.y, it.z, base[k], sx[k]);
-                    rowptr[stage * NPOPS + r] = base[k];
-                    rowsx[stage * NPOPS + r] = sx[k];
-                    pieces += sx[k] != 0;
+            const R* src = nullptr;
+            int sx = 0;
+            if (r < NROWS) {
+                if (crosses(it.y, it.z, dy, dz)) {
+                    if (own) src = own + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx;
+                } else {
+                    const int yy = wrap(it.y + dy, p.ny), zz = D == 3 ? wrap(it.z + dz, p.nz) : 0;
+                    src = nbr + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
+                    sx = sx0;
                 }
+                rowptr[stage * 64 + r] = (unsigned long long)src;
+                if (r < NPOPS) rowsx[stage * NPOPS + r] = sx;
             }
-            pieces = __reduce_add_sync(0xffffffffu, pieces);
-            __syncwarp();                                  // the row tables of all lanes are written
-            TILE_TRACE(9, n);
-            if constexpr (TILE_BULK) {
-                // one cp.async.bulk (UBLKCP) per row and piece, completion as transaction bytes on the barrier
-                if (lane == 0) mbar_arrive_expect_tx(&full[stage], (unsigned)nrows * (unsigned)(len * B) + 16u * pieces);
-                __syncwarp();
-#pragma unroll
-                for (int k = 0; k < 2; ++k) {
-                    const int r = lane + 32 * k;
-                    if (r < nrows) {
-                        const unsigned dst = smem_u32(stages + ((size_t)stage * NPOPS + r) * RS);
-                        const char* g = (const char*)base[k];
-                        bulk_g2s(dst + H * B, g + (size_t)x0 * B, (unsigned)(len * B), &full[stage]);
-                        if (sx[k] < 0) bulk_g2s(dst, g + (size_t)(x0 == 0 ? p.nx - H : x0 - H) * B, 16u, &full[stage]);
-                        if (sx[k] > 0) bulk_g2s(dst + (H + len) * B, g + (size_t)(x0 + len == p.nx ? 0 : x0 + len) * B, 16u, &full[stage]);
-                    }
-                }
-            } else {
-                // 16-byte cp.async (LDGSTS.128): lane l copies chunk l (and l + 32, ...) of every row, then the piece(s) of
-                // its own rows; the barrier completes when the copies of all 32 lanes have landed
-                const unsigned s0 = smem_u32(stages + (size_t)stage * NPOPS * RS) + (unsigned)((H + lane * H) * B);
-                const unsigned goff = (unsigned)((x0 + lane * H) * B);
-                const int nchunk = len / H;
-                for (int r0 = 0; r0 < nrows; r0 += 8) {       // batches: 8 table reads, then 8 copies per lane
-                    const char* g[8];
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) g[j] = (const char*)rowptr[stage * NPOPS + min(r0 + j, nrows - 1)] + goff;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        if (r0 + j < nrows) {
-                            const unsigned d = s0 + (unsigned)((r0 + j) * RS * B);
-#pragma unroll
-                            for (int q = 0; q < TILE_TX / H / 32; ++q)
-                                if (lane + 32 * q < nchunk) cp_async16(d + (unsigned)(32 * q * H * B), g[j] + 32 * q * H * B);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < 2; ++k) {
-                    const int r = lane + 32 * k;
-                    if (r < nrows && sx[k] != 0) {
-                        const unsigned dst = smem_u32(stages + ((size_t)stage * NPOPS + r) * RS);
-                        const char* g = (const char*)base[k];
-                        if (sx[k] < 0) cp_async16(dst, g + (size_t)(x0 == 0 ? p.nx - H : x0 - H) * B);
-                        else cp_async16(dst + (unsigned)((H + len) * B), g + (size_t)(x0 + len == p.nx ? 0 : x0 + len) * B);
-                    }
-                }
-                cp_async_arrive(&full[stage]);
+            // One cp.async.bulk (TMA unit, UBLKCP: no load/store-unit slots) per row for the segment, issued by the lane
+            // that owns the row; completion: transaction bytes on the stage's barrier.  The 16-byte pieces beside the
+            // segment (periodic wrap in x) are 16-byte cp.async; the barrier also counts one arrival per lane for them.
+            const unsigned dst = smem_u32(stages + ((size_t)stage * NROWS + r) * RS);
+            const unsigned bytes = __reduce_add_sync(0xffffffffu, src ? (unsigned)(len * B) : 0u);
+            if (lane == 0) mbar_arrive_expect_tx(&full[stage], bytes);
+            __syncwarp();
+            if (src) {
+                bulk_g2s(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage]);
+                if (sx < 0 || r >= NPOPS) cp_async16(dst, src + (x0 == 0 ? p.nx - H : x0 - H));
+                if (sx > 0 || r >= NPOPS) cp_async16(dst + (unsigned)((H + len) * B), src + (x0 + len == p.nx ? 0 : x0 + len));
             }
-            TILE_TRACE(0, n);
+            cp_async_arrive(&full[stage]);
+            if (pwid == 0) TILE_TRACE(0, n);
         }
     }
 
@@ -373,155 +384,12 @@ struct Tile {
         });
     }
 
-    // ---------------- psi warp ----------------
-    __device__ __forceinline__ void psi_role(unsigned n_mine, unsigned b0, unsigned stride) const {
-        const int lane = (int)(threadIdx.x & 31);
-        const int nm = D == 3 ? p.ny : 1;
-        for (unsigned n = 0; n < n_mine; ++n) {
-            const int stage = (int)(n % NS);
-            const unsigned ph = (n / NS) & 1u;
-            const TileItem it = item_of(b0 + n * stride);
-            if (!mbar_wait(&full[stage], ph, w.status)) return;
-            TILE_TRACE(1, n);
-            const int x0 = it.xs * TILE_TX;
-            const int len = min(TILE_TX, p.nx - x0);
-            const bool edge = WALLYZ && ((wall_y() && (it.y == 0 || it.y == p.ny - 1)) || (wall_z() && (it.z == 0 || it.z == p.nz - 1)));
-            const size_t row0 = ((size_t)it.z * p.ny + it.y) * (size_t)p.nx;
-            // every lane takes its cell(s) of each 32 * CPT-cell chunk of the tile; the chunks are independent and
-            // unrolled together, so that their (serial, index-ordered) sums overlap
-            constexpr int NCH = TILE_TX / (32 * CPT);
-            V ps[NCH][S];
-#pragma unroll
-            for (int c = 0; c < NCH; ++c) {
-                const int t = c * 32 * CPT + lane * CPT;
-                if (t < len) {
-                    const R* sb = stages + (size_t)stage * NPOPS * RS + H + t;
-                    static_for<0, S>([&](auto sc) {
-                        constexpr int s = decltype(sc)::value;
-                        V fl[Q];
-                        if (WALLYZ && edge) read_pops<L, s * Q, true>(sb, stage, fl);
-                        else read_pops<L, s * Q, false>(sb, stage, fl);
-                        V rho = fl[0];
-                        static_for<1, Q>([&](auto ic) { rho = rho + fl[decltype(ic)::value]; });      // Eq. 7 / 18, index order
-                        ps[c][s] = psi_of(rho, p.psi_kind, p.rho0_psi);
-                    });
-                }
-            }
-#pragma unroll
-            for (int c = 0; c < NCH; ++c) {
-                const int t = c * 32 * CPT + lane * CPT;
-                if (t < len) {
-                    static_for<0, S>([&](auto sc) {
-                        constexpr int s = decltype(sc)::value;
-                        R* dst = p.psi + (size_t)s * (size_t)p.N + row0 + (size_t)(x0 + t);
-                        if constexpr (C::PACK) *reinterpret_cast<unsigned long long*>(dst) = ps[c][s].v;
-                        else *dst = ps[c][s];
-                    });
-                }
-            }
-            __syncwarp();
-            if (lane == 0) {
-                const int ms = D == 3 ? it.y : 0, ss = D == 3 ? it.z : it.y;
-                st_release(w.flags + ((size_t)ss * nm + ms) * w.nxs + it.xs, w.epoch);
-                mbar_arrive(&psi_done[stage]);
-            }
-            TILE_TRACE(2, n);
-        }
-    }
-
-    // ---------------- halo warp ----------------
-    // wait until the psi of the (up to) 27 tiles around (xs, y, z) is published
-    __device__ __forceinline__ bool wait_flags(const TileItem& it) const {
-        const int l = (int)(threadIdx.x & 31);
-        const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
-        const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
-        const bool wm = D == 3 ? wall_y() : false, wsl = D == 3 ? wall_z() : wall_y();
-        bool ok = true;
-        if (l < 27) {
-            const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
-            int mm = m + dm, ss = s + ds;
-            const bool beyond = (wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0);
-            if (!beyond) {
-                const int xx = wrap(it.xs + dx, w.nxs);
-                mm = wrap(mm, nm); ss = wrap(ss, ns);
-                const int* fl = w.flags + ((size_t)ss * nm + mm) * w.nxs + xx;
-                // relaxed polls (no L1 invalidation per poll), one acquire fence once every flag has been seen
-                ok = ld_relaxed(fl) == w.epoch;
-                if (!ok) {
-                    const long long t0 = clock64();
-                    while (!(ok = (ld_relaxed(fl) == w.epoch))) {
-                        __nanosleep(100);
-                        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { *w.status = 1; break; }
-                    }
-                }
-            }
-        }
-        ok = __all_sync(0xffffffffu, ok);
-        fence_acq_rel_gpu();                               // with the relaxed loads above: acquire of every flag
-        __syncwarp();                                      // every lane's copies below come after every lane's acquire
-        return ok;
-    }
-    __device__ __forceinline__ void halo_role(unsigned n_mine, unsigned b0, unsigned stride) const {
-        const int lane = (int)(threadIdx.x & 31);
-        unsigned h = 0;
-        for (unsigned n = 0; n < n_mine; ++n) {
-            const TileItem it = item_of(b0 + n * stride);
-            if (it.kind != TILE_FULL) continue;
-#ifndef LBM_TILE_NOWAIT
-            if (!wait_flags(it)) return;
-#endif
-            TILE_TRACE(3, n);
-            const int buf = (int)(h % TILE_NHB);
-            if (!mbar_wait(&halo_empty[buf], ((h / TILE_NHB) & 1u) ^ 1u, w.status)) return;
-            TILE_TRACE(8, n);
-            const int x0 = it.xs * TILE_TX;
-            const int len = min(TILE_TX, p.nx - x0);
-            const int chunks = len / H + 2;                // segment plus one piece on either side
-            const unsigned hb = smem_u32(halo + (size_t)buf * C::NP * RS);
-            // asynchronous 16-byte copies (L2 only: cp.async.cg never reads a stale L1 line); the warp does not wait
-            // for them but goes on to the flags of its next tile.  Per psi row: the segment chunks by all lanes,
-            // the two 16-byte pieces left and right of it (periodic wrap in x) by lanes 0 and 1
-            const int nchunk = len / H;
-            const int xl = x0 == 0 ? p.nx - H : x0 - H, xr = x0 + len == p.nx ? 0 : x0 + len;
-            // lane r < NP works out the source of psi row r (nullptr: beyond a wall, never read) ...
-            const R* mine = nullptr;
-            if (lane < C::NP) {
-                const int t = lane / C::NPSI, q = lane - t * C::NPSI;
-                const int dy = q % 3 - 1, dz = D == 3 ? q / 3 - 1 : 0;
-                if (!crosses(it.y, it.z, dy, dz)) {
-                    const int yy = wrap(it.y + dy, p.ny), zz = D == 3 ? wrap(it.z + dz, p.nz) : 0;
-                    mine = p.psi + (size_t)t * (size_t)p.N + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
-                }
-                // ... and copies its two pieces
-                if (mine) {
-                    const unsigned dst = hb + (unsigned)(lane * RS * B);
-                    cp_async16(dst, mine + xl);
-                    cp_async16(dst + (unsigned)((H + len) * B), mine + xr);
-                }
-            }
-            // the segment of every row: chunk `lane` (and lane + 32, ...) by all lanes
-#pragma unroll
-            for (int row = 0; row < C::NP; ++row) {
-                const R* src = (const R*)__shfl_sync(0xffffffffu, (unsigned long long)mine, row);
-                if (src) {
-                    const unsigned dst = hb + (unsigned)((row * RS + H) * B);
-#pragma unroll
-                    for (int k = 0; k < TILE_TX / H / 32; ++k)
-                        if (lane + 32 * k < nchunk) cp_async16(dst + (unsigned)((lane + 32 * k) * H * B), src + x0 + (lane + 32 * k) * H);
-                }
-            }
-            cp_async_arrive(&halo_full[buf]);
-            TILE_TRACE(4, n);
-            ++h;
-        }
-    }
-
     // ---------------- step warps ----------------
     // f*_{opp(i)} back to P_i(x): the global row the stage row came from, column x + shift (periodic wrap).
     // col[0..3] = x - 1, x, x + 1, x + 2 with wrap (x + 1 only for the second cell of a packed pair)
     template <class LL, int R0, int I, bool EDGE>
     __device__ __forceinline__ void write_pop(int stage, const int* col, V val) const {
-        R* g0 = (R*)rowptr[stage * NPOPS + R0 + I];
+        R* g0 = (R*)rowptr[stage * 64 + R0 + I];
         if constexpr (PARITY == 0 || I == 0 || LL::c(I, 0) == 0) {
             st_global(g0 + col[1], val);
         } else {
@@ -548,10 +416,10 @@ struct Tile {
             write_pop<LL, R0, i, EDGE>(stage, col, fl[LL::opp(i)]);
         });
     }
-    // psi of the thread's cell(s) at offset (CX, CY, CZ) from the halo buffer; hb: position of the first cell in row 0
+    // psi(t) of the thread's cell(s) at offset (CX, CY, CZ) from the psi rows of the stage; sb as in read_pop
     template <int CX, int CY, int CZ>
-    __device__ __forceinline__ V psi_at(const R* hb, int t) const {
-        const R* q = hb + C::psi_row(t, CY, CZ) * RS + CX;
+    __device__ __forceinline__ V psi_at(const R* sb, int t) const {
+        const R* q = sb + C::psi_row(t, CY, CZ) * RS + CX;
         if constexpr (C::PACK) {
             if constexpr (CX == 0) { F2 v; v.v = *reinterpret_cast<const unsigned long long*>(q); return v; }
             else return pack2(q[0], q[1]);
@@ -560,19 +428,23 @@ struct Tile {
         }
     }
     template <bool EDGE>
-    __device__ __forceinline__ void step_cells(int stage, int buf, const TileItem& it, int t) const {
+    __device__ __forceinline__ void step_cells(int stage, const TileItem& it, int t) const {
         const int x = it.xs * TILE_TX + t;
-        const R* sb = stages + (size_t)stage * NPOPS * RS + H + t;
-        const R* hb = halo + (size_t)buf * C::NP * RS + H + t;
-        V fl[S][Q];
+        const R* sb = stages + (size_t)stage * NROWS * RS + H + t;
+        // The populations are read from the stage twice -- for the moments here, for the collision below -- instead of
+        // being kept in registers in between (2 x 19 + 7 values per cell, two cells per thread): the step role then fits
+        // 128 registers, which buys a second team of step warps per SM.  Same values, same arithmetic.
+        CellMacro<V, L, MODEL> m;
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
-            read_pops<L, s * Q, EDGE>(sb, stage, fl[s]);
+            V fl[Q];
+            read_pops<L, s * Q, EDGE>(sb, stage, fl);
+            m.j[s][0] = m.j[s][1] = m.j[s][2] = vconst<V>(0.0);
+            moments<L>(fl, m.rho[s], m.j[s]);
         });
-        V hl[LS::Q];
-        if constexpr (MT::SCALAR) read_pops<LS, NF, EDGE>(sb, stage, hl);
+        asm volatile("" ::: "memory");                     // (the second read below is a real read)
 
-        // stencil sums from the halo buffer, the order of sc_stencil (row a3)
+        // stencil sums from the psi rows, the order of sc_stencil (row a3)
         V acc[S][3], psi_own[S], adh[3];
         adh[0] = adh[1] = adh[2] = vconst<V>(0.0);
         static_for<0, S>([&](auto tc) {
@@ -584,7 +456,7 @@ struct Tile {
                 bool out = false;
                 if constexpr (EDGE) out = crosses(it.y, it.z, CY, CZ);
                 V pv = vconst<V>(0.0);
-                if (!out) pv = psi_at<CX, CY, CZ>(hb, tt);
+                if (!out) pv = psi_at<CX, CY, CZ>(sb, tt);
                 static_for<0, D>([&](auto ac) {
                     constexpr int a = decltype(ac)::value;
                     constexpr int c = L::c(i, a);
@@ -596,83 +468,247 @@ struct Tile {
                     }
                 });
             });
-            psi_own[tt] = psi_at<0, 0, 0>(hb, tt);
+            psi_own[tt] = psi_at<0, 0, 0>(sb, tt);
         });
-        CellMacro<V, L, MODEL> m;
-        cell_macros_core<V, L, MODEL, true, WALLYZ>(p, fl, acc, psi_own, m, adh);
+        cell_force_velocity<V, L, MODEL, true, WALLYZ>(p, acc, psi_own, m, adh);
         const int col[4] = {x == 0 ? p.nx - 1 : x - 1, x, x + 1 == p.nx ? 0 : x + 1, x + 2 >= p.nx ? x + 2 - p.nx : x + 2};
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
-            collide_component<V, L, true, s>(p, fl[s], m.rho[s], m.u, m.F[s]);
-            write_pops<L, s * Q, EDGE>(stage, col, fl[s]);
+            V fl[Q];
+            read_pops<L, s * Q, EDGE>(sb, stage, fl);
+            collide_component<V, L, true, s>(p, fl, m.rho[s], m.u, m.F[s]);
+            write_pops<L, s * Q, EDGE>(stage, col, fl);
         });
         if constexpr (MT::SCALAR) {
+            V hl[LS::Q];
+            read_pops<LS, NF, EDGE>(sb, stage, hl);
             collide_scalar<V, LS>(p, hl, m.rho[0], m.rho[S - 1], m.inv_rho, m.u);
             write_pops<LS, NF, EDGE>(stage, col, hl);
         }
     }
-    __device__ __forceinline__ void step_role(unsigned n_mine, unsigned b0, unsigned stride) const {
-        const int t = (int)threadIdx.x * CPT;
-        const int lane = (int)(threadIdx.x & 31);
-        unsigned h = 0;
+    // team `team` takes the tickets n = team, team + TEAMS, ... of the block
+    __device__ __forceinline__ void step_role(int team, unsigned n_mine, unsigned b0, unsigned stride) const {
+        const int t = ((int)threadIdx.x - team * C::STEP_THREADS) * CPT;
+        const int lane = (int)(threadIdx.x & 31), wid = (int)(threadIdx.x >> 5);
+        unsigned cnt = 0;
         for (unsigned n = 0; n < n_mine; ++n) {
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
-            const TileItem it = item_of(b0 + n * stride);
-            if (!mbar_wait(&full[stage], ph, w.status)) return;
-            if (!mbar_wait(&psi_done[stage], ph, w.status)) return;
-            if (it.kind == TILE_FULL) {
-                const int buf = (int)(h % TILE_NHB);
-                if (!mbar_wait(&halo_full[buf], (h / TILE_NHB) & 1u, w.status)) return;
-                if (threadIdx.x == 0) TILE_TRACE(5, n);
-                const int len = min(TILE_TX, p.nx - it.xs * TILE_TX);
-                if (t < len) {
-                    const bool edge = WALLYZ && ((wall_y() && (it.y == 0 || it.y == p.ny - 1)) ||
-                                                 (wall_z() && (it.z == 0 || it.z == p.nz - 1)));
-                    if (WALLYZ && edge) step_cells<WALLYZ>(stage, buf, it, t);
-                    else step_cells<false>(stage, buf, it, t);
-                }
-                __syncwarp();
-                if (threadIdx.x == 0) TILE_TRACE(6, n);
-                if (lane == 0) mbar_arrive(&halo_empty[buf]);
-                ++h;
-            } else {
-                __syncwarp();
+            // every team consumes every phase of every stage in order -- a parity wait must never be asked about a phase
+            // two ahead of the last one seen, so a stage is refilled only after ALL step warps have let go of it -- and
+            // works on its own tickets
+            if (!mbar_wait(&full[stage], ph, w.status, 1)) return;
+            if (n % C::TEAMS != (unsigned)team) {
+                if (lane == 0) mbar_arrive(&empty[stage]);
+                continue;
             }
-            if (lane == 0) mbar_arrive(&empty[stage]);
+            const TileItem it = item_of(w.step_items, b0 + n * stride);
+            if (threadIdx.x == 0) TILE_TRACE(5, n);
+            const int len = min(TILE_TX, p.nx - it.xs * TILE_TX);
+#ifndef LBM_TILE_NOSTEP
+            if (t < len) {
+                if (edge_row(it.y, it.z)) step_cells<WALLYZ>(stage, it, t);
+                else step_cells<false>(stage, it, t);
+            }
+#endif
+            __syncwarp();
+            if (threadIdx.x == 0) TILE_TRACE(6, n);
+            if (lane == 0) {
+                TILE_MARK(0, n, 1);
+                st_release_cta_shared(&done[wid], ++cnt);      // after the stores of the whole warp (syncwarp above)
+                mbar_arrive(&empty[stage]);
+            }
+        }
+    }
+
+    // ---------------- publisher ----------------
+    // the flags of the tiles every step warp of this block has stored: one gpu-scope fence (cumulative over the
+    // stores it has observed through the done counters), then the flags
+    __device__ __forceinline__ void publish_role(unsigned n_mine, unsigned b0, unsigned stride) const {
+        const int lane = (int)(threadIdx.x & 31);
+        unsigned k[C::TEAMS], left = n_mine;
+#pragma unroll
+        for (int tm = 0; tm < C::TEAMS; ++tm) k[tm] = 0;
+        long long t0 = clock64();
+        while (left > 0) {
+            bool any = false;
+#pragma unroll
+            for (int tm = 0; tm < C::TEAMS; ++tm) {
+                unsigned m = ld_acquire_cta_shared(&done[tm * C::STEP_WARPS]);
+#pragma unroll
+                for (int q = 1; q < C::STEP_WARPS; ++q) m = min(m, ld_acquire_cta_shared(&done[tm * C::STEP_WARPS + q]));
+                // one value for the whole warp: the lanes may have read the counters at different times (independent
+                // thread scheduling), and each lane publishes the tickets k + lane, k + lane + 32, ... below m
+                m = __shfl_sync(0xffffffffu, m, 0);
+                if (m > k[tm]) {
+                    fence_acq_rel_gpu();
+                    for (unsigned j = k[tm] + lane; j < m; j += 32) {
+                        const TileItem it = item_of(w.step_items, b0 + (j * C::TEAMS + tm) * stride);
+                        st_relaxed(flag_of(it.xs, it.y, it.z), w.epoch);
+                        TILE_MARK(1, j * C::TEAMS + tm, 1 + 1000 * it.xs + 10000 * it.y + 10000000LL * it.z);
+                    }
+                    TILE_TRACE(2, (m - 1) * C::TEAMS + tm);
+                    left -= m - k[tm];
+                    k[tm] = m;
+                    any = true;
+                }
+            }
+            if (any) {
+                t0 = clock64();
+            } else {
+                __nanosleep(200);
+                if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 4); return; }
+            }
+        }
+    }
+
+    // ---------------- psi warps ----------------
+    // wait until the step of the (up to) 27 tiles around (xs, y, z) is complete
+    __device__ __forceinline__ bool wait_flags(const TileItem& it) const {
+        const int l = (int)(threadIdx.x & 31);
+        const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
+        const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
+        const bool wm = D == 3 ? wall_y() : false, wsl = D == 3 ? wall_z() : wall_y();
+        bool ok = true;
+        if (l < 27) {
+            const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
+            int mm = m + dm, ss = s + ds;
+            const bool beyond = (wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0);
+            if (!beyond) {
+                const int xx = wrap(it.xs + dx, w.nxs);
+                mm = wrap(mm, nm); ss = wrap(ss, ns);
+                const int* fl = w.flags + ((size_t)ss * nm + mm) * w.nxs + xx;
+                ok = ld_acquire(fl) == w.epoch;
+                if (!ok) {
+                    const long long t0 = clock64();
+                    while (!(ok = (ld_acquire(fl) == w.epoch))) {
+                        __nanosleep(200);
+                        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 8); break; }
+                    }
+                }
+            }
+        }
+        ok = __all_sync(0xffffffffu, ok);                  // (a warp barrier: every lane's loads below come after every lane's acquire)
+        return ok;
+    }
+    // rho^sigma(t + 1) in index order (Eq. 7 / 18) from the slots of the next parity, psi^sigma to psi_out, for the
+    // 32 * VE cells of the tile from offset t0 on: every lane owns VE = 16 / sizeof(R) consecutive cells and loads one
+    // 16-byte vector per slot row (ld.global.cg.v4 / .v2); a row that is shifted by one cell in x takes the missing
+    // cell from the neighbouring lane (shuffle), the first / last lane from one extra element (periodic wrap)
+    __device__ __forceinline__ void psi_pass(const TileItem& it, int x0, int len, int t0, int lane) const {
+        constexpr int PN = 1 - PARITY;                     // parity of time level t + 1
+        constexpr int VE = 16 / B;
+        using VT = std::conditional_t<B == 4, float4, double2>;
+        constexpr int SB = (S * Q * 4 <= 96) ? S : 1;      // components loaded together (registers: 4 per vector)
+        const int nv = min(32, (len - t0) / VE);           // lanes with cells
+        const int xb = x0 + t0;
+        const int xc = xb + (lane < nv ? lane : 0) * VE;   // idle lanes repeat lane 0 (and do not store)
+        const int xleft = xb == 0 ? p.nx - 1 : xb - 1, xright = xb + nv * VE == p.nx ? 0 : xb + nv * VE;
+        R* out = (R*)w.psi_out + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx + xc;
+        static_for<0, S / SB>([&](auto bc) {
+            constexpr int s0 = decltype(bc)::value * SB;
+            VT v[SB][Q];
+            R hal[SB][Q];
+            int sxs[SB][Q];
+            static_for<0, SB>([&](auto sc) {
+                constexpr int ss = decltype(sc)::value;
+                static_for<0, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    unsigned long long base;
+                    row_source<PN>((s0 + ss) * Q + i, it.y, it.z, base, sxs[ss][i]);
+                    const R* g = (const R*)base;
+                    v[ss][i] = __ldcg((const VT*)(g + xc));
+                    if constexpr (PN == 1 && L::c(i, 0) != 0) {
+                        hal[ss][i] = (R)0;
+                        if (sxs[ss][i] < 0 && lane == 0) hal[ss][i] = __ldcg(g + xleft);
+                        if (sxs[ss][i] > 0 && lane == nv - 1) hal[ss][i] = __ldcg(g + xright);
+                    }
+                });
+            });
+            static_for<0, SB>([&](auto sc) {
+                constexpr int ss = decltype(sc)::value;
+                R rho[VE];
+                static_for<0, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    R e[VE];
+                    if constexpr (B == 4) { e[0] = v[ss][i].x; e[1] = v[ss][i].y; e[VE - 2] = v[ss][i].z; e[VE - 1] = v[ss][i].w; }
+                    else { e[0] = v[ss][i].x; e[1] = v[ss][i].y; }
+                    if constexpr (PN == 1 && L::c(i, 0) != 0) {
+                        const int sx = sxs[ss][i];
+                        if (sx > 0) {                      // cell x reads column x + 1
+                            R nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
+                            if (lane == nv - 1) nxt = hal[ss][i];
+#pragma unroll
+                            for (int k = 0; k < VE - 1; ++k) e[k] = e[k + 1];
+                            e[VE - 1] = nxt;
+                        } else if (sx < 0) {               // cell x reads column x - 1
+                            R prv = __shfl_up_sync(0xffffffffu, e[VE - 1], 1);
+                            if (lane == 0) prv = hal[ss][i];
+#pragma unroll
+                            for (int k = VE - 1; k > 0; --k) e[k] = e[k - 1];
+                            e[0] = prv;
+                        }
+                    }
+#pragma unroll
+                    for (int k = 0; k < VE; ++k) rho[k] = i == 0 ? e[k] : rho[k] + e[k];
+                });
+                VT o;
+                if constexpr (B == 4) {
+                    o.x = psi_of(rho[0], p.psi_kind, p.rho0_psi); o.y = psi_of(rho[1], p.psi_kind, p.rho0_psi);
+                    o.z = psi_of(rho[VE - 2], p.psi_kind, p.rho0_psi); o.w = psi_of(rho[VE - 1], p.psi_kind, p.rho0_psi);
+                } else {
+                    o.x = psi_of(rho[0], p.psi_kind, p.rho0_psi); o.y = psi_of(rho[1], p.psi_kind, p.rho0_psi);
+                }
+                if (lane < nv) *(VT*)(out + (size_t)(s0 + ss) * (size_t)p.N) = o;
+            });
+        });
+    }
+    __device__ __forceinline__ void psi_role(int pw, unsigned b0, unsigned stride) const {
+        const int lane = (int)(threadIdx.x & 31);
+        const unsigned worker = b0 * TILE_PSI_WARPS + (unsigned)pw, nworkers = stride * TILE_PSI_WARPS;
+        unsigned n = 0;
+        for (unsigned ticket = worker; ticket < w.n_items; ticket += nworkers, ++n) {
+            const TileItem it = item_of(w.psi_items, ticket);
+            if (!wait_flags(it)) return;
+            if (pw == 0) TILE_TRACE(3, n);
+            const int x0 = it.xs * TILE_TX;
+            const int len = min(TILE_TX, p.nx - x0);
+            for (int t0 = 0; t0 < len; t0 += 32 * (16 / B)) psi_pass(it, x0, len, t0, lane);
+            if (pw == 0) TILE_TRACE(4, n);
         }
     }
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLYZ, int NS>
-__global__ void __launch_bounds__(TileCfg<R, L, MODEL, NS>::THREADS) k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
-    using T = Tile<R, L, MODEL, PARITY, WALLYZ, NS>;
+template <class R, class L, int MODEL, int PARITY, bool WALLYZ>
+__global__ void __launch_bounds__(TileCfg<R, L, MODEL>::THREADS, 1)
+k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
+    using T = Tile<R, L, MODEL, PARITY, WALLYZ>;
     using C = typename T::C;
     extern __shared__ __align__(128) unsigned char tile_smem[];
     const T tl(p, w, tile_smem);
     const int wid = (int)(threadIdx.x >> 5);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NS; ++s) {
-            mbar_init(&tl.full[s], TILE_BULK ? 1 : 32);
-            mbar_init(&tl.psi_done[s], 1);
-            mbar_init(&tl.empty[s], C::STEP_WARPS);
+        for (int s = 0; s < C::NS; ++s) {
+            mbar_init(&tl.full[s], 33 * TILE_PROD_WARPS);     // per producer warp: one expect_tx arrival, 32 cp.async arrivals
+            mbar_init(&tl.empty[s], C::TEAMS * C::STEP_WARPS);
         }
-        for (int b = 0; b < TILE_NHB; ++b) {
-            mbar_init(&tl.halo_full[b], 32);
-            mbar_init(&tl.halo_empty[b], C::STEP_WARPS);
-        }
+        for (int k = 0; k < 8; ++k) tl.done[k] = 0u;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    // static work distribution: block b owns the tickets b, b + gridDim.x, ...
+    // static work distribution: block b owns the STEP tickets b, b + gridDim.x, ...
     const unsigned b0 = blockIdx.x, stride = gridDim.x;
     const unsigned n_mine = b0 < w.n_items ? (w.n_items - b0 + stride - 1) / stride : 0u;
-    // warp roles: the step warps have the lowest warp ids, the (short, latency-critical) producer the highest -- the warp
+    // warp roles: the step warps have the lowest warp ids, the (short, latency-critical) producers the highest -- the warp
     // scheduler favours the highest id among the eligible warps of a sub-partition
-    if (wid < C::STEP_WARPS) tl.step_role(n_mine, b0, stride);
-    else if (wid == C::STEP_WARPS) tl.halo_role(n_mine, b0, stride);
-    else if (wid == C::STEP_WARPS + 1) tl.psi_role(n_mine, b0, stride);
-    else tl.produce(n_mine, b0, stride);
+    constexpr int SW = C::TEAMS * C::STEP_WARPS;
+    if (wid < SW) tl.step_role(wid / C::STEP_WARPS, n_mine, b0, stride);
+#ifdef LBM_TILE_NOPSI
+    else if (wid < SW + C::PSI_WARPS) return;    // developer experiment: the step role alone (wrong results)
+#endif
+    else if (wid < SW + C::PSI_WARPS) tl.psi_role(wid - SW, b0, stride);
+    else if (wid == SW + C::PSI_WARPS) tl.publish_role(n_mine, b0, stride);
+    else tl.produce(wid - (SW + C::PSI_WARPS + 1), n_mine, b0, stride);
 }
 
 }  // namespace lbm

@@ -2,17 +2,19 @@
 // rows of one time step of a Shan-Chen model.
 //
 // Why: psi^sigma(x + c_i, t) must be known for all neighbours before cell x is collided (Eq. 11 / 13,
-// PAPER.md:128, 136; R9), and with in-place streaming a cell's populations can only be read before its
-// own step overwrites them.  The resident-tile kernel loads the populations of a tile ONCE into shared memory,
-// computes and publishes its psi (step a2), keeps the tile resident until the psi of the tiles around it has been
-// published by the blocks that own them, and then collides and streams it (a1, a3-a8) from shared memory.
+// PAPER.md:128, 136; R9), and psi(t + 1) of a cell can only be formed once the step of all its neighbours
+// has written the populations that stream into it (Eq. 5 / 7).  One launch therefore does two things per row:
 //
-// A FULL row item is one such load-psi-wait-step life cycle for every tile of the row.  The step of row (m, s)
-// needs psi of the 3 x 3 rows around it.  Rows whose own FULL item comes within `window` rows after it provide
-// their psi in time by themselves; any other needed row that has not been computed yet in this launch (the wrapped
-// neighbour plane at the start of a pencil, the first row of the next pencil) gets a PSI_ONLY item first: its flow
-// populations are loaded, psi is computed and published, and the tile is dropped -- its FULL item comes later and
-// reads the populations a second time (a fraction 1 / rows_per_pencil of the rows in 3D, one row in 2D).
+//   STEP item  the fused step a1, a3-a8 of time level t for the row, reading psi(t) (complete: it was written by the
+//              previous launch).  STEP items depend on nothing inside the launch; they come in pencil order: pencils of
+//              `py` rows of the slower-but-one axis, marched along the slowest axis.
+//   PSI item   step a2 for time level t + 1: rho^sigma(t + 1) of the row from the populations the STEP items of the 3 x 3
+//              rows around it (periodic wrap; none beyond a wall) have just written, psi(t + 1) to the OTHER psi
+//              buffer.  It becomes ready when the last of those STEP items is done and is listed right after it, so
+//              that a worker that takes PSI items in list order never waits for a dependency that comes later than
+//              the dependencies of the items behind it -- and finds the populations still in L2 (the distance is one
+//              plane of the pencil, py + 1 rows).  The rows at the edge of a pencil wait for the neighbouring pencil
+//              and are read from HBM again (a fraction 1 / py of the rows in 3D, none in 2D).
 //
 // Row coordinates: (m, s) = (y, z) for D3Q19; (0, y) for D2Q9 (the marching axis is always the slowest one).
 #pragma once
@@ -21,78 +23,71 @@
 
 namespace lbm {
 
-enum { TILE_FULL = 0, TILE_PSI_ONLY = 1 };
+enum { TILE_STEP = 0, TILE_PSI = 1 };
 
 struct TileRow {
     int32_t kind, m, s;
 };
 
 // py: rows per pencil (clamped to [1, nm]); wrap_m / wrap_s: that axis is periodic (else: walls, no neighbour beyond).
-// *lead_rows (optional): the largest distance, in items of the returned list, from a FULL item to the LAST item that
-// provides a psi row it needs and comes after it -- what the kernel's pipeline depth must cover (tile.cuh).
-inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, bool wrap_s, int* lead_rows) {
+// Returns the merged list (2 * nm * ns items): every STEP row followed by the PSI rows that it completes.
+// *deferred_rows (optional): PSI rows listed more than 2 * py + 8 STEP rows after their own STEP row (they wait for
+// another pencil or for the wrapped plane: their populations have left L2 by then).
+inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, bool wrap_s, int* deferred_rows) {
     std::vector<TileRow> items;
-    if (lead_rows) *lead_rows = 0;
+    if (deferred_rows) *deferred_rows = 0;
     if (nm < 1 || ns < 1) return items;
     if (py < 1) py = 1;
     if (py > nm) py = nm;
-    struct MS { int m, s; };
-    std::vector<MS> order;
-    order.reserve((size_t)nm * ns);
-    std::vector<int64_t> pos_full((size_t)nm * ns, 0);
-    std::vector<int> window((size_t)nm * ns, 0);
-    for (int m0 = 0; m0 < nm; m0 += py) {
-        const int rows = (m0 + py <= nm ? py : nm - m0);
-        for (int s = 0; s < ns; ++s)
-            for (int m = m0; m < m0 + rows; ++m) {
-                pos_full[(size_t)s * nm + m] = (int64_t)order.size();
-                window[(size_t)s * nm + m] = rows + 1;      // FULL(m + 1, s + 1) comes rows + 1 items after FULL(m, s)
-                order.push_back(MS{m, s});
-            }
-    }
+    const size_t R = (size_t)nm * ns;
     auto nbr = [](int v, int d, int n, bool wrap, int* out) {
         int q = v + d;
         if (q < 0 || q >= n) {
             if (!wrap) return false;
             q = q < 0 ? q + n : q - n;
+            if (q < 0 || q >= n) return false;      // n == 1: the only row is its own neighbour
         }
         *out = q;
         return true;
     };
-    std::vector<uint8_t> have((size_t)nm * ns, 0);
-    std::vector<int64_t> provider((size_t)nm * ns, -1);    // position of the first item that computes psi of the row
-    items.reserve(order.size() + order.size() / (size_t)py + 64);
-    for (size_t idx = 0; idx < order.size(); ++idx) {
-        const MS r = order[idx];
+    // the (up to 9, possibly coinciding) rows around (m, s), itself included
+    auto around = [&](int m, int s, int (*out)[2]) {
+        int n = 0;
         for (int ds = -1; ds <= 1; ++ds)
             for (int dm = -1; dm <= 1; ++dm) {
                 int mm, ss;
-                if (!nbr(r.m, dm, nm, wrap_m, &mm) || !nbr(r.s, ds, ns, wrap_s, &ss)) continue;
-                const size_t k = (size_t)ss * nm + mm;
-                if (have[k]) continue;
-                const int64_t d = pos_full[k] - (int64_t)idx;
-                if (d >= 0 && d <= window[(size_t)r.s * nm + r.m]) continue;     // its own FULL item comes soon enough
-                have[k] = 1;
-                provider[k] = (int64_t)items.size();
-                items.push_back(TileRow{TILE_PSI_ONLY, mm, ss});
+                if (!nbr(m, dm, nm, wrap_m, &mm) || !nbr(s, ds, ns, wrap_s, &ss)) continue;
+                bool dup = false;
+                for (int k = 0; k < n; ++k) dup = dup || (out[k][0] == mm && out[k][1] == ss);
+                if (!dup) { out[n][0] = mm; out[n][1] = ss; ++n; }
             }
-        const size_t k = (size_t)r.s * nm + r.m;
-        if (!have[k]) { have[k] = 1; provider[k] = (int64_t)items.size(); }
-        items.push_back(TileRow{TILE_FULL, r.m, r.s});
-    }
-    if (lead_rows) {
-        int64_t lead = 0;
-        for (size_t p = 0; p < items.size(); ++p) {
-            if (items[p].kind != TILE_FULL) continue;
-            for (int ds = -1; ds <= 1; ++ds)
-                for (int dm = -1; dm <= 1; ++dm) {
-                    int mm, ss;
-                    if (!nbr(items[p].m, dm, nm, wrap_m, &mm) || !nbr(items[p].s, ds, ns, wrap_s, &ss)) continue;
-                    const int64_t d = provider[(size_t)ss * nm + mm] - (int64_t)p;
-                    if (d > lead) lead = d;
+        return n;
+    };
+    std::vector<uint8_t> stepped(R, 0), listed(R, 0);
+    std::vector<int64_t> step_pos(R, 0);
+    items.reserve(2 * R);
+    int64_t n_step = 0;
+    for (int m0 = 0; m0 < nm; m0 += py) {
+        const int rows = (m0 + py <= nm ? py : nm - m0);
+        for (int s = 0; s < ns; ++s)
+            for (int m = m0; m < m0 + rows; ++m) {
+                items.push_back(TileRow{TILE_STEP, m, s});
+                stepped[(size_t)s * nm + m] = 1;
+                step_pos[(size_t)s * nm + m] = n_step++;
+                int q[9][2], r[9][2];
+                const int nq = around(m, s, q);
+                for (int k = 0; k < nq; ++k) {
+                    const size_t qi = (size_t)q[k][1] * nm + q[k][0];
+                    if (listed[qi]) continue;
+                    const int nr = around(q[k][0], q[k][1], r);
+                    bool ready = true;
+                    for (int j = 0; j < nr; ++j) ready = ready && stepped[(size_t)r[j][1] * nm + r[j][0]];
+                    if (!ready) continue;
+                    listed[qi] = 1;
+                    items.push_back(TileRow{TILE_PSI, q[k][0], q[k][1]});
+                    if (deferred_rows && n_step - 1 - step_pos[qi] > 2 * (int64_t)py + 8) ++*deferred_rows;
                 }
-        }
-        *lead_rows = (int)lead;
+            }
     }
     return items;
 }

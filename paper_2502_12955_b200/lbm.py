@@ -143,8 +143,8 @@ def make_params(**kw):
 
 
 def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True):
-    """The resident-tile kernel's row schedule as an (n, 3) int32 array of (kind, m, s), and its lead in rows;
-    host-only call (kind 0: full life cycle of the row, 1: psi only)."""
+    """The resident-tile kernel's row schedule as an (n, 3) int32 array of (kind, m, s), and the number of psi rows
+    that wait for another pencil; host-only call (kind 0: step of the row, 1: psi of the next time level)."""
     import numpy as np
     L = lib()
     n = C.c_size_t(0)

@@ -156,37 +156,42 @@ def test_product_path_never_touches_the_oracle():
                                       (16, 9, 5), (6, 5, 100), (40, 12, 7)])
 @pytest.mark.parametrize("wrap_m,wrap_s", [(True, True), (False, True), (True, False), (False, False)])
 def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s):
-    """Host logic of the resident-tile kernel (tile_schedule.h).  Every row has exactly one FULL item (load, psi,
-    wait, step), in pencil order.  The step of a FULL item needs psi of the 3 x 3 rows around it (periodic wrap or
-    wall): each of them is computed by some item (PSI_ONLY, or its own FULL item), and the FIRST such item lies at
-    most `lead` items after the FULL item -- the number the kernel's pipeline depth has to cover for its bounded
-    waits to be deadlock-free; the results equal the two-pass order (psi of the whole field, then
-    the step: R9).  PSI_ONLY items re-read a row: they must stay a small fraction."""
+    """Host logic of the resident-tile kernel (tile_schedule.h).  Every row has exactly one STEP item (pencil order)
+    and exactly one PSI item (psi of the next time level, R9).  A PSI item needs the step of the 3 x 3 rows around
+    its row (periodic wrap or wall; Eq. 5 / 7): it is listed right after the LAST of their STEP items -- never
+    before (the psi warps would wait for every later step), never later than needed (the populations would leave
+    L2) -- so the PSI items are ordered by the time they become ready.  Rows that wait for another pencil or for the
+    wrapped plane are re-read from HBM: they must stay a small fraction."""
     import paper_2502_12955_b200 as pkg
-    it, lead = pkg.lbm.tile_schedule(nm, ns, py, wrap_m, wrap_s)
-    first = {}
-    full_pos = {}
+    it, deferred = pkg.lbm.tile_schedule(nm, ns, py, wrap_m, wrap_s)
+    assert len(it) == 2 * nm * ns
+    step_pos, psi_pos = {}, {}
     for k, (kind, m, s) in enumerate(it.tolist()):
         assert kind in (0, 1) and 0 <= m < nm and 0 <= s < ns
-        first.setdefault((m, s), k)
-        if kind == 0:
-            assert (m, s) not in full_pos
-            full_pos[(m, s)] = k
-    assert len(full_pos) == nm * ns
-    worst = 0
-    for (m, s), k in full_pos.items():
+        d = step_pos if kind == 0 else psi_pos
+        assert (m, s) not in d
+        d[(m, s)] = k
+    assert len(step_pos) == nm * ns and len(psi_pos) == nm * ns
+    p = max(1, min(py, nm))
+    steps = [(m, s) for kind, m, s in it.tolist() if kind == 0]
+    assert steps == [(m, s) for m0 in range(0, nm, p) for s in range(ns) for m in range(m0, min(m0 + p, nm))]
+    order = {ms: k for k, ms in enumerate(steps)}
+    late = 0
+    for (m, s), k in psi_pos.items():
+        deps = []
         for dm in (-1, 0, 1):
             for ds in (-1, 0, 1):
                 mm, ss = m + dm, s + ds
                 if (not wrap_m and not 0 <= mm < nm) or (not wrap_s and not 0 <= ss < ns):
                     continue
-                worst = max(worst, first[(mm % nm, ss % ns)] - k)
-    assert worst == lead
-    p = max(1, min(py, nm))
-    # one plane of the pencil and its two edge rows; at the start of a pencil also the wrapped plane's PSI_ONLY items
-    assert lead <= 2 * p + 8
-    fulls = [(m, s) for kind, m, s in it.tolist() if kind == 0]
-    assert fulls == [(m, s) for m0 in range(0, nm, p) for s in range(ns) for m in range(m0, min(m0 + p, nm))]
-    n_psi_only = len(it) - nm * ns
+                deps.append(step_pos[(mm % nm, ss % ns)])
+        last = max(deps)
+        assert last < k                                   # after its last dependency ...
+        assert all(kind == 1 for kind, _, _ in it[last + 1:k].tolist())     # ... with no step item in between
+        if max(order[(it[d][1], it[d][2])] for d in deps) - order[(m, s)] > 2 * p + 8:
+            late += 1
+    assert late == deferred
     pencils = -(-nm // p)
-    assert n_psi_only <= pencils * (2 * ns + 2 * (p + 2)) + 2
+    assert deferred <= pencils * (2 * ns + 2 * (p + 2)) + 2
+
+
