@@ -176,11 +176,12 @@ int lbm_get_path(const lbm_ctx* ctx);
 
 /* The row schedule of LBM_PATH_PIPELINE for nm x ns rows (D3Q19: nm = ny, ns = nz; D2Q9: nm = 1, ns = ny;
  * wrap_m / wrap_s: that axis is periodic): *count = 2 * nm * ns items; if items != NULL (HOST, capacity items of 3
- * int32: kind 0 = step of the row / 1 = psi of the next time level of the row, m, s) they are written out: every
- * step row in pencil order, followed by the psi rows whose last dependency it is.  *deferred_rows (optional)
- * receives the number of psi rows that wait for another pencil (re-read from HBM).  Host-only, needs no GPU. */
-int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
-                      size_t* count, int* deferred_rows);
+ * int32: kind 0 = step of the row / 1 = psi of the next time level of the row, m, s) they are written out: the
+ * step rows in pencil order; the psi rows whose last dependency is the k-th step row follow step row
+ * k + delay_rows.  *deferred_rows (optional) receives the number of psi rows that wait for another pencil
+ * (re-read from HBM).  Host-only, needs no GPU. */
+int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int delay_rows, int32_t* items,
+                      size_t capacity, size_t* count, int* deferred_rows);
 
 /* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a bounded wait of LBM_PATH_PIPELINE
  * timed out; lbm_run_host performs the same check before it returns). */

@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -20,6 +21,10 @@ namespace {
 // rows per pencil of the resident-tile schedule unless the caller chooses (lbm_set_path)
 #ifndef LBM_TILE_DEFAULT_PY
 #define LBM_TILE_DEFAULT_PY 32
+#endif
+// rounds of the round-robin between a STEP ticket and the PSI tickets that depend on it (tile_schedule.h)
+#ifndef LBM_TILE_DELAY
+#define LBM_TILE_DELAY 3
 #endif
 
 thread_local std::string g_err;
@@ -287,7 +292,7 @@ const char* tile_ineligible(const lbm_ctx* c) {
     return nullptr;
 }
 
-// Switch to the resident-tile path: build the schedule (one STEP and one PSI entry per tile), the flags and the
+// Switch to the resident-tile path: build the schedule (one STEP and one PSI ticket per tile), the flags and the
 // second psi buffer; py <= 0 picks the default
 int path_setup(lbm_ctx* c, int py) {
     CK(cudaStreamSynchronize(c->stream));
@@ -306,29 +311,33 @@ int path_setup(lbm_ctx* c, int py) {
     if (py <= 0) py = LBM_TILE_DEFAULT_PY;
     if (py < 1) py = 1;
     if (py > nm) py = nm;
-    const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, nullptr);
     const size_t n_tiles = (size_t)nm * ns * nxs;
-    if ((double)n_tiles > 2.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 2e9 tiles");
-    std::vector<lbm::TileItem> items(2 * n_tiles);
-    size_t k_step = 0, k_psi = n_tiles;
+    if ((double)n_tiles > 1.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 1e9 tiles");
+    const int blocks = (long long)resident < (long long)(2 * n_tiles) ? resident : (int)(2 * n_tiles);
+    // a PSI ticket comes LBM_TILE_DELAY rounds of the round-robin after the last STEP ticket it depends on
+    int delay_tiles = LBM_TILE_DELAY * blocks;
+#ifdef LBM_TUNING
+    if (const char* e = getenv("LBM_TILE_DELAY")) delay_tiles = atoi(e);
+#endif
+    const int delay_rows = (delay_tiles + nxs - 1) / nxs;
+    const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, delay_rows, nullptr);
+    std::vector<lbm::TileItem> items;
+    items.reserve(2 * n_tiles);
     for (const lbm::TileRow& r : rows) {
         lbm::TileItem it;
         it.y = sh.d == 3 ? r.m : r.s;
         it.z = sh.d == 3 ? r.s : 0;
-        it.pad = 0;
-        for (int xs = 0; xs < nxs; ++xs) {
-            it.xs = xs;
-            if (r.kind == lbm::TILE_STEP) items[k_step++] = it; else items[k_psi++] = it;
-        }
+        it.kind = r.kind;
+        for (int xs = 0; xs < nxs; ++xs) { it.xs = xs; items.push_back(it); }
     }
-    if (k_step != n_tiles || k_psi != 2 * n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
+    if (items.size() != 2 * n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
     c->tile_py = py;
-    c->tile_blocks = (long long)resident < (long long)n_tiles ? resident : (int)n_tiles;
-    c->tile_n_items = (long long)n_tiles;
+    c->tile_blocks = blocks;
+    c->tile_n_items = (long long)items.size();
     c->tile_nxs = nxs;
     c->tile_n_tiles = n_tiles;
     cudaError_t e = cudaMalloc((void**)&c->tile_items, items.size() * sizeof(lbm::TileItem));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&c->tile_flags, (c->tile_n_tiles + 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&c->tile_flags, (c->tile_n_tiles + 1) * sizeof(int));    // flags, status word
     if (e == cudaSuccess) e = cudaMalloc(&c->psi_alt, sh.psi_bytes);
     if (e != cudaSuccess) { cudaGetLastError(); tile_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
     CK(cudaMemcpyAsync(c->tile_items, items.data(), items.size() * sizeof(lbm::TileItem), cudaMemcpyHostToDevice, c->stream));
@@ -350,8 +359,7 @@ int run_tile(lbm_ctx* c) {
         c->tile_epoch = 0;
     }
     lbm::TileArgs wa;
-    wa.step_items = c->tile_items;
-    wa.psi_items = c->tile_items + c->tile_n_items;
+    wa.items = c->tile_items;
     wa.n_items = (unsigned)c->tile_n_items;
     wa.nxs = c->tile_nxs;
     wa.flags = c->tile_flags;
@@ -359,8 +367,7 @@ int run_tile(lbm_ctx* c) {
     wa.status = c->tile_flags + c->tile_n_tiles;
     wa.psi_out = c->psi_alt;
 #ifdef LBM_TILE_TRACE
-    if (!g_trace) cudaMalloc((void**)&g_trace, sizeof(long long) * (10 * 4096 + 2 * 160 * 1024));
-    cudaMemsetAsync(g_trace, 0, sizeof(long long) * (10 * 4096 + 2 * 160 * 1024), c->stream);
+    if (!g_trace) { cudaMalloc((void**)&g_trace, sizeof(long long) * 10 * 4096); cudaMemset(g_trace, 0, sizeof(long long) * 10 * 4096); }
     wa.trace = g_trace;
 #endif
     int rc = mark(c, 0);
@@ -513,12 +520,14 @@ namespace {
 constexpr int GRAPH_STEPS = 32;                 // even: a replay starts and ends at even parity
 constexpr size_t GRAPH_MAX_CELLS = 1u << 21;    // above this a step takes far longer than a launch call
 
-// Default launch path, chosen at the first step unless the caller chose one (lbm_set_path): Shan-Chen models on
-// grids too large for the CUDA-graph replay take the resident-tile kernel where it applies (tile.cuh)
+// Default launch path, chosen at the first step unless the caller chose one (lbm_set_path): the resident-tile kernel
+// where it applies AND is the faster of the two (measured): the two-component D3Q19 models in fp32 on
+// grids too large for the CUDA-graph replay.  (D2Q9 in fp64: the register kernels are faster.)
 void choose_default_path(lbm_ctx* c) {
     if (c->path_user_set || c->path != LBM_PATH_REGISTER) return;
     c->path_user_set = true;                    // decide once
     if (c->sh.N <= GRAPH_MAX_CELLS || tile_ineligible(c) != nullptr) return;
+    if (!(c->lattice == LBM_D3Q19 && c->p.precision == 32 && c->sh.S == 2)) return;
     if (path_setup(c, 0) != 0) { cudaGetLastError(); tile_free(c); }
 }
 
@@ -744,12 +753,12 @@ int lbm_set_mask(lbm_ctx* c, const unsigned char* mask) {
     return 0;
 }
 
-int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int32_t* items, size_t capacity,
-                      size_t* count, int* deferred_rows) {
+int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int delay_rows, int32_t* items,
+                      size_t capacity, size_t* count, int* deferred_rows) {
     if (!count) return fail(LBM_EINVAL, "count is NULL");
     if (nm < 1 || ns < 1) return fail(LBM_EINVAL, "nm and ns must be >= 1");
     int deferred = 0;
-    const std::vector<lbm::TileRow> v = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, &deferred);
+    const std::vector<lbm::TileRow> v = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, delay_rows, &deferred);
     *count = v.size();
     if (deferred_rows) *deferred_rows = deferred;
     if (items) {
@@ -771,15 +780,7 @@ int lbm_check(lbm_ctx* c) {
 }
 
 #ifdef LBM_TILE_TRACE
-int lbm_debug_flags(lbm_ctx* c, int* out, size_t cap, int* epoch, int* blocks) {
-    cudaDeviceSynchronize();
-    *epoch = c->tile_epoch; *blocks = c->tile_blocks;
-    size_t n = c->tile_n_tiles + 1 < cap ? c->tile_n_tiles + 1 : cap;
-    cudaMemcpy(out, c->tile_flags, n * sizeof(int), cudaMemcpyDeviceToHost);
-    return (int)n;
-}
 int lbm_debug_trace(void* out) { return (int)cudaMemcpy(out, g_trace, sizeof(long long) * 10 * 4096, cudaMemcpyDeviceToHost); }
-int lbm_debug_marks(void* out) { return (int)cudaMemcpy(out, g_trace + 10 * 4096, sizeof(long long) * 2 * 160 * 1024, cudaMemcpyDeviceToHost); }
 #endif
 
 int64_t lbm_time(const lbm_ctx* c) { return c ? c->t : -1; }

@@ -36,27 +36,20 @@
 namespace lbm {
 
 constexpr int TILE_ROW_BYTES = 1024;  // bytes of one row segment of a tile: 256 fp32 / 128 fp64 cells (one bulk copy)
-constexpr int TILE_PROD_WARPS = 2;    // producer warps per block (each issues the bulk copies of half the rows)
-// psi warps per block.  With two teams of four step warps, two producers and the publisher that makes 15 warps = 480
-// threads of up to 136 registers: 16 warps of 128 registers would claim the whole register file of the SM, and a
-// launch of one such block per SM was observed NOT to be fully co-resident (the psi warps then wait for tiles of a
-// block that has not started).
-#ifndef LBM_TILE_PSIW
-#define LBM_TILE_PSIW 4
-#endif
+constexpr int TILE_PROD_WARPS = 4;    // producer warps per block (each issues the bulk copies of a quarter of the rows)
 
 struct TileItem {
-    int xs, y, z, pad;                // x-segment, row
+    int xs, y, z;                     // x-segment, row
+    int kind;                         // TILE_STEP / TILE_PSI (tile_schedule.h)
 };
 
 struct TileArgs {
-    const TileItem* step_items;       // the STEP tickets of one time step (device)
-    const TileItem* psi_items;        // the PSI tickets, in the order they become ready
-    unsigned n_items;                 // tiles = STEP tickets = PSI tickets
+    const TileItem* items;            // the tickets of one time step (device), STEP and PSI tickets in schedule order
+    unsigned n_items;                 // 2 * tiles
     int nxs;                          // tiles per row
     int* flags;                       // one per tile (z, y, xs): launch epoch of the last completed step
     int epoch;                        // > 0, differs from every earlier launch since the flags were cleared
-    int* status;                      // set to 1 if a wait timed out
+    int* status;                      // bits set when a bounded wait timed out
     void* psi_out;                    // psi(t + 1): S * N values, not the buffer KP::psi points at
 #ifdef LBM_TILE_TRACE
     long long* trace;
@@ -74,10 +67,7 @@ __device__ __forceinline__ void tile_trace(long long* buf, int what, unsigned n)
     }
 }
 #define TILE_TRACE(what, n) tile_trace(w.trace, what, n)
-// per block and ticket marks: 0 stepped (count of warps), 1 published
-#define TILE_MARK(kind, n, v) do { if ((n) < 1024) atomicAdd((unsigned long long*)&w.trace[10 * 4096 + ((kind) * 160 + blockIdx.x) * 1024 + (n)], (unsigned long long)(v)); } while (0)
 #else
-#define TILE_MARK(kind, n, v)
 #define TILE_TRACE(what, n)
 #endif
 
@@ -88,6 +78,11 @@ __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)_
 __device__ __forceinline__ int ld_acquire(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void st_relaxed(int* p, int v) {
@@ -141,6 +136,18 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, u
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned long long* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
                  "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// the same with an L2 eviction policy (createpolicy): populations are read once per launch -- evict_first keeps L2 for
+// the lines the step WRITES, which the trailing psi tickets read back
+__device__ __forceinline__ unsigned long long l2_evict_first() {
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s_hint(unsigned dst, const void* src, unsigned bytes, unsigned long long* bar, unsigned long long pol) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
                  : "memory");
 }
 // 16-byte asynchronous copy global -> shared (LDGSTS.128, L2 only) and its completion on an mbarrier: the barrier
@@ -198,21 +205,21 @@ struct TileCfg {
     static constexpr int NROWS = NPOPS + NP;                     // rows of a stage: populations, then psi
     static constexpr int STEP_THREADS = TX / CPT;
     static constexpr int STEP_WARPS = STEP_THREADS / 32;
-    // Two teams of step warps work on two stages at a time (two warps per scheduler hide each other's latencies):
-    // 512 threads of at most 128 registers.  The step role of the D3Q19 models in fp64 needs more registers (19
-    // doubles per component and thread): one team, 256 threads.
+    // Two teams of step warps work on two stages at a time (two warps per scheduler hide each other's latencies).  The
+    // step role of the D3Q19 models in fp64 needs more registers (19 doubles per component and thread): one team.
     static constexpr bool HEAVY = B == 8 && Q > 9;
     static constexpr int TEAMS = HEAVY ? 1 : 2;
-    static constexpr int PSI_WARPS = HEAVY ? 1 : LBM_TILE_PSIW;
-    static constexpr int AUX_WARPS = PSI_WARPS + 1 + TILE_PROD_WARPS;      // psi, publisher, producers
+    static constexpr int AUX_WARPS = 1 + TILE_PROD_WARPS;                  // publisher, producers
     static constexpr int THREADS = 32 * AUX_WARPS + TEAMS * STEP_THREADS;
     static constexpr size_t STAGE_BYTES = (size_t)NROWS * RS * B;
+    // one ring of NS stages for the STEP and the PSI tickets alike (two rings -- NS stages of each kind -- were measured
+    // and are slower: only two STEP stages fit beside two PSI stages)
     static constexpr int NS = (215 * 1024) / STAGE_BYTES >= 6 ? 6 : (int)((215 * 1024) / STAGE_BYTES);   // stages
     static constexpr size_t ROWPTR_BYTES = (size_t)NS * 64 * sizeof(unsigned long long);    // pointers of the (up to 64) rows of a stage
     static constexpr size_t ROWSX_BYTES = ((size_t)NS * NPOPS * sizeof(int) + 15) / 16 * 16;
     static constexpr int NBAR = 2 * NS;
     static constexpr size_t SMEM = NS * STAGE_BYTES + ROWPTR_BYTES + ROWSX_BYTES + NBAR * 8 + 32;
-    static_assert(NROWS <= 32 * TILE_PROD_WARPS, "one row per producer lane");
+    static_assert(NROWS <= 16 * TILE_PROD_WARPS, "one row per producer lane (16 lanes per warp issue)");
     static_assert(TEAMS * STEP_WARPS <= 8, "done counters");
     static_assert(NS >= 2 && SMEM <= 227 * 1024, "shared memory");
     __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return NPOPS + t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
@@ -225,7 +232,7 @@ struct Tile {
     using LS = typename C::LS;
     using V = typename C::V;
     static constexpr int S = C::S, Q = C::Q, D = C::D, B = C::B, H = C::H, RS = C::RS, NF = C::NF, NPOPS = C::NPOPS, CPT = C::CPT;
-    static constexpr int NROWS = C::NROWS, NS = C::NS, TILE_TX = C::TX, TILE_PSI_WARPS = C::PSI_WARPS;
+    static constexpr int NROWS = C::NROWS, NS = C::NS, TILE_TX = C::TX;
 
     const KP<R>& p;
     const TileArgs& w;
@@ -242,6 +249,9 @@ struct Tile {
         full = (unsigned long long*)((unsigned char*)rowsx + C::ROWSX_BYTES);
         empty = full + NS;
         done = (unsigned*)(empty + NS);
+    }
+    __device__ __forceinline__ R* slot_base(int stage) const {
+        return stages + (size_t)stage * NROWS * RS;
     }
     static __device__ __forceinline__ int wrap(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
     __device__ __forceinline__ bool wall_y() const { return WALLYZ && p.bc[1]; }
@@ -265,41 +275,46 @@ struct Tile {
     }
 
     // ---------------- producer ----------------
-    // population row r of an item at (y, z) at the parity PAR: slot array, source row, x-shift
-    template <int PAR>
-    __device__ __forceinline__ void row_source(int r, int y, int z, unsigned long long& base, int& sx) const {
-        const size_t N = (size_t)p.N;
-        int i, c0, c1, c2, op;
-        const R* arr;
-        if (r < NF) {
-            const int s = r / Q;
-            i = r - s * Q;
-            arr = p.f + (size_t)s * Q * N;
-            c0 = c_runtime<L, 0>(i); c1 = c_runtime<L, 1>(i); c2 = D == 3 ? c_runtime<L, 2>(i) : 0; op = L::opp(i);
-        } else {
-            i = r - NF;
-            arr = p.h;
-            c0 = c_runtime<LS, 0>(i); c1 = c_runtime<LS, 1>(i); c2 = D == 3 ? c_runtime<LS, 2>(i) : 0; op = LS::opp(i);
+    // wait until the step of the (up to) 27 tiles around (xs, y, z) is complete
+    __device__ __forceinline__ bool wait_flags(const TileItem& it) const {
+        const int l = (int)(threadIdx.x & 31);
+        const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
+        const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
+        const bool wm = D == 3 ? wall_y() : false, wsl = D == 3 ? wall_z() : wall_y();
+        bool ok = true;
+        if (l < 27) {
+            const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
+            int mm = m + dm, ss = s + ds;
+            const bool beyond = (wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0);
+            if (!beyond) {
+                const int xx = wrap(it.xs + dx, w.nxs);
+                mm = wrap(mm, nm); ss = wrap(ss, ns);
+                const int* fl = w.flags + ((size_t)ss * nm + mm) * w.nxs + xx;
+                ok = ld_acquire(fl) == w.epoch;
+                if (!ok) {
+                    const long long t0 = clock64();
+                    while (!(ok = (ld_acquire(fl) == w.epoch))) {
+                        __nanosleep(200);
+                        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 8); break; }
+                    }
+                }
+            }
         }
-        int slot = i, yy = y, zz = z;
-        sx = 0;
-        if (PAR == 1 && i != 0 && !crosses(y, z, -c1, -c2)) {
-            // P_i(x) = slot opp(i) of cell x - c_i; beyond a bounce-back wall: slot i of x itself
-            slot = op; yy = wrap(y - c1, p.ny); zz = D == 3 ? wrap(z - c2, p.nz) : 0; sx = -c0;
-        }
-        base = (unsigned long long)(arr + (size_t)slot * N + ((size_t)zz * p.ny + yy) * (size_t)p.nx);
+        return __all_sync(0xffffffffu, ok);                // (a warp barrier: every lane's copies below come after every lane's acquire)
     }
-    // producer warp `pwid` looks after the rows r = 32 * pwid + lane of every stage
-    __device__ __forceinline__ void produce(int pwid, unsigned n_mine, unsigned b0, unsigned stride) const {
-        const int lane = (int)(threadIdx.x & 31);
-        const int r = 32 * pwid + lane;
+    // Row r of a ticket of kind K at parity PAR (STEP: the parity of this launch, all rows; PSI: the next parity, the
+    // flow populations only): where it comes from relative to the ticket's row.  nbr: element 0 of row (0, 0) of the
+    // source array / slot; own: the same for the cell's own slot (a population row that would cross a wall; a psi row is
+    // left out)
+    struct RowDesc {
+        const R* nbr;
+        const R* own;
+        int dy, dz, sx;
+    };
+    __device__ __forceinline__ RowDesc row_desc(int r, int par, bool psi_ticket) const {
         const size_t N = (size_t)p.N;
-        // where row r comes from relative to the item's row.  nbr: element 0 of row (0, 0) of the source array / slot;
-        // own: the same for the cell's own slot (a population row that would cross a wall; a psi row is left out)
-        const R* nbr = nullptr;
-        const R* own = nullptr;
-        int dy = 0, dz = 0, sx0 = 0;
-        if (r < NPOPS) {
+        RowDesc d{nullptr, nullptr, 0, 0, 0};
+        if (r < NPOPS && !(psi_ticket && r >= NF)) {
             int i, c0, c1, c2, op;
             const R* arr;
             if (r < NF) {
@@ -312,20 +327,34 @@ struct Tile {
                 arr = p.h;
                 c0 = c_runtime<LS, 0>(i); c1 = c_runtime<LS, 1>(i); c2 = D == 3 ? c_runtime<LS, 2>(i) : 0; op = LS::opp(i);
             }
-            own = arr + (size_t)i * N;
-            nbr = own;
-            if (PARITY == 1 && i != 0) {       // P_i(x) = slot opp(i) of cell x - c_i; beyond a wall: slot i of x itself
-                nbr = arr + (size_t)op * N; dy = -c1; dz = -c2; sx0 = -c0;
+            d.own = arr + (size_t)i * N;
+            d.nbr = d.own;
+            if (par == 1 && i != 0) {          // P_i(x) = slot opp(i) of cell x - c_i; beyond a wall: slot i of x itself
+                d.nbr = arr + (size_t)op * N; d.dy = -c1; d.dz = -c2; d.sx = -c0;
             }
-        } else if (r < NROWS) {
+        } else if (r >= NPOPS && r < NROWS && !psi_ticket) {
             const int q0 = r - NPOPS, t = q0 / C::NPSI, q = q0 - t * C::NPSI;
-            dy = D == 3 ? q % 3 - 1 : q - 1; dz = D == 3 ? q / 3 - 1 : 0;
-            nbr = p.psi + (size_t)t * N;
+            d.dy = D == 3 ? q % 3 - 1 : q - 1; d.dz = D == 3 ? q / 3 - 1 : 0;
+            d.nbr = p.psi + (size_t)t * N;
         }
+        return d;
+    }
+    // producer warp `pwid` looks after the rows r = pwid + TILE_PROD_WARPS * lane (lane < 16) of every stage
+    __device__ __forceinline__ void produce(int pwid, unsigned n_mine, unsigned b0, unsigned stride) const {
+        const int lane = (int)(threadIdx.x & 31);
+        const int r = lane < 16 ? pwid + TILE_PROD_WARPS * lane : NROWS;
+        const RowDesc d_step = row_desc(r, PARITY, false), d_psi = row_desc(r, 1 - PARITY, true);
+        const unsigned long long pol = l2_evict_first();
         for (unsigned n = 0; n < n_mine; ++n) {
+            const TileItem it = item_of(w.items, b0 + n * stride);
+            const bool ps = it.kind == TILE_PSI;
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
-            const TileItem it = item_of(w.step_items, b0 + n * stride);
+            const RowDesc d{ps ? d_psi.nbr : d_step.nbr, ps ? d_psi.own : d_step.own, ps ? d_psi.dy : d_step.dy,
+                            ps ? d_psi.dz : d_step.dz, ps ? d_psi.sx : d_step.sx};
+            // a PSI ticket reads what the step of the tiles around it has written: listed well after them (tile_schedule.h),
+            // so this wait is a formality -- but it is what makes the read correct
+            if (it.kind == TILE_PSI && !wait_flags(it)) return;
             if (!mbar_wait(&empty[stage], ph ^ 1u, w.status, 2)) return;
             if (pwid == 0) TILE_TRACE(7, n);
             const int x0 = it.xs * TILE_TX;
@@ -333,12 +362,12 @@ struct Tile {
             const R* src = nullptr;
             int sx = 0;
             if (r < NROWS) {
-                if (crosses(it.y, it.z, dy, dz)) {
-                    if (own) src = own + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx;
-                } else {
-                    const int yy = wrap(it.y + dy, p.ny), zz = D == 3 ? wrap(it.z + dz, p.nz) : 0;
-                    src = nbr + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
-                    sx = sx0;
+                if (crosses(it.y, it.z, d.dy, d.dz)) {
+                    if (d.own) src = d.own + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx;
+                } else if (d.nbr) {
+                    const int yy = wrap(it.y + d.dy, p.ny), zz = D == 3 ? wrap(it.z + d.dz, p.nz) : 0;
+                    src = d.nbr + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
+                    sx = d.sx;
                 }
                 rowptr[stage * 64 + r] = (unsigned long long)src;
                 if (r < NPOPS) rowsx[stage * NPOPS + r] = sx;
@@ -346,11 +375,15 @@ struct Tile {
             // One cp.async.bulk (TMA unit, UBLKCP: no load/store-unit slots) per row for the segment, issued by the lane
             // that owns the row; completion: transaction bytes on the stage's barrier.  The 16-byte pieces beside the
             // segment (periodic wrap in x) are 16-byte cp.async; the barrier also counts one arrival per lane for them.
-            const unsigned dst = smem_u32(stages + ((size_t)stage * NROWS + r) * RS);
+            const unsigned dst = smem_u32(slot_base(stage) + (size_t)(r < NROWS ? r : 0) * RS);
             const unsigned bytes = __reduce_add_sync(0xffffffffu, src ? (unsigned)(len * B) : 0u);
             if (lane == 0) mbar_arrive_expect_tx(&full[stage], bytes);
             __syncwarp();
             if (src) {
+#ifndef LBM_TILE_NOHINT
+                if (r < NPOPS) bulk_g2s_hint(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage], pol);
+                else
+#endif
                 bulk_g2s(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage]);
                 if (sx < 0 || r >= NPOPS) cp_async16(dst, src + (x0 == 0 ? p.nx - H : x0 - H));
                 if (sx > 0 || r >= NPOPS) cp_async16(dst + (unsigned)((H + len) * B), src + (x0 + len == p.nx ? 0 : x0 + len));
@@ -363,10 +396,10 @@ struct Tile {
     // ---------------- reading a stage ----------------
     // population I of lattice LL (rows R0 ...) of the thread's cell(s); sb: position of the first cell in row 0 of the stage.
     // EDGE: the item touches a bounce-back wall, rows may have been redirected (shift from the table)
-    template <class LL, int R0, int I, bool EDGE>
+    template <class LL, int R0, int I, bool EDGE, int PAR = PARITY>
     __device__ __forceinline__ V read_pop(const R* sb, int stage) const {
         const R* q = sb + (R0 + I) * RS;
-        if constexpr (PARITY == 0 || I == 0 || LL::c(I, 0) == 0) {
+        if constexpr (PAR == 0 || I == 0 || LL::c(I, 0) == 0) {
             if constexpr (C::PACK) { F2 v; v.v = *reinterpret_cast<const unsigned long long*>(q); return v; }
             else return *q;
         } else {
@@ -376,11 +409,11 @@ struct Tile {
             else return q[sh];
         }
     }
-    template <class LL, int R0, bool EDGE>
+    template <class LL, int R0, bool EDGE, int PAR = PARITY>
     __device__ __forceinline__ void read_pops(const R* sb, int stage, V* fl) const {
         static_for<0, LL::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            fl[i] = read_pop<LL, R0, i, EDGE>(sb, stage);
+            fl[i] = read_pop<LL, R0, i, EDGE, PAR>(sb, stage);
         });
     }
 
@@ -430,7 +463,7 @@ struct Tile {
     template <bool EDGE>
     __device__ __forceinline__ void step_cells(int stage, const TileItem& it, int t) const {
         const int x = it.xs * TILE_TX + t;
-        const R* sb = stages + (size_t)stage * NROWS * RS + H + t;
+        const R* sb = slot_base(stage) + H + t;
         // The populations are read from the stage twice -- for the moments here, for the collision below -- instead of
         // being kept in registers in between (2 x 19 + 7 values per cell, two cells per thread): the step role then fits
         // 128 registers, which buys a second team of step warps per SM.  Same values, same arithmetic.
@@ -486,6 +519,21 @@ struct Tile {
             write_pops<LS, NF, EDGE>(stage, col, hl);
         }
     }
+    // step a2 for time level t + 1 (a PSI ticket): rho^sigma in index order (Eq. 7 / 18) from the flow populations the
+    // stage holds at the NEXT parity, psi^sigma (Eq. 10 / 24 or psi = rho) to the second psi buffer
+    template <bool EDGE>
+    __device__ __forceinline__ void psi_cells(int stage, const TileItem& it, int t) const {
+        const R* sb = slot_base(stage) + H + t;
+        R* out = (R*)w.psi_out + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx + (it.xs * TILE_TX + t);
+        static_for<0, S>([&](auto sc) {
+            constexpr int s = decltype(sc)::value;
+            V fl[Q];
+            read_pops<L, s * Q, EDGE, 1 - PARITY>(sb, stage, fl);
+            V rho = fl[0];
+            static_for<1, Q>([&](auto ic) { rho = rho + fl[decltype(ic)::value]; });
+            st_global(out + (size_t)s * (size_t)p.N, psi_of(rho, p.psi_kind, p.rho0_psi));
+        });
+    }
     // team `team` takes the tickets n = team, team + TEAMS, ... of the block
     __device__ __forceinline__ void step_role(int team, unsigned n_mine, unsigned b0, unsigned stride) const {
         const int t = ((int)threadIdx.x - team * C::STEP_THREADS) * CPT;
@@ -502,19 +550,23 @@ struct Tile {
                 if (lane == 0) mbar_arrive(&empty[stage]);
                 continue;
             }
-            const TileItem it = item_of(w.step_items, b0 + n * stride);
+            const TileItem it = item_of(w.items, b0 + n * stride);
+            const bool ps = it.kind == TILE_PSI;
             if (threadIdx.x == 0) TILE_TRACE(5, n);
             const int len = min(TILE_TX, p.nx - it.xs * TILE_TX);
 #ifndef LBM_TILE_NOSTEP
             if (t < len) {
-                if (edge_row(it.y, it.z)) step_cells<WALLYZ>(stage, it, t);
-                else step_cells<false>(stage, it, t);
+                const bool edge = edge_row(it.y, it.z);
+                if (ps) {
+                    if (edge) psi_cells<WALLYZ>(stage, it, t); else psi_cells<false>(stage, it, t);
+                } else {
+                    if (edge) step_cells<WALLYZ>(stage, it, t); else step_cells<false>(stage, it, t);
+                }
             }
 #endif
             __syncwarp();
             if (threadIdx.x == 0) TILE_TRACE(6, n);
             if (lane == 0) {
-                TILE_MARK(0, n, 1);
                 st_release_cta_shared(&done[wid], ++cnt);      // after the stores of the whole warp (syncwarp above)
                 mbar_arrive(&empty[stage]);
             }
@@ -543,9 +595,8 @@ struct Tile {
                 if (m > k[tm]) {
                     fence_acq_rel_gpu();
                     for (unsigned j = k[tm] + lane; j < m; j += 32) {
-                        const TileItem it = item_of(w.step_items, b0 + (j * C::TEAMS + tm) * stride);
-                        st_relaxed(flag_of(it.xs, it.y, it.z), w.epoch);
-                        TILE_MARK(1, j * C::TEAMS + tm, 1 + 1000 * it.xs + 10000 * it.y + 10000000LL * it.z);
+                        const TileItem it = item_of(w.items, b0 + (j * C::TEAMS + tm) * stride);
+                        if (it.kind == TILE_STEP) st_relaxed(flag_of(it.xs, it.y, it.z), w.epoch);
                     }
                     TILE_TRACE(2, (m - 1) * C::TEAMS + tm);
                     left -= m - k[tm];
@@ -559,122 +610,6 @@ struct Tile {
                 __nanosleep(200);
                 if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 4); return; }
             }
-        }
-    }
-
-    // ---------------- psi warps ----------------
-    // wait until the step of the (up to) 27 tiles around (xs, y, z) is complete
-    __device__ __forceinline__ bool wait_flags(const TileItem& it) const {
-        const int l = (int)(threadIdx.x & 31);
-        const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
-        const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
-        const bool wm = D == 3 ? wall_y() : false, wsl = D == 3 ? wall_z() : wall_y();
-        bool ok = true;
-        if (l < 27) {
-            const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
-            int mm = m + dm, ss = s + ds;
-            const bool beyond = (wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0);
-            if (!beyond) {
-                const int xx = wrap(it.xs + dx, w.nxs);
-                mm = wrap(mm, nm); ss = wrap(ss, ns);
-                const int* fl = w.flags + ((size_t)ss * nm + mm) * w.nxs + xx;
-                ok = ld_acquire(fl) == w.epoch;
-                if (!ok) {
-                    const long long t0 = clock64();
-                    while (!(ok = (ld_acquire(fl) == w.epoch))) {
-                        __nanosleep(200);
-                        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 8); break; }
-                    }
-                }
-            }
-        }
-        ok = __all_sync(0xffffffffu, ok);                  // (a warp barrier: every lane's loads below come after every lane's acquire)
-        return ok;
-    }
-    // rho^sigma(t + 1) in index order (Eq. 7 / 18) from the slots of the next parity, psi^sigma to psi_out, for the
-    // 32 * VE cells of the tile from offset t0 on: every lane owns VE = 16 / sizeof(R) consecutive cells and loads one
-    // 16-byte vector per slot row (ld.global.cg.v4 / .v2); a row that is shifted by one cell in x takes the missing
-    // cell from the neighbouring lane (shuffle), the first / last lane from one extra element (periodic wrap)
-    __device__ __forceinline__ void psi_pass(const TileItem& it, int x0, int len, int t0, int lane) const {
-        constexpr int PN = 1 - PARITY;                     // parity of time level t + 1
-        constexpr int VE = 16 / B;
-        using VT = std::conditional_t<B == 4, float4, double2>;
-        constexpr int SB = (S * Q * 4 <= 96) ? S : 1;      // components loaded together (registers: 4 per vector)
-        const int nv = min(32, (len - t0) / VE);           // lanes with cells
-        const int xb = x0 + t0;
-        const int xc = xb + (lane < nv ? lane : 0) * VE;   // idle lanes repeat lane 0 (and do not store)
-        const int xleft = xb == 0 ? p.nx - 1 : xb - 1, xright = xb + nv * VE == p.nx ? 0 : xb + nv * VE;
-        R* out = (R*)w.psi_out + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx + xc;
-        static_for<0, S / SB>([&](auto bc) {
-            constexpr int s0 = decltype(bc)::value * SB;
-            VT v[SB][Q];
-            R hal[SB][Q];
-            int sxs[SB][Q];
-            static_for<0, SB>([&](auto sc) {
-                constexpr int ss = decltype(sc)::value;
-                static_for<0, Q>([&](auto ic) {
-                    constexpr int i = decltype(ic)::value;
-                    unsigned long long base;
-                    row_source<PN>((s0 + ss) * Q + i, it.y, it.z, base, sxs[ss][i]);
-                    const R* g = (const R*)base;
-                    v[ss][i] = __ldcg((const VT*)(g + xc));
-                    if constexpr (PN == 1 && L::c(i, 0) != 0) {
-                        hal[ss][i] = (R)0;
-                        if (sxs[ss][i] < 0 && lane == 0) hal[ss][i] = __ldcg(g + xleft);
-                        if (sxs[ss][i] > 0 && lane == nv - 1) hal[ss][i] = __ldcg(g + xright);
-                    }
-                });
-            });
-            static_for<0, SB>([&](auto sc) {
-                constexpr int ss = decltype(sc)::value;
-                R rho[VE];
-                static_for<0, Q>([&](auto ic) {
-                    constexpr int i = decltype(ic)::value;
-                    R e[VE];
-                    if constexpr (B == 4) { e[0] = v[ss][i].x; e[1] = v[ss][i].y; e[VE - 2] = v[ss][i].z; e[VE - 1] = v[ss][i].w; }
-                    else { e[0] = v[ss][i].x; e[1] = v[ss][i].y; }
-                    if constexpr (PN == 1 && L::c(i, 0) != 0) {
-                        const int sx = sxs[ss][i];
-                        if (sx > 0) {                      // cell x reads column x + 1
-                            R nxt = __shfl_down_sync(0xffffffffu, e[0], 1);
-                            if (lane == nv - 1) nxt = hal[ss][i];
-#pragma unroll
-                            for (int k = 0; k < VE - 1; ++k) e[k] = e[k + 1];
-                            e[VE - 1] = nxt;
-                        } else if (sx < 0) {               // cell x reads column x - 1
-                            R prv = __shfl_up_sync(0xffffffffu, e[VE - 1], 1);
-                            if (lane == 0) prv = hal[ss][i];
-#pragma unroll
-                            for (int k = VE - 1; k > 0; --k) e[k] = e[k - 1];
-                            e[0] = prv;
-                        }
-                    }
-#pragma unroll
-                    for (int k = 0; k < VE; ++k) rho[k] = i == 0 ? e[k] : rho[k] + e[k];
-                });
-                VT o;
-                if constexpr (B == 4) {
-                    o.x = psi_of(rho[0], p.psi_kind, p.rho0_psi); o.y = psi_of(rho[1], p.psi_kind, p.rho0_psi);
-                    o.z = psi_of(rho[VE - 2], p.psi_kind, p.rho0_psi); o.w = psi_of(rho[VE - 1], p.psi_kind, p.rho0_psi);
-                } else {
-                    o.x = psi_of(rho[0], p.psi_kind, p.rho0_psi); o.y = psi_of(rho[1], p.psi_kind, p.rho0_psi);
-                }
-                if (lane < nv) *(VT*)(out + (size_t)(s0 + ss) * (size_t)p.N) = o;
-            });
-        });
-    }
-    __device__ __forceinline__ void psi_role(int pw, unsigned b0, unsigned stride) const {
-        const int lane = (int)(threadIdx.x & 31);
-        const unsigned worker = b0 * TILE_PSI_WARPS + (unsigned)pw, nworkers = stride * TILE_PSI_WARPS;
-        unsigned n = 0;
-        for (unsigned ticket = worker; ticket < w.n_items; ticket += nworkers, ++n) {
-            const TileItem it = item_of(w.psi_items, ticket);
-            if (!wait_flags(it)) return;
-            if (pw == 0) TILE_TRACE(3, n);
-            const int x0 = it.xs * TILE_TX;
-            const int len = min(TILE_TX, p.nx - x0);
-            for (int t0 = 0; t0 < len; t0 += 32 * (16 / B)) psi_pass(it, x0, len, t0, lane);
-            if (pw == 0) TILE_TRACE(4, n);
         }
     }
 };
@@ -703,12 +638,8 @@ k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
     // scheduler favours the highest id among the eligible warps of a sub-partition
     constexpr int SW = C::TEAMS * C::STEP_WARPS;
     if (wid < SW) tl.step_role(wid / C::STEP_WARPS, n_mine, b0, stride);
-#ifdef LBM_TILE_NOPSI
-    else if (wid < SW + C::PSI_WARPS) return;    // developer experiment: the step role alone (wrong results)
-#endif
-    else if (wid < SW + C::PSI_WARPS) tl.psi_role(wid - SW, b0, stride);
-    else if (wid == SW + C::PSI_WARPS) tl.publish_role(n_mine, b0, stride);
-    else tl.produce(wid - (SW + C::PSI_WARPS + 1), n_mine, b0, stride);
+    else if (wid == SW) tl.publish_role(n_mine, b0, stride);
+    else tl.produce(wid - (SW + 1), n_mine, b0, stride);
 }
 
 }  // namespace lbm

@@ -10,11 +10,12 @@
 //              `py` rows of the slower-but-one axis, marched along the slowest axis.
 //   PSI item   step a2 for time level t + 1: rho^sigma(t + 1) of the row from the populations the STEP items of the 3 x 3
 //              rows around it (periodic wrap; none beyond a wall) have just written, psi(t + 1) to the OTHER psi
-//              buffer.  It becomes ready when the last of those STEP items is done and is listed right after it, so
-//              that a worker that takes PSI items in list order never waits for a dependency that comes later than
-//              the dependencies of the items behind it -- and finds the populations still in L2 (the distance is one
-//              plane of the pencil, py + 1 rows).  The rows at the edge of a pencil wait for the neighbouring pencil
-//              and are read from HBM again (a fraction 1 / py of the rows in 3D, none in 2D).
+//              buffer.  It becomes ready when the last of those STEP items is done and is
+//              listed `delay` STEP rows later: by then the blocks that took those STEP items (the list is dealt out
+//              round-robin) have long finished them, so the block that takes the PSI item does not wait, and the
+//              populations are still in L2 (the distance is one plane of the pencil, py + 1 rows, plus the delay).
+//              The rows at the edge of a pencil wait for the neighbouring pencil and are read from HBM again (a
+//              fraction 1 / py of the rows in 3D, none in 2D).
 //
 // Row coordinates: (m, s) = (y, z) for D3Q19; (0, y) for D2Q9 (the marching axis is always the slowest one).
 #pragma once
@@ -30,10 +31,11 @@ struct TileRow {
 };
 
 // py: rows per pencil (clamped to [1, nm]); wrap_m / wrap_s: that axis is periodic (else: walls, no neighbour beyond).
-// Returns the merged list (2 * nm * ns items): every STEP row followed by the PSI rows that it completes.
-// *deferred_rows (optional): PSI rows listed more than 2 * py + 8 STEP rows after their own STEP row (they wait for
-// another pencil or for the wrapped plane: their populations have left L2 by then).
-inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, bool wrap_s, int* deferred_rows) {
+// Returns the merged list (2 * nm * ns items): the STEP rows in pencil order; a PSI row that the k-th STEP row completes
+// comes right after STEP row k + delay (all that are left after the last STEP row).
+// *deferred_rows (optional): PSI rows that become ready more than 2 * py + 8 STEP rows after their own STEP row (they
+// wait for another pencil or for the wrapped plane: their populations have left L2 by then).
+inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, bool wrap_s, int delay, int* deferred_rows) {
     std::vector<TileRow> items;
     if (deferred_rows) *deferred_rows = 0;
     if (nm < 1 || ns < 1) return items;
@@ -63,6 +65,10 @@ inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, b
             }
         return n;
     };
+    if (delay < 0) delay = 0;
+    struct Ready { int32_t m, s; int64_t at; };
+    std::vector<Ready> fifo;                 // PSI rows that are ready, in the order they became ready
+    size_t head = 0;
     std::vector<uint8_t> stepped(R, 0), listed(R, 0);
     std::vector<int64_t> step_pos(R, 0);
     items.reserve(2 * R);
@@ -84,11 +90,14 @@ inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, b
                     for (int j = 0; j < nr; ++j) ready = ready && stepped[(size_t)r[j][1] * nm + r[j][0]];
                     if (!ready) continue;
                     listed[qi] = 1;
-                    items.push_back(TileRow{TILE_PSI, q[k][0], q[k][1]});
+                    fifo.push_back(Ready{q[k][0], q[k][1], n_step - 1});
                     if (deferred_rows && n_step - 1 - step_pos[qi] > 2 * (int64_t)py + 8) ++*deferred_rows;
                 }
+                for (; head < fifo.size() && fifo[head].at + delay <= n_step - 1; ++head)
+                    items.push_back(TileRow{TILE_PSI, fifo[head].m, fifo[head].s});
             }
     }
+    for (; head < fifo.size(); ++head) items.push_back(TileRow{TILE_PSI, fifo[head].m, fifo[head].s});
     return items;
 }
 

@@ -79,7 +79,7 @@ def lib():
     L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int]
     L.lbm_get_path.argtypes = [C.c_void_p]
     L.lbm_set_mask.argtypes = [C.c_void_p, C.c_void_p]
-    L.lbm_tile_schedule.argtypes = [C.c_int] * 5 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
+    L.lbm_tile_schedule.argtypes = [C.c_int] * 6 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
     L.lbm_check.argtypes = [C.c_void_p]
     L.lbm_time.restype = C.c_int64
     L.lbm_time.argtypes = [C.c_void_p]
@@ -142,18 +142,18 @@ def make_params(**kw):
     return p
 
 
-def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True):
+def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True, delay_rows=0):
     """The resident-tile kernel's row schedule as an (n, 3) int32 array of (kind, m, s), and the number of psi rows
     that wait for another pencil; host-only call (kind 0: step of the row, 1: psi of the next time level)."""
     import numpy as np
     L = lib()
     n = C.c_size_t(0)
     lead = C.c_int(0)
-    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), None, 0, C.byref(n), C.byref(lead))
+    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), int(delay_rows), None, 0, C.byref(n), C.byref(lead))
     if rc != 0:
         raise LbmError(rc, last_error())
     out = np.zeros((n.value, 3), np.int32)
-    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), out.ctypes.data, n.value, C.byref(n), C.byref(lead))
+    rc = L.lbm_tile_schedule(nm, ns, rows_per_pencil, int(wrap_m), int(wrap_s), int(delay_rows), out.ctypes.data, n.value, C.byref(n), C.byref(lead))
     if rc != 0:
         raise LbmError(rc, last_error())
     return out, lead.value

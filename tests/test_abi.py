@@ -155,15 +155,16 @@ def test_product_path_never_touches_the_oracle():
 @pytest.mark.parametrize("nm,ns,py", [(1, 1, 1), (1, 7, 1), (1, 64, 1), (5, 4, 2), (8, 8, 3), (8, 8, 8), (2, 2, 1), (3, 1, 2),
                                       (16, 9, 5), (6, 5, 100), (40, 12, 7)])
 @pytest.mark.parametrize("wrap_m,wrap_s", [(True, True), (False, True), (True, False), (False, False)])
-def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s):
+@pytest.mark.parametrize("delay", [0, 3])
+def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s, delay):
     """Host logic of the resident-tile kernel (tile_schedule.h).  Every row has exactly one STEP item (pencil order)
     and exactly one PSI item (psi of the next time level, R9).  A PSI item needs the step of the 3 x 3 rows around
-    its row (periodic wrap or wall; Eq. 5 / 7): it is listed right after the LAST of their STEP items -- never
-    before (the psi warps would wait for every later step), never later than needed (the populations would leave
-    L2) -- so the PSI items are ordered by the time they become ready.  Rows that wait for another pencil or for the
-    wrapped plane are re-read from HBM: they must stay a small fraction."""
+    its row (periodic wrap or wall; Eq. 5 / 7): it is listed exactly `delay` STEP rows after the LAST of their STEP
+    items (or at the very end) -- never before (the block that takes it would wait for a later step), never later
+    than asked (the populations would leave L2) -- so the PSI items are ordered by the time they become ready.  Rows
+    that wait for another pencil or for the wrapped plane are re-read from HBM: they must stay a small fraction."""
     import paper_2502_12955_b200 as pkg
-    it, deferred = pkg.lbm.tile_schedule(nm, ns, py, wrap_m, wrap_s)
+    it, deferred = pkg.lbm.tile_schedule(nm, ns, py, wrap_m, wrap_s, delay)
     assert len(it) == 2 * nm * ns
     step_pos, psi_pos = {}, {}
     for k, (kind, m, s) in enumerate(it.tolist()):
@@ -187,7 +188,8 @@ def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s):
                 deps.append(step_pos[(mm % nm, ss % ns)])
         last = max(deps)
         assert last < k                                   # after its last dependency ...
-        assert all(kind == 1 for kind, _, _ in it[last + 1:k].tolist())     # ... with no step item in between
+        between = sum(1 for kind, _, _ in it[last + 1:k].tolist() if kind == 0)
+        assert between == delay or (between < delay and all(kind == 1 for kind, _, _ in it[k:].tolist()))     # ... by `delay` step rows
         if max(order[(it[d][1], it[d][2])] for d in deps) - order[(m, s)] > 2 * p + 8:
             late += 1
     assert late == deferred
