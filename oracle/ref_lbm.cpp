@@ -151,6 +151,7 @@ struct Sim : ref_ctx {
     /* constants, rounded once to R */
     R w[19], ws[7];
     R omega[2], tau_r[2], omega_c, inv_cs2g;
+    R omega_s, inv_rho_solid;      /* solid-phase internal-energy lattice: 1/tau_{e,s} (0: off), 1/rho_s */
     R cfw[2][19];          /* (1 - 1/(2 tau^s)) w_i: prefactor of the Guo term in Eq. 15 */
     R w6[19];              /* 6 w_i = 2 w_i / c_s^2: moving-wall bounce-back (DESIGN R24) */
     R G[2][2], G_ads[2], rho0_psi, force[3], k_react;
@@ -201,6 +202,8 @@ struct Sim : ref_ctx {
             for (int t = 0; t < 2; ++t) G[s][t] = (R)pp.G[s][t];
         }
         omega_c = (R)(1.0 / pp.tau_c);                     /* Eq. 34 */
+        omega_s = pp.tau_s > 0.0 ? (R)(1.0 / pp.tau_s) : (R)0;     /* Eq. 31 */
+        inv_rho_solid = (R)(1.0 / pp.rho_solid);
         inv_cs2g = (R)((double)d / (1.0 - w0s));           /* 1/c_{s,g}^2, Eq. 35, DESIGN R6 */
         rho0_psi = (R)pp.rho0_psi;
         psi_wall = pp.rho_wall > 0.0 ? psi_of((R)pp.rho_wall) : (R)0;
@@ -232,6 +235,20 @@ struct Sim : ref_ctx {
         }
         out = cell_of(q[0], q[1], q[2]);
         return !solid[out];          /* a solid node reflects like a wall */
+    }
+    /* the same seen from a SOLID node (solid-phase lattice, Eq. 31): its neighbour must be a solid node too; a fluid
+     * node or a wall reflects (adiabatic interface: the conjugate coupling Eq. 37-40 is out of scope) */
+    bool solid_neighbour(int x, int y, int z, const int* c, size_t& out) const {
+        int q[3] = {x + c[0], y + c[1], z + c[2]};
+        const int n[3] = {nx, ny, nz};
+        for (int a = 0; a < 3; ++a) {
+            if (q[a] < 0 || q[a] >= n[a]) {
+                if (p.bc[a] == 1) return false;
+                q[a] = (q[a] + n[a]) % n[a];
+            }
+        }
+        out = cell_of(q[0], q[1], q[2]);
+        return solid[out] != 0;
     }
 
     /* velocity of the wall a population leaving (x, y, z) along c hits: the first wall axis (x, y, z order) it crosses */
@@ -370,7 +387,22 @@ struct Sim : ref_ctx {
                         for (int s = 0; s < S; ++s)
                             for (int i = 0; i < Q; ++i) F_(fnew, s, i, cell) = F_(f, s, i, cell);
                         if (has_scalar) for (int i = 0; i < Qs; ++i) H_(hnew, i, cell) = H_(h, i, cell);
-                        if (has_thermal) for (int i = 0; i < Q; ++i) H_(gnew, i, cell) = H_(g, i, cell);
+                        if (has_thermal && omega_s > (R)0) {
+                            /* solid-phase internal-energy lattice, Eq. 31 with g^eq_{s,i} = w_i rho_s eps_s
+                             * (Eq. 32, no velocity) and rho_s eps_s = sum_i g_{s,i} (Eq. 33): pure diffusion with
+                             * alpha_s = (tau_{e,s} - 1/2) / 3 among the solid nodes */
+                            R E = (R)0;
+                            for (int i = 0; i < Q; ++i) E = E + H_(g, i, cell);
+                            for (int i = 0; i < Q; ++i) {
+                                R gi = H_(g, i, cell);
+                                R gstar = std::fma(-omega_s, std::fma(-w[i], E, gi), gi);
+                                size_t nb;
+                                if (solid_neighbour(x, y, z, L.c[i], nb)) H_(gnew, i, nb) = gstar;
+                                else H_(gnew, L.opp[i], cell) = gstar;
+                            }
+                        } else if (has_thermal) {
+                            for (int i = 0; i < Q; ++i) H_(gnew, i, cell) = H_(g, i, cell);
+                        }
                         continue;
                     }
                     R u[3] = {ub[cell], ub[N + cell], ub[2 * N + cell]};
@@ -602,8 +634,13 @@ struct Sim : ref_ctx {
             for (size_t cell = 0; cell < N; ++cell) {
                 R C = (R)0;
                 if (has_thermal) {      /* internal energy eps = sum_i g_i / rho, Eq. 29 */
-                    for (int i = 0; i < Q && !solid[cell]; ++i) C = C + H_(g, i, cell);
-                    if (!solid[cell]) C = C * ((R)1 / rho[cell]);
+                    if (!solid[cell]) {
+                        for (int i = 0; i < Q; ++i) C = C + H_(g, i, cell);
+                        C = C * ((R)1 / rho[cell]);
+                    } else if (omega_s > (R)0) {   /* eps_s = sum_i g_{s,i} / rho_s, Eq. 33 */
+                        for (int i = 0; i < Q; ++i) C = C + H_(g, i, cell);
+                        C = C * inv_rho_solid;
+                    }
                     Cc[cell] = C;
                     continue;
                 }
@@ -670,6 +707,10 @@ ref_ctx* ref_create(int nx, int ny, int nz, int lattice, int model, const ref_pa
     for (int s = 0; s < S; ++s)
         if (!(p->tau[s] > 0.5)) { g_err = "tau must exceed 0.5"; return nullptr; }
     if ((model == REF_SC2_ADE || model == REF_BGK_T) && !(p->tau_c > 0.5)) { g_err = "tau_c must exceed 0.5"; return nullptr; }
+    if (p->tau_s != 0.0 && (model != REF_BGK_T || !(p->tau_s > 0.5) || !(p->rho_solid > 0.0))) {
+        g_err = "tau_s (solid-phase lattice) needs REF_BGK_T, tau_s > 0.5 and rho_solid > 0";
+        return nullptr;
+    }
     for (int a = 0; a < 3; ++a) {
         if (p->bc[a] != 0 && p->bc[a] != 1) { g_err = "bad bc"; return nullptr; }
 

@@ -52,6 +52,9 @@ typedef struct ref_params {
     double   G_ads[2];      /* fluid-solid adhesion coefficient per component, Eq. 14; solid = beyond a wall */
     double   rho_wall;      /* SC1: density rho_s of the solid nodes in Eq. 12; 0: no such term */
     double   wall_u[3][2][3]; /* velocity of the wall at the low / high face of each wall axis (moving-wall bounce-back) */
+    double   tau_s;         /* REF_BGK_T: relaxation time tau_{e,s} = 3 alpha_s + 1/2 of the solid-phase internal-energy lattice g_{s,i} on
+                             * the solid nodes of the mask, Eq. 31-33; 0: solid nodes carry no lattice */
+    double   rho_solid;     /* rho_s of Eq. 32-33 (eps_s = sum_i g_{s,i} / rho_s) */
 } ref_params;
 
 typedef struct ref_ctx ref_ctx;

@@ -80,9 +80,9 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+__device__ __forceinline__ int ld_relaxed(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ void st_relaxed(int* p, int v) {
@@ -275,32 +275,38 @@ struct Tile {
     }
 
     // ---------------- producer ----------------
-    // wait until the step of the (up to) 27 tiles around (xs, y, z) is complete
-    __device__ __forceinline__ bool wait_flags(const TileItem& it) const {
+    // The flag this lane looks at for a PSI ticket at (xs, y, z): lane l < 27 has one of the (up to) 27 tiles around it
+    // (nullptr: no such tile beyond a wall, or lane >= 27)
+    __device__ __forceinline__ const int* flag_around(const TileItem& it) const {
         const int l = (int)(threadIdx.x & 31);
         const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
         const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
         const bool wm = D == 3 ? wall_y() : false, wsl = D == 3 ? wall_z() : wall_y();
-        bool ok = true;
-        if (l < 27) {
-            const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
-            int mm = m + dm, ss = s + ds;
-            const bool beyond = (wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0);
-            if (!beyond) {
-                const int xx = wrap(it.xs + dx, w.nxs);
-                mm = wrap(mm, nm); ss = wrap(ss, ns);
-                const int* fl = w.flags + ((size_t)ss * nm + mm) * w.nxs + xx;
-                ok = ld_acquire(fl) == w.epoch;
-                if (!ok) {
-                    const long long t0 = clock64();
-                    while (!(ok = (ld_acquire(fl) == w.epoch))) {
-                        __nanosleep(200);
-                        if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 8); break; }
-                    }
+        if (l >= 27) return nullptr;
+        const int dx = l % 3 - 1, dm = (l / 3) % 3 - 1, ds = l / 9 - 1;
+        int mm = m + dm, ss = s + ds;
+        if ((wm && (mm < 0 || mm >= nm)) || (wsl && (ss < 0 || ss >= ns)) || (D == 2 && dm != 0)) return nullptr;
+        mm = wrap(mm, nm); ss = wrap(ss, ns);
+        return w.flags + ((size_t)ss * nm + mm) * w.nxs + wrap(it.xs + dx, w.nxs);
+    }
+    // wait until the step of the tiles around a PSI ticket is complete.  seen: the value a relaxed load of the lane's
+    // flag returned one ticket earlier (the load's latency is hidden behind the previous ticket).  Once every lane has
+    // SEEN the epoch, the copies issued afterwards read what was published before the flags: they are issued after the
+    // loads have returned and read L2, where the publisher's fence has made the populations visible.  Otherwise: poll
+    // with acquire loads.
+    __device__ __forceinline__ bool wait_flags(const int* fl, int seen) const {
+        bool ok = fl == nullptr || seen == w.epoch;
+        if (!__all_sync(0xffffffffu, ok)) {
+            if (!ok) {
+                const long long t0 = clock64();
+                while (!(ok = (ld_acquire(fl) == w.epoch))) {
+                    __nanosleep(200);
+                    if (clock64() - t0 > TILE_TIMEOUT_CYCLES) { atomicOr(w.status, 8); break; }
                 }
             }
+            ok = __all_sync(0xffffffffu, ok);              // (a warp barrier: every lane's copies come after every lane's acquire)
         }
-        return __all_sync(0xffffffffu, ok);                // (a warp barrier: every lane's copies below come after every lane's acquire)
+        return ok;
     }
     // Row r of a ticket of kind K at parity PAR (STEP: the parity of this launch, all rows; PSI: the next parity, the
     // flow populations only): where it comes from relative to the ticket's row.  nbr: element 0 of row (0, 0) of the
@@ -345,8 +351,19 @@ struct Tile {
         const int r = lane < 16 ? pwid + TILE_PROD_WARPS * lane : NROWS;
         const RowDesc d_step = row_desc(r, PARITY, false), d_psi = row_desc(r, 1 - PARITY, true);
         const unsigned long long pol = l2_evict_first();
+        // the ticket after the current one and (PSI tickets) the flag value are loaded one ticket ahead
+        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : TileItem{0, 0, 0, TILE_STEP};
+        const int* nfl = nxt.kind == TILE_PSI ? flag_around(nxt) : nullptr;
+        int nseen = nfl ? ld_relaxed(nfl) : 0;
         for (unsigned n = 0; n < n_mine; ++n) {
-            const TileItem it = item_of(w.items, b0 + n * stride);
+            const TileItem it = nxt;
+            const int* fl = nfl;
+            const int seen = nseen;
+            if (n + 1 < n_mine) {
+                nxt = item_of(w.items, b0 + (n + 1) * stride);
+                nfl = nxt.kind == TILE_PSI ? flag_around(nxt) : nullptr;
+                nseen = nfl ? ld_relaxed(nfl) : 0;
+            }
             const bool ps = it.kind == TILE_PSI;
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
@@ -354,7 +371,7 @@ struct Tile {
                             ps ? d_psi.dz : d_step.dz, ps ? d_psi.sx : d_step.sx};
             // a PSI ticket reads what the step of the tiles around it has written: listed well after them (tile_schedule.h),
             // so this wait is a formality -- but it is what makes the read correct
-            if (it.kind == TILE_PSI && !wait_flags(it)) return;
+            if (ps && !wait_flags(fl, seen)) return;
             if (!mbar_wait(&empty[stage], ph ^ 1u, w.status, 2)) return;
             if (pwid == 0) TILE_TRACE(7, n);
             const int x0 = it.xs * TILE_TX;
@@ -539,6 +556,7 @@ struct Tile {
         const int t = ((int)threadIdx.x - team * C::STEP_THREADS) * CPT;
         const int lane = (int)(threadIdx.x & 31), wid = (int)(threadIdx.x >> 5);
         unsigned cnt = 0;
+        TileItem nxt = (unsigned)team < n_mine ? item_of(w.items, b0 + (unsigned)team * stride) : TileItem{0, 0, 0, TILE_STEP};
         for (unsigned n = 0; n < n_mine; ++n) {
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
@@ -550,7 +568,8 @@ struct Tile {
                 if (lane == 0) mbar_arrive(&empty[stage]);
                 continue;
             }
-            const TileItem it = item_of(w.items, b0 + n * stride);
+            const TileItem it = nxt;                       // (loaded one own ticket ahead)
+            if (n + C::TEAMS < n_mine) nxt = item_of(w.items, b0 + (n + C::TEAMS) * stride);
             const bool ps = it.kind == TILE_PSI;
             if (threadIdx.x == 0) TILE_TRACE(5, n);
             const int len = min(TILE_TX, p.nx - it.xs * TILE_TX);

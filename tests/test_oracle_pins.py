@@ -1037,6 +1037,63 @@ def test_thermal_uniform_state_and_init():
     assert np.abs(m["u"][0]).max() > 1e-5
 
 
+@pytest.mark.parametrize("lattice,grid,axis", [("D2Q9", (5, 40, 1), 1), ("D3Q19", (4, 3, 40), 2), ("D2Q9", (40, 6, 1), 0)])
+def test_solid_phase_energy_lattice(lattice, grid, axis):
+    """Solid-phase internal-energy lattice on the solid nodes of the mask, Eq. 31-33: g^eq_s = w_i rho_s
+    eps_s (no velocity), tau_{e,s} = 3 alpha_s + 1/2, eps_s = sum_i g_s / rho_s.  A solid slab of H nodes between fluid
+    (adiabatic interface: halfway reflection, the wall half a cell outside the nodes) has the eigenmode
+    cos(pi (j + 1/2) / H), which must decay as exp(-alpha_s (pi / H)^2 t); sum g_s over the solid and sum g over the fluid
+    are conserved separately (nothing crosses the interface); the fluid keeps its uniform eps; eps_s is scaled by
+    1 / rho_s; with tau_s = 0 the solid nodes carry no lattice (all outputs zero there)."""
+    c, w = lattice_table(lattice)
+    n = grid[axis]
+    a, H = 8, 24
+    shape = (grid[2], grid[1], grid[0])
+    coord = np.arange(n)
+    idx = [None] * 3; idx[2 - axis] = slice(None)
+    band = np.broadcast_to(((coord >= a) & (coord < a + H))[tuple(idx)], shape).ravel()
+    mode = np.broadcast_to(np.cos(np.pi * (coord - a + 0.5) / H)[tuple(idx)], shape).ravel()
+    tau_s, tau_c, rho_s, rho_f = 1.1, 0.7, 2.5, 1.2
+
+    def setup(ts):
+        r = RefLBM(*grid, lattice, "BGK_T", precision=64, tau=(0.9, 0.9), tau_c=tau_c, tau_s=ts, rho_solid=rho_s)
+        eps = np.where(band, 1.0 + 0.1 * mode, 0.6)
+        f = (w * rho_f)[:, None] * np.ones(r.N)
+        g = w[:, None] * (np.where(band, rho_s, rho_f) * eps)[None, :]
+        r.set_populations(np.concatenate([f.ravel(), g.ravel()]))
+        r.set_mask(band)
+        return r, g
+
+    r, g0 = setup(tau_s)
+    e0 = r.get_macros()["C"]
+    assert np.allclose(e0[band], (1.0 + 0.1 * mode)[band], atol=1e-15) and np.allclose(e0[~band], 0.6, atol=1e-15)
+    T = 300
+    r.step(T)
+    e1 = r.get_macros()["C"]
+    amp = ((e1 - 1.0) * mode)[band].sum() / (mode ** 2)[band].sum()
+    alpha_s = (tau_s - 0.5) / 3
+    assert abs(amp / (0.1 * np.exp(-alpha_s * (np.pi / H) ** 2 * T)) - 1) < 3e-3
+    assert abs(np.exp(-(tau_c - 0.5) / 3 * (np.pi / H) ** 2 * T) / np.exp(-alpha_s * (np.pi / H) ** 2 * T) - 1) > 0.05   # tau_c would not pass
+    _, g1 = r.split_populations(r.get_populations())
+    assert abs(g1[:, band].sum() - g0[:, band].sum()) < 1e-12 * g0[:, band].sum()
+    assert abs(g1[:, ~band].sum() - g0[:, ~band].sum()) < 1e-12 * g0[:, ~band].sum()
+    assert np.abs(e1[~band] - 0.6).max() < 1e-13
+    # without the solid lattice the solid nodes are inert and read zero
+    r0, _ = setup(0.0)
+    r0.step(5)
+    m0 = r0.get_macros()
+    assert np.all(m0["C"][band] == 0.0) and np.abs(m0["C"][~band] - 0.6).max() < 1e-13
+    _, g2 = r0.split_populations(r0.get_populations())
+    assert np.array_equal(g2[:, band], g0[:, band])
+
+
+def test_solid_phase_lattice_needs_the_thermal_model():
+    with pytest.raises(Exception):
+        RefLBM(4, 4, 1, "D2Q9", "BGK", precision=64, tau=(0.9, 0.9), tau_s=0.8)
+    with pytest.raises(Exception):
+        RefLBM(4, 4, 1, "D2Q9", "BGK_T", precision=64, tau=(0.9, 0.9), tau_c=0.8, tau_s=0.4)
+
+
 def test_single_component_solid_term_of_eq12():
     """Eq. 12: next to a solid node the single-component force gains -G psi(x) sum_solid w_i psi(rho_s) c_i.
     Uniform fluid next to a flat wall with inward normal n: sum_fluid w_i c_i = +n/6, sum_solid w_i c_i = -n/6, so the
