@@ -96,6 +96,12 @@ typedef struct lbm_params {
                                bc[axis] == 1).  A population reflected by a moving wall loses
                                2 w_i rho (c_i . u_w) / c_s^2 (Couette flow Eq. 41).  LBM_BGK with
                                forcing 0 on LBM_PATH_REGISTER only */
+    double   tau_s;         /* LBM_BGK_T with a solid-node mask: relaxation time tau_{e,s} = 3 alpha_s + 1/2 of the
+                               solid-phase internal-energy lattice g_{s,i} on the solid nodes, Eq. 31-33
+                               (PAPER.md:316-327): g^eq_s = w_i rho_s eps_s, pure diffusion among solid nodes, the
+                               fluid-solid interface is adiabatic (Eq. 37-40 are out of scope); the C output reads
+                               eps_s = sum_i g_{s,i} / rho_solid there.  0: solid nodes carry no lattice */
+    double   rho_solid;     /* rho_s of Eq. 32-33, > 0 when tau_s is set */
     void*    workspace;     /* DEVICE memory of >= lbm_workspace_bytes() bytes, 256-byte aligned (e.g. from
                                torch), or NULL: the library allocates (cudaMalloc) and frees it */
     void*    stream;        /* cudaStream_t, or NULL for the legacy default stream */

@@ -135,12 +135,12 @@ struct Launch {
     }
 
     template <class LL, bool TOC>
-    static void permute2(const KP<R>& p, int parity, int wmode, R* slots, R* canon, int nl, cudaStream_t st) {
+    static void permute2(const KP<R>& p, int parity, int wmode, R* slots, R* canon, int nl, cudaStream_t st, bool solid_lattice = false) {
         const dim3 g = grid_for(p);
         if (parity) {
-            with_int<3>(wmode, [&](auto W) { k_permute<R, LL, 1, decltype(W)::value, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl); });
+            with_int<3>(wmode, [&](auto W) { k_permute<R, LL, 1, decltype(W)::value, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl, solid_lattice); });
         } else {
-            k_permute<R, LL, 0, 0, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl);
+            k_permute<R, LL, 0, 0, TOC><<<g, block_for(p), 0, st>>>(p, slots, canon, nl, false);
         }
     }
     static cudaError_t permute(const void* kp, int model, int parity, int wmode, void* canon, int to_canonical,
@@ -156,10 +156,11 @@ struct Launch {
             if (to_canonical) permute2<LS, true>(p, parity, wmode, p.h, ch, 1, st);
             else permute2<LS, false>(p, parity, wmode, p.h, ch, 1, st);
         }
-        if (model == M_BGK_T) {     // the internal-energy lattice lives on the flow lattice
+        if (model == M_BGK_T) {     // the internal-energy lattice lives on the flow lattice; solid nodes may carry it too (Eq. 31)
             R* ch = cf + (size_t)S * L::Q * (size_t)p.N;
-            if (to_canonical) permute2<L, true>(p, parity, wmode, p.h, ch, 1, st);
-            else permute2<L, false>(p, parity, wmode, p.h, ch, 1, st);
+            const bool sl = p.omega_s > (R)0;
+            if (to_canonical) permute2<L, true>(p, parity, wmode, p.h, ch, 1, st, sl);
+            else permute2<L, false>(p, parity, wmode, p.h, ch, 1, st, sl);
         }
         return cudaGetLastError();
     }

@@ -53,6 +53,7 @@ struct KP {
     R rho0_psi;
     R force[3];
     R k_react;
+    R omega_s, inv_rho_solid; // solid-phase internal-energy lattice on the solid nodes (M_BGK_T): 1/tau_{e,s} (0: none), 1/rho_s; Eq. 31-33
 };
 
 struct InitArgs {
@@ -89,7 +90,7 @@ struct Nbr {
     bool solid;            // this cell is a solid node itself
 
     template <class R>
-    __device__ __forceinline__ Nbr(const KP<R>& p, int x, int y, int z) {
+    __device__ __forceinline__ Nbr(const KP<R>& p, int x, int y, int z, bool solid_lattice = false) {
         const int nx = p.nx, ny = p.ny;
         xx[0] = (x == 0) ? nx - 1 : x - 1; xx[1] = x; xx[2] = (x == nx - 1) ? 0 : x + 1;
         ry[0] = ((y == 0) ? ny - 1 : y - 1) * nx; ry[1] = y * nx; ry[2] = ((y == ny - 1) ? 0 : y + 1) * nx;
@@ -117,6 +118,9 @@ struct Nbr {
                         if (p.mask[(rz[cz + 1] + ry[cy + 1]) + xx[cx + 1]]) blocked |= 1u << o;
                     }
                 });
+                // a solid node that carries the solid-phase lattice (Eq. 31): its neighbours must be solid nodes too,
+                // the fluid nodes reflect (adiabatic interface) -- the same slot map with the roles exchanged
+                if (solid && solid_lattice) blocked = ~blocked;
             }
         } else {
             lo[0] = lo[1] = lo[2] = hi[0] = hi[1] = hi[2] = false;
@@ -528,8 +532,28 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     using LS = typename ScalarOf<L>::type;
     constexpr int S = MT::S, Q = L::Q;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, WALLS> nb(p, x, y, z);
-    if (WALLS == 2 && nb.solid) return;              // solid nodes are not updated
+    const bool solid_lattice = MT::THERMAL && WALLS == 2 && p.omega_s > (R)0;
+    const Nbr<L::D, WALLS> nb(p, x, y, z, solid_lattice);
+    if (WALLS == 2 && nb.solid) {                    // solid nodes are not updated ...
+        if constexpr (MT::THERMAL && WALLS == 2) {
+            if (solid_lattice) {
+                // ... except for the solid-phase internal-energy lattice, Eq. 31: g^eq_{s,i} = w_i rho_s eps_s
+                // (Eq. 32) with rho_s eps_s = sum_i g_{s,i} (Eq. 33); streams among solid nodes, reflected by fluid nodes
+                R gl[Q];
+                load_pops<L, PARITY, WALLS>(p.h, nb, N, gl);
+                R E = gl[0];
+                static_for<1, Q>([&](auto ic) { E = E + gl[decltype(ic)::value]; });
+                static_for<0, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    gl[i] = vfma(-p.omega_s, vfma((R)(-L::w(i)), E, gl[i]), gl[i]);
+                });
+                Nbr<L::D, WALLS> ns = nb;
+                asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));
+                store_pops<L, PARITY, WALLS>(p.h, ns, N, gl);
+            }
+        }
+        return;
+    }
 
     R fl[S][Q];
     static_for<0, S>([&](auto sc) {
@@ -665,13 +689,26 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<D, WALLS> nb(p, x, y, z);
+    const bool solid_lattice = MT::THERMAL && WALLS == 2 && p.omega_s > (R)0;
+    const Nbr<D, WALLS> nb(p, x, y, z, solid_lattice);
     const int cell = nb.cell;
     if (WALLS == 2 && nb.solid) {        // no fluid here: every field reads as zero
         if (rho_o) static_for<0, S>([&](auto sc) { rho_o[(size_t)decltype(sc)::value * N + cell] = (R)0; });
         if (u_o) static_for<0, D>([&](auto ac) { u_o[(size_t)decltype(ac)::value * N + cell] = (R)0; });
         if (phi_o) phi_o[cell] = (R)0;
-        if (C_o) C_o[cell] = (R)0;
+        if (C_o) {
+            R eps_s = (R)0;
+            if constexpr (MT::THERMAL && WALLS == 2) {
+                if (solid_lattice) {     // eps_s = sum_i g_{s,i} / rho_s, Eq. 33
+                    R gl[Q];
+                    load_pops<L, PARITY, WALLS>(p.h, nb, N, gl);
+                    R E = gl[0];
+                    static_for<1, Q>([&](auto ic) { E = E + gl[decltype(ic)::value]; });
+                    eps_s = E * p.inv_rho_solid;
+                }
+            }
+            C_o[cell] = eps_s;
+        }
         if (F_o) static_for<0, S * D>([&](auto kc) { F_o[(size_t)decltype(kc)::value * N + cell] = (R)0; });
         return;
     }
@@ -720,11 +757,11 @@ __global__ void __launch_bounds__(BLOCK) k_macros(const __grid_constant__ KP<R> 
 // canonical populations f_i(x,t) out of the slot array at the current parity (and back)
 template <class R, class L, int PARITY, int WALLS, bool TO_CANONICAL>
 __global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R> p, R* __restrict__ slots,
-                                                   R* __restrict__ canon, int n_lattices) {
+                                                   R* __restrict__ canon, int n_lattices, bool solid_lattice) {
     int x, y, z;
     if (!thread_cell(p.nx, x, y, z)) return;
     const size_t N = (size_t)p.N;
-    const Nbr<L::D, WALLS> nb(p, x, y, z);
+    const Nbr<L::D, WALLS> nb(p, x, y, z, WALLS == 2 && solid_lattice);   // solid_lattice: the solid nodes carry this lattice too (Eq. 31)
     const int cell = nb.cell;
     for (int s = 0; s < n_lattices; ++s) {
         R* sb = slots + (size_t)s * L::Q * N;
@@ -732,7 +769,7 @@ __global__ void __launch_bounds__(BLOCK) k_permute(const __grid_constant__ KP<R>
         static_for<0, L::Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             R* P = slot_of<L, PARITY, WALLS, i>(sb, nb, N);
-            if (WALLS == 2 && nb.solid) P = sb + ((size_t)i * N + cell);      // a solid node keeps its values in its own slots
+            if (WALLS == 2 && nb.solid && !solid_lattice) P = sb + ((size_t)i * N + cell);      // an inert solid node keeps its values in its own slots
             if constexpr (TO_CANONICAL) cb[(size_t)i * N + cell] = *P;
             else *P = cb[(size_t)i * N + cell];
         });

@@ -82,6 +82,8 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     if (model != LBM_BGK && p->psi_kind == 0 && !(p->rho0_psi > 0.0)) return "rho0_psi must be > 0";
     if (p->w0_scalar < 0.0 || p->w0_scalar >= 1.0) return "w0_scalar must lie in [0, 1)";
     if (p->rho_wall < 0.0) return "rho_wall must be >= 0";
+    if (p->tau_s != 0.0 && (model != LBM_BGK_T || !(p->tau_s > 0.5) || !(p->rho_solid > 0.0)))
+        return "tau_s (solid-phase lattice) needs LBM_BGK_T, tau_s > 0.5 and rho_solid > 0";
     if (p->init_kind < LBM_INIT_REST || p->init_kind > LBM_INIT_RANDOM_DROPLETS) return "unknown init_kind";
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
@@ -204,6 +206,8 @@ void fill_kp(lbm::KP<R>& k, const lbm_ctx* c) {
     }
     k.rho0_psi = (R)p.rho0_psi;
     k.k_react = (R)p.k_react;
+    k.omega_s = p.tau_s > 0.0 ? (R)(1.0 / p.tau_s) : (R)0;
+    k.inv_rho_solid = p.tau_s > 0.0 ? (R)(1.0 / p.rho_solid) : (R)0;
 }
 
 // host copy of the counter-based generator (integer arithmetic, bit-identical to the device one)

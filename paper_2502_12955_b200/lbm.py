@@ -40,6 +40,7 @@ class LbmParams(C.Structure):
         ("rho_in", C.c_double), ("rho_out", C.c_double), ("radius", C.c_double), ("width", C.c_double),
         ("noise_amp", C.c_double), ("u0", C.c_double), ("rmin", C.c_double), ("rmax", C.c_double),
         ("vol_frac", C.c_double), ("G_ads", C.c_double * 2), ("rho_wall", C.c_double), ("wall_u", ((C.c_double * 3) * 2) * 3),
+        ("tau_s", C.c_double), ("rho_solid", C.c_double),
         ("workspace", C.c_void_p), ("stream", C.c_void_p),
     ]
 
@@ -134,6 +135,8 @@ def make_params(**kw):
     ga = kw.get("G_ads", (0.0, 0.0))
     p.G_ads[0], p.G_ads[1] = float(ga[0]), float(ga[1])
     p.rho_wall = float(kw.get("rho_wall", 0.0))
+    p.tau_s = float(kw.get("tau_s", 0.0))
+    p.rho_solid = float(kw.get("rho_solid", 1.0))
     for (axis, side), v in kw.get("wall_u", {}).items():      # {(axis, side): (ux, uy, uz)}, side 0 = low, 1 = high face
         for a in range(3):
             p.wall_u[axis][side][a] = float(v[a])

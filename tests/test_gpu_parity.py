@@ -505,3 +505,186 @@ def test_default_path_of_large_shan_chen_grids(gpu):
     c.init_from_seed(3)
     c.step(2)
     assert c.get_path() == "register"
+
+
+MASK_CASES = [
+    ("cfg1", (20, 13, 1), dict(force=(1e-5, 2e-5, 0.0))),
+    ("cfg1", (132, 9, 1), {}),
+    ("cfg4", (9, 8, 7), dict(bc=(0, 0, 1))),
+    ("cfg4", (12, 6, 5), dict(bc=(0, 0, 0), precision=32)),
+    ("cfg4", (7, 6, 5), dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, 0.0, 0.0)})),
+    ("cfg2", (16, 12, 1), dict(radius=4.0, G_ads=(-0.3, 0.0))),
+    ("cfgT", (9, 8, 6), {}),
+    # solid-phase internal-energy lattice on the solid nodes (Eq. 31-33), walls in z / fully periodic / 2D fp32
+    ("cfgT", (9, 8, 6), dict(tau_s=0.9, rho_solid=2.0)),
+    ("cfgT", (7, 6, 5), dict(tau_s=1.4, rho_solid=0.5, bc=(0, 0, 0), force=(0.0, 0.0, 0.0))),
+    ("cfgT2", (13, 11, 1), dict(tau_s=0.75, rho_solid=1.5, precision=32)),
+    # Eq. 12 solid term next to solid nodes of the mask (and next to walls as well)
+    ("cfg2", (16, 12, 1), dict(radius=4.0, rho_wall=1.5)),
+    ("cfg2", (14, 10, 1), dict(radius=3.0, rho_wall=0.4, G_ads=(-0.2, 0.0), bc=(0, 1, 0))),
+    ("cfg3", (14, 11, 1), dict(G_ads=(-0.2, 0.3))),
+    ("cfg5", (10, 8, 6), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, G_ads=(0.2, -0.2))),
+    ("cfg5", (8, 7, 6), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, forcing=1, bc=(0, 1, 0), precision=64, tau=(0.9, 1.2))),
+]
+
+
+@pytest.mark.parametrize("name,grid,over", MASK_CASES, ids=lambda v: str(v).replace(" ", ""))
+def test_solid_mask_matches_oracle(gpu, name, grid, over):
+    """lbm_set_mask: a random 15 % of the nodes solid (isolated nodes, clusters, nodes next to walls and across the
+    periodic seam): populations at every step 1..12 (odd and even AA parity), macros and forces against the oracle."""
+    cfg = workloads.config(name, grid=grid, **over)
+    ref, dev = make_pair(gpu, cfg)
+    mask = (np.random.default_rng(1).random(ref.N) < 0.15).astype(np.uint8)
+    ref.init_from_seed(3)
+    dev.set_populations(torch.from_numpy(ref.get_populations()))
+    ref.set_mask(mask)
+    dev.set_mask(mask)
+    exact = not (cfg["model"] == "SC1" and cfg["params"].get("psi_kind", 0) == 0)
+    for step in range(1, 13):
+        ref.step(1)
+        dev.step(1)
+        fr = ref.get_populations()
+        fd = dev.get_populations().cpu().numpy()
+        if exact:
+            assert np.array_equal(fr, fd), "step %d" % step
+        else:
+            assert np.abs(fr - fd).max() <= 1e-13 * np.abs(fr).max(), "step %d" % step
+        if step == 11:
+            with pytest.raises(gpu.LbmError):
+                dev.set_mask(None)                 # odd time level: the layout depends on the mask
+    mr, md = ref.get_macros(), dev.get_macros()
+    tol = 0.0 if exact else 1e-13
+    assert field_err(md["rho"].cpu().numpy(), mr["rho"]) <= tol
+    assert field_err(md["u"].cpu().numpy(), mr["u"]) <= tol
+    if mr["C"] is not None:                        # scalar / internal energy, eps_s on solid nodes that carry a lattice
+        assert field_err(md["C"].cpu().numpy(), mr["C"]) <= tol
+        if cfg["params"].get("tau_s", 0.0) > 0.0:
+            assert np.all(mr["C"][mask != 0] > 0.0)
+    solid = mask != 0
+    assert not md["rho"].cpu().numpy()[:, solid].any() and not md["u"].cpu().numpy()[:, solid].any()
+    Fr, Fd = ref.get_force(), dev.get_force().cpu().numpy()
+    assert np.abs(Fr - Fd).max() <= tol * max(np.abs(Fr).max(), 1e-300)
+    # clearing the mask returns to the plain kernels
+    dev.set_mask(None)
+    ref.set_mask(None)
+    ref.step(2)
+    dev.step(2)
+    if exact:
+        assert np.array_equal(ref.get_populations(), dev.get_populations().cpu().numpy())
+    with pytest.raises(gpu.LbmError):
+        dev.set_mask(mask)
+        dev.set_path("pipeline")                 # a masked context runs on the register path
+
+
+def test_masked_graph_replay_and_mass(gpu):
+    """Flow past an obstacle over 200 steps (CUDA-graph replay on a small grid, rebuilt after lbm_set_mask):
+    equals the oracle bit for bit; mass of the fluid nodes conserved."""
+    nx, ny = 24, 17
+    cfg = workloads.config("cfg1", grid=(nx, ny, 1), init_kind="REST", force=(1e-6, 0.0, 0.0))
+    ref, dev = make_pair(gpu, cfg)
+    m = np.zeros((ny, nx), np.uint8)
+    m[6:11, 8:13] = 1
+    ref.init_from_seed(0)
+    dev.init_from_seed(0)
+    dev.step(40)                              # builds the graph without a mask
+    ref.step(40)
+    ref.set_mask(m)
+    dev.set_mask(m)
+    ref.step(200)
+    dev.step(200)
+    fr, fd = ref.get_populations(), dev.get_populations().cpu().numpy()
+    assert np.array_equal(fr, fd)
+    fluid = np.tile(m.ravel() == 0, 9)
+    assert abs(fd[fluid].sum() - (m == 0).sum()) < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------------
+# the BASELINE.json configurations at their full sizes and step counts, checked by what the method fixes
+# (closed forms and invariants; DESIGN.md R15: field parity with the oracle is at 1000 steps, see above)
+# ------------------------------------------------------------------------------------------------------
+def test_cfg2_laplace_law_full_run(gpu):
+    """configs[1] as stated: 256x256, R in {20, 30, 40, 50}, 20000 steps each: the pressure jump of the relaxed
+    droplet, p = rho/3 + (G/6) psi^2, times the MEASURED radius is the same constant for every droplet
+    (Laplace law dp = gamma / R: PAPER.md:636-676); mass conserved to round-off."""
+    res = []
+    for R in (20.0, 30.0, 40.0, 50.0):
+        cfg = workloads.config("cfg2", radius=R)
+        dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+        dev.init_from_seed(2)
+        m0 = dev.get_macros(u=False, phi=False)["rho"].sum().item()
+        dev.step(20000)
+        mac = dev.get_macros(phi=False)
+        rho = mac["rho"][0].cpu().numpy().reshape(256, 256)
+        assert abs(rho.sum() / m0 - 1) < 1e-10
+        psi = 1 - np.exp(-rho)
+        p = rho / 3 + (-5.0 / 6) * psi ** 2
+        rin, rout = rho[128, 128], rho[0, 0]
+        assert rin > 1.8 and rout < 0.2
+        reff = np.sqrt(((rho - rout) / (rin - rout)).sum() / np.pi)
+        res.append((1 / reff, p[128, 128] - p[0, 0]))
+        assert mac["u"].abs().max().item() < 0.02
+    inv_r, dp = np.array(res).T
+    gamma = dp / inv_r
+    assert (dp > 0).all() and (np.diff(dp) < 0).all()
+    assert gamma[1:].max() / gamma[1:].min() - 1 < 0.03        # the three larger droplets
+    assert gamma.max() / gamma.min() - 1 < 0.10                # all four (the smallest shrinks to R_eff ~ 8)
+
+
+def test_cfg3_full_run_mass_and_demixing(gpu):
+    """configs[2] as stated: 512x512, 10000 steps of spinodal decomposition: per-component mass conserved to
+    round-off, the mixture has separated into A-rich and B-rich domains, everything finite."""
+    cfg = workloads.config("cfg3")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(3)
+    m0 = dev.get_macros(u=False, phi=False)["rho"].sum(1).cpu().numpy()
+    dev.step(10000)
+    mac = dev.get_macros()
+    m1 = mac["rho"].sum(1).cpu().numpy()
+    assert np.abs(m1 / m0 - 1).max() < 1e-10
+    phi = mac["phi"].cpu().numpy()
+    assert np.isfinite(phi).all() and bool(torch.isfinite(mac["u"]).all().item())
+    assert (phi > 0.5).mean() > 0.2 and (phi < -0.5).mean() > 0.2       # two phases, each a sizeable share of the box
+    assert abs(phi.mean()) < 0.05                                        # symmetric mixture
+
+
+def test_cfg5_full_run_invariants(gpu):
+    """configs[4] as stated: 512^3, fp32, 2000 steps: masses of A and B conserved (fp32 populations, fp64 sums),
+    total C decreasing and bounded below by C0 (1 - k)^t (the reaction factor 4 rhoA rhoB / rho^2 is <= 1), no NaN."""
+    cfg = workloads.config("cfg5")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(42)
+    m = dev.get_macros(u=False, phi=False)
+    m0 = m["rho"].double().sum(1).cpu().numpy()
+    c0 = m["C"].double().sum().item()
+    del m
+    dev.step(2000)
+    m = dev.get_macros(phi=False)
+    assert bool(torch.isfinite(m["u"]).all().item()) and bool(torch.isfinite(m["rho"]).all().item())
+    m1 = m["rho"].double().sum(1).cpu().numpy()
+    c1 = m["C"].double().sum().item()
+    assert np.abs(m1 / m0 - 1).max() <= 1e-3
+    assert c0 * (1 - 1e-3) ** 2000 * (1 - 1e-4) <= c1 < c0
+    del m, dev
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("LBM_LONG"), reason="9 min on a B200: set LBM_LONG=1")
+def test_cfg4_full_size_steady_state(gpu):
+    """configs[3] 'run to steady state' at the full 256^3 (700 000 steps, fp64): the Poiseuille profile with the
+    halfway-bounce-back slip term, u_x(z) = g/(2 nu) (z+1/2)(H-z-1/2) + g/(8 nu) (16 (tau-1/2)^2/3 - 1)."""
+    cfg = workloads.config("cfg4")
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    dev.init_from_seed(0)
+    for _ in range(70):
+        dev.step(10000)
+        dev.synchronize()
+    nz, tau, g = 256, 0.9, 1e-6
+    nu = (tau - 0.5) / 3
+    u = dev.get_macros(phi=False)["u"].reshape(3, nz, -1)
+    z = np.arange(nz)
+    exact = g / (2 * nu) * (z + 0.5) * (nz - z - 0.5) + g / (8 * nu) * (16 * (tau - 0.5) ** 2 / 3 - 1)
+    ux = u[0].cpu().numpy()
+    err = np.abs(ux - exact[:, None]).max() / exact.max()
+    print("cfg4 256^3 steady state: max |u_x - exact| / u_max = %.3e" % err)
+    assert err < 1e-5
+    assert u[1:].abs().max().item() < 1e-9 * exact.max()
