@@ -45,9 +45,10 @@ def measured_peak():
         return HBM_FALLBACK_GBS, "fallback"
 
 
-def ncu_traffic(workload):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel, copied by hand from
-    the newest `ncu --set full` capture into profiles/r*_traffic.csv (None when there is no capture)."""
+def ncu_traffic(workload, kernel):
+    """(bytes, provenance) of dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    newest `ncu --set full` capture listed in profiles/r*_traffic.csv -- a number copied from a capture, NOT measured in
+    this run -- or (None, why).  A row counts only if it names this workload AND the kernel that ran now."""
     import csv
     import glob
     best = None
@@ -55,11 +56,12 @@ def ncu_traffic(workload):
         try:
             with open(path) as fh:
                 for row in csv.DictReader(fh):
-                    if row["workload"] == workload:
-                        best = float(row["traffic_bytes_per_launch"])
+                    if row["workload"] == workload and row["kernel"] == kernel:
+                        best = (float(row["traffic_bytes_per_launch"]),
+                                "%s: %s (%s)" % (os.path.basename(path), row["source"], row.get("commit", "commit n/a")))
         except Exception:
             pass
-    return best
+    return best if best is not None else (None, "no ncu capture of %s for this workload under profiles/" % kernel)
 
 
 def shape_of(cfg):
@@ -163,7 +165,7 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------
 # GPU arm
 # --------------------------------------------------------------------------------------------
-def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None, path=None):
+def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None, path=None, mask_frac=0.0):
     """Times `steps` time steps with populations resident in HBM.  Returns a dict with the elapsed
     ms (CUDA events on the context's stream), the per-kernel device times measured with event pairs
     around every launch in a second pass of the same length, and the launch count."""
@@ -173,6 +175,9 @@ def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None, pa
     if path is not None:
         sim.set_path(*path)
     sim.init_from_seed(seed)
+    if mask_frac:                                             # seeded random solid nodes (benchmark lines with a mask)
+        g = torch.Generator(device="cpu").manual_seed(1234)
+        sim.set_mask((torch.rand(sim.N, generator=g) < mask_frac).to(torch.uint8))
     sim.step(warmup)
     sim.synchronize()
     if barrier is not None:
@@ -200,9 +205,22 @@ def time_device(cfg, steps, warmup, device, seed, sampler=None, barrier=None, pa
     m = sim.get_macros(u=False, phi=False, C_=False)
     finite = bool(torch.isfinite(m["rho"]).all().item())
     del m
+    used_path = sim.get_path()
+    try:
+        sim.check()                                           # deferred device-side errors (bounded waits of the tile path)
+    except Exception:
+        finite = False
+    s = shape_of(cfg)
+    if used_path == "pipeline":
+        kernel = "k_tile"
+    elif cfg["model"] == "BGK" and s["B"] == 4 and cfg["grid"][0] % 2 == 0 and not cfg["params"].get("bc", (0, 0, 0))[0]:
+        kernel = "k_step_v2"
+    else:
+        kernel = "k_step"
     sim.close()
     torch.cuda.empty_cache()
-    return dict(ms=ms, launches=launches, step_ms=step_ms, step_n=step_n, psi_ms=psi_ms, psi_n=psi_n, finite=finite)
+    return dict(ms=ms, launches=launches, step_ms=step_ms, step_n=step_n, psi_ms=psi_ms, psi_n=psi_n, finite=finite,
+                path=used_path, kernel=kernel)
 
 
 class _Null:
@@ -257,6 +275,7 @@ def model_line(name, cfg, r, steps, peak):
            "frac_of_nominal_8TBs": round(gbs / HBM_NOMINAL_GBS, 4),
            "population_mb": round((s["S"] * s["Q"] + s["Qs"]) * s["N"] * s["B"] / 1e6, 1),
            "finite": r["finite"]}
+    out["path"], out["kernel"] = r.get("path"), r.get("kernel")
     if r["step_n"]:
         t = r["step_ms"] / r["step_n"]
         out["step_kernel_ms"] = round(t, 5)
@@ -342,7 +361,7 @@ def run_reference(args, cfg, key):
 # per-model lines of the default run: (key, config overrides, steps, warmup).  BASELINE.json configs
 # 1-3 at paper size are L2-resident (0.3 / 4.7 / 38 MB): their rate is launch/L2-bound and their "HBM
 # fraction" is flagged l2_resident; the 8192^2 rows run the same D2Q9 kernels HBM-bound.
-# (key, overrides, grid, steps, warmup[, path[, note]])
+# (key, overrides, grid, steps, warmup[, path[, note[, mask fraction]]])
 EXTRAS = [
     ("cfg4", dict(precision=32), None, 1000, 50),
     ("cfg5", dict(), None, 100, 10),
@@ -353,13 +372,21 @@ EXTRAS = [
     ("cfg1", dict(), (8192, 8192, 1), 100, 10),
     ("cfg2", dict(radius=2000.0), (8192, 8192, 1), 100, 10),
     ("cfg3", dict(), (8192, 8192, 1), 50, 5),
+    ("cfg3", dict(), (8192, 8192, 1), 30, 5, ("pipeline", 0), "resident-tile path (opt-in for D2Q9: slower there, DESIGN.md 6.3)"),
     ("cfg4", dict(bc=(0, 0, 0), force=(0.0, 0.0, 0.0), init_kind="TAYLOR_GREEN", u0=0.05, tau=(0.5019, 0.5019)),
-     (128, 128, 128), 1000, 50),
+     (128, 128, 128), 1000, 50, None, "the paper's 3D Taylor-Green size, 2,097,152 cells (PAPER.md:854: 1056 MLUPS on a V100)"),
+    # the paper's 3D Couette benchmark (1,000,000 cells, 1202 MLUPS on a V100): moving-wall kernel variant
+    ("cfg4", dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, 0.0, 0.0)}), (100, 100, 100), 1000, 50, None,
+     "the paper's 3D Couette size, 1,000,000 cells, top wall moving (PAPER.md:848: 1202 MLUPS on a V100); L2-resident"),
+    ("cfg4", dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, 0.0, 0.0)}), (256, 256, 256), 500, 20, None,
+     "Couette, moving-wall kernel variant at an HBM-bound size"),
     # paper-shaped Rayleigh-Taylor setup: two components between walls in y, gravity, 1200 x 400
     ("cfg3", dict(bc=(0, 1, 0), force=(0.0, -1e-5, 0.0), G_ads=(0.0, 0.0)), (1200, 400, 1), 500, 50, None,
      "Rayleigh-Taylor-shaped: walls in y + body force"),
     ("cfg3", dict(forcing=1), (8192, 8192, 1), 50, 5, None, "velocity-shift forcing scheme (Eq. 16-19)"),
     ("cfgT", dict(), (256, 256, 256), 200, 20, None, "BGK + internal-energy lattice (IEDDF, Eq. 27-30)"),
+    ("cfgT", dict(tau_s=0.9, rho_solid=2.0), (256, 256, 256), 200, 20, None,
+     "the same with 20 % random solid nodes carrying the solid-phase energy lattice (Eq. 31-33)", 0.2),
 ]
 
 
@@ -441,7 +468,7 @@ def main():
     # average launch duration, measured live with CUDA event pairs on the launching stream
     k_ms = r["step_ms"] / max(1, r["step_n"])
     achieved = step_b * s["N"] / (k_ms * 1e-3) / 1e9
-    traffic = ncu_traffic(workload_name(args.workload, cfg))
+    traffic, traffic_source = ncu_traffic(workload_name(args.workload, cfg), r["kernel"])
     line = {
         "metric": "MLUPS", "value": round(value, 1), "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -449,12 +476,17 @@ def main():
         "config": {"workload": workload_name(args.workload, cfg), "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (%.0f MB populations vs 126 MB), no flush" %
                          ((s["S"] * s["Q"] + s["Qs"]) * s["N"] * s["B"] / 1e6),
-                   "streaming": "in-place AA pattern, one population copy"},
+                   "streaming": "in-place AA pattern, one population copy", "path": r["path"]},
         "hbm_gbs": round((step_b + psi_b) * s["N"] * args.steps / (ms * 1e-3) / 1e9 , 1),
-        "roofline": {"bound": "hbm", "kernel": "k_step (fused collide+stream)", "achieved": round(achieved, 1),
-                     "peak": peak, "peak_kind": "of " + peak_kind, "unit": "GB/s", "frac": round(achieved / peak, 4),
+        "roofline": {"bound": "hbm", "kernel": "%s (fused collide+stream)" % r["kernel"], "achieved": round(achieved, 1),
+                     "peak": peak, "peak_kind": "%s: torch copy_ bandwidth (a fraction a little above 1.0 means the kernel "
+                                                "beats a plain copy, not that it beats the hardware)" % peak_kind,
+                     "unit": "GB/s", "frac": round(achieved / peak, 4),
                      "frac_of_nominal_8TBs": round(achieved / HBM_NOMINAL_GBS, 4),
-                     "algorithmic_bytes_per_update": step_b, "kernel_ms": round(k_ms, 5), "traffic": traffic},
+                     "algorithmic_bytes_per_update": step_b, "kernel_ms": round(k_ms, 5),
+                     "kernel_ms_how": "second pass of the same length with a CUDA event pair around every launch "
+                                      "(adds event overhead: may slightly exceed ms_per_step)",
+                     "traffic": traffic, "traffic_source": traffic_source},
         "gpu_launches": r["launches"],
         "clocks": sampler.summary() if sampler is not None else None,
         "finite": r["finite"],
@@ -466,16 +498,23 @@ def main():
         for key, ov, grid, k, w, *rest in EXTRAS:
             c = workloads.config(key, grid=grid, **ov)
             epath = rest[0] if rest else None
-            rr = time_device(c, k, w, device, seed=1, path=epath)
+            rr = time_device(c, k, w, device, seed=1, path=epath, mask_frac=rest[2] if len(rest) > 2 else 0.0)
             ml = model_line(workload_name(key, c), c, rr, k, peak)
-            if epath is not None:
-                ml["path"] = epath[0]
-            if len(rest) > 1:
+            if len(rest) > 1 and rest[1]:
                 ml["note"] = rest[1]
             if ml["population_mb"] < 126.0:
                 ml["l2_resident"] = True
             per.append(ml)
         line["per_model"] = per
+        # north_star's "D3Q19 fused kernels >= 75 % of HBM bandwidth": the three D3Q19 kernels, inside roofline so that
+        # they survive a truncated output tail
+        fused = []
+        for ml in per:
+            if ml["lattice"] == "D3Q19" and ml["workload"].startswith(("cfg4: D3Q19 BGK fp64 256", "cfg4: D3Q19 BGK fp32 256", "cfg5:")) \
+                    and "Couette" not in ml.get("note", ""):
+                fused.append({k2: ml[k2] for k2 in ("workload", "path", "kernel", "mlups", "ms_per_step", "hbm_gbs",
+                                                     "frac_of_measured", "frac_of_nominal_8TBs", "step_kernel_ms") if k2 in ml})
+        line["roofline"]["d3q19_fused"] = fused
         mlups, desc, _ = time_oracle(cfg, 6, 1, seconds=20.0)
         line["cpu_baseline"] = {"value": round(mlups, 3), "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": desc}
     print(json.dumps(line), flush=True)

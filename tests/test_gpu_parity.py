@@ -647,6 +647,10 @@ def test_cfg3_full_run_mass_and_demixing(gpu):
     assert abs(phi.mean()) < 0.05                                        # symmetric mixture
 
 
+# measured on the B200 (this test prints it): see DESIGN.md R13
+DRIFT_BOUND_CFG5 = 1e-4     # measured 3.3e-5 (A), 3.1e-5 (B) relative drift after 2000 fp32 steps: 3 x that = SURVEY 8(c)'s 1e-4
+
+
 def test_cfg5_full_run_invariants(gpu):
     """configs[4] as stated: 512^3, fp32, 2000 steps: masses of A and B conserved (fp32 populations, fp64 sums),
     total C decreasing and bounded below by C0 (1 - k)^t (the reaction factor 4 rhoA rhoB / rho^2 is <= 1), no NaN."""
@@ -662,10 +666,60 @@ def test_cfg5_full_run_invariants(gpu):
     assert bool(torch.isfinite(m["u"]).all().item()) and bool(torch.isfinite(m["rho"]).all().item())
     m1 = m["rho"].double().sum(1).cpu().numpy()
     c1 = m["C"].double().sum().item()
-    assert np.abs(m1 / m0 - 1).max() <= 1e-3
+    drift = np.abs(m1 / m0 - 1).max()
+    print("cfg5 512^3 fp32, 2000 steps: relative mass drift per component", (m1 / m0 - 1).tolist())
+    assert drift <= DRIFT_BOUND_CFG5
     assert c0 * (1 - 1e-3) ** 2000 * (1 - 1e-4) <= c1 < c0
     del m, dev
     torch.cuda.empty_cache()
+
+
+def test_contact_angle_versus_adhesion(gpu):
+    """Wettability: a half droplet of component 1 on the wall y = -1/2 in component 2, D2Q9 two
+    components with psi = rho, cohesion G_c, adhesion G_ads,1 = -G_ads,2 (Eq. 14).  The contact angle is measured as the
+    paper does, from the height h and the contact length b of the region where component 1 dominates (Eq. 49-50), for
+    dG = G_ads,2 - G_ads,1 in {-0.4, -0.2, 0, 0.2, 0.4}.  What the method fixes and this test asserts: a neutral wall gives
+    90 degrees; cos(theta) is odd and LINEAR in dG (Eq. 48: cos(theta) = dG / (G_c (rho_1 - rho_2) / 2)).  The measured
+    slope is 1.9 times the slope Eq. 48 prints (R26 records the discrepancy and bounds it here)."""
+    nx, ny, Gc, rho_m, rho_d, R0 = 200, 100, 1.5, 2.0, 0.06, 30.0
+    c, w, _ = gpu.lbm.lattice_table("D2Q9")
+    y, x = np.mgrid[0:ny, 0:nx]
+    d = np.sqrt((x - (nx - 1) / 2) ** 2 + (y + 0.5) ** 2)          # centre on the wall
+    ind = 0.5 * (1 - np.tanh(2 * (d - R0) / 4.0))
+    rA, rB = rho_d + (rho_m - rho_d) * ind, rho_m - (rho_m - rho_d) * ind
+    f0 = np.concatenate([(w[:, None] * rA.ravel()[None, :]).ravel(), (w[:, None] * rB.ravel()[None, :]).ravel()])
+
+    def cos_theta(dG):
+        sim = gpu.LBM(nx, ny, 1, "D2Q9", "SC2", precision=64, tau=(1.0, 1.0), psi_kind=1, G=((0.0, Gc), (Gc, 0.0)),
+                      bc=(0, 1, 0), G_ads=(-dG / 2.0, dG / 2.0))
+        sim.set_populations(torch.from_numpy(f0))
+        sim.step(16000)
+        rho = sim.get_macros(u=False, phi=False)["rho"].cpu().numpy().reshape(2, ny, nx)
+        sim.close()
+        phi = rho[0] - rho[1]
+        col = phi[:, nx // 2]
+        j = np.where(col > 0)[0].max()
+        h = (j + 0.5) + col[j] / (col[j] - col[j + 1])               # height above the wall (cell centres at y = j)
+        row = 1.5 * phi[0] - 0.5 * phi[1]                              # phi extrapolated to the wall
+        k = np.where(row > 0)[0]
+        b = (k.max() + row[k.max()] / (row[k.max()] - row[k.max() + 1])) - (k.min() - row[k.min()] / (row[k.min()] - row[k.min() - 1]))
+        r = (4 * h * h + b * b) / (8 * h)                              # Eq. 49
+        theta = np.pi - np.arctan(b / (2 * (h - r))) if h > r else np.arctan(b / (2 * (r - h)))     # Eq. 50 and its lower branch
+        inside = rho[0] > rho[1]
+        return np.cos(theta), rho[0][inside].max(), rho[0][ny - 5, 5]
+
+    res = {dG: cos_theta(dG) for dG in (-0.4, -0.2, 0.0, 0.2, 0.4)}
+    cs = {k: v[0] for k, v in res.items()}
+    print("contact angle: cos(theta) by dG", cs)
+    assert abs(cs[0.0]) < 0.05                                         # neutral wall: 90 degrees
+    assert abs(cs[0.2] + cs[-0.2]) < 0.06 and abs(cs[0.4] + cs[-0.4]) < 0.06          # odd in dG
+    assert cs[-0.4] < cs[-0.2] < cs[0.0] < cs[0.2] < cs[0.4]           # G_ads,1 < 0: component 1 wets the wall more
+    assert abs(cs[0.4] / cs[0.2] - 2.0) < 0.15 and abs(cs[-0.4] / cs[-0.2] - 2.0) < 0.15   # linear
+    slope = (cs[0.4] - cs[-0.4]) / 0.8
+    rho1, rho2 = res[0.0][1], res[0.0][2]
+    slope48 = 1.0 / (Gc * (rho1 - rho2) / 2.0)                         # Eq. 48
+    print("slope %.3f, Eq. 48 slope %.3f, ratio %.2f" % (slope, slope48, slope / slope48))
+    assert 1.6 < slope / slope48 < 2.2
 
 
 @pytest.mark.skipif(not __import__("os").environ.get("LBM_LONG"), reason="9 min on a B200: set LBM_LONG=1")
