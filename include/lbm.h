@@ -161,19 +161,21 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *   LBM_PATH_REGISTER   one thread per cell (two in fp32 BGK), populations loaded straight into registers: one launch
  *                       of the fused step kernel per time step, preceded by the psi pass for Shan-Chen models
  *                       (which reads the flow populations a second time).  Works for every shape and boundary.
- *   LBM_PATH_PIPELINE   Shan-Chen models: ONE persistent, warp-specialised launch per time step (tile.cuh).  A block
- *                       copies the populations of a 128-cell row segment and the psi rows around it into shared
- *                       memory (cp.async + mbarrier, a ring of stages) and collides and streams it (a1, a3-a8) from
- *                       there, two fp32 cells per thread in packed arithmetic; psi of the NEXT time level (step a2;
- *                       Eq. 11 / 13 need psi of all neighbours at one time level: PAPER.md:128, 136; R9) is formed by
- *                       trailing psi warps of the same launch as soon as the step of the tiles around a tile is
- *                       complete, from populations still in L2, into a second psi buffer (allocated by the library,
- *                       S * N values): every population crosses HBM once per step in each direction.  Needs
- *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing and no solid-node mask (LBM_EINVAL
- *                       otherwise); walls in y / z are handled.
- * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a Shan-Chen
- * context with more than 2^21 cells to LBM_PATH_PIPELINE where it applies (smaller grids replay a CUDA graph of
- * the register kernels).  lbm_set_mask falls back to LBM_PATH_REGISTER.
+ *   LBM_PATH_PIPELINE   Shan-Chen models: ONE persistent, warp-specialised launch per time step (tile.cuh), one
+ *                       block per SM.  Producer warps bulk-copy (cp.async.bulk + mbarrier, TMA unit) the populations
+ *                       of a tile of 1 KB rows and the psi rows around it into a ring of shared-memory stages; two
+ *                       teams of step warps collide and stream it (a1, a3-a8) from there, two fp32 cells per thread
+ *                       in packed arithmetic; psi of the NEXT time level (step a2; Eq. 11 / 13 need psi of all
+ *                       neighbours at one time level: PAPER.md:128, 136; R9) is formed by PSI tickets of the same
+ *                       launch once the step of the tiles around a tile is complete, from populations still in L2,
+ *                       into a second psi buffer (allocated by the library, S * N values): every population crosses
+ *                       HBM once per step in each direction (ncu: 1.015 x the algorithmic bytes on config 5).  Needs
+ *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing, no solid-node mask (LBM_EINVAL
+ *                       otherwise) and the GPU to itself (all blocks co-resident); walls in y / z are handled.
+ * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a
+ * two-component D3Q19 fp32 context with more than 2^21 cells to LBM_PATH_PIPELINE where it applies -- the one case
+ * in which it is the faster path; smaller grids replay a CUDA graph of the register kernels.
+ * lbm_set_mask falls back to LBM_PATH_REGISTER.
  * rows_per_pencil: rows of the slower-but-one axis that are marched together along the slowest axis (<= 0:
  * default).  Synchronises the stream. */
 enum { LBM_PATH_REGISTER = 0, LBM_PATH_PIPELINE = 1 };

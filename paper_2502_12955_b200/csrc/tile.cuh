@@ -4,27 +4,30 @@
 // The problem: Eq. 11 / 13 need psi(x + c_i, t) of all neighbours before cell x
 // is collided (R9), and rho(x, t + 1) = sum_i f*_i(x - c_i, t) (Eq. 5 / 7) needs the step of all neighbours.  Two
 // launches per time step (k_psi, k_step) read the flow populations twice from HBM.  Here the psi pass of time level
-// t + 1 TRAILS the step of time level t inside the same launch, a few rows behind it, so that it reads the
-// populations the step has just written while they are still in L2 (126 MB):
+// t + 1 TRAILS the step of time level t inside the same launch, so that it reads the populations the step has just
+// written while they are still in L2 (126 MB).  One block per SM works through the tickets b, b + B, ... of a
+// host-built list (tile_schedule.h) of STEP and PSI tickets, one ticket = one tile of 1 KB rows (256 fp32 / 128 fp64
+// cells of an x-row):
 //
-//   producer warp   copies (16-byte cp.async, LDGSTS.128) the S*Q + Q_s slot rows P_i(x) of a 128-cell tile and the
-//                   psi(t) rows around it (3 x 3 rows per component, with a one-cell halo in x) into the next free
-//                   stage of a ring of NS shared-memory stages; at odd parity a population row comes from the
-//                   neighbour row (y - c_y, z - c_z) and is shifted by -c_x, so it is the aligned segment plus the
-//                   16-byte piece left or right of it.  No registers, no per-cell instructions.
-//   step warps      steps a1, a3-a8 from the stage: moments, psi stencil, force, collide, store to the global slots
-//                   the rows came from; in fp32 every thread owns TWO cells and runs the packed f32x2 instantiation
-//                   (V = F2) of the cell arithmetic.  They never wait for another block.
-//   publisher warp  once all step warps have stored a tile: fence, then the tile's flag (launch epoch) in global memory.
-//   psi warps       step a2 for t + 1: wait (acquire) for the flags of the up to 27 tiles around a tile, then rho^sigma
-//                   in index order (Eq. 7 / 18) from the slots of the NEXT parity (ld.global.cg: L2, never a stale L1
-//                   line) and psi^sigma (Eq. 10 / 24 or psi = rho) to the second psi buffer, which the next launch reads.
+//   producer warps  (4) For a STEP ticket: the S*Q + Q_s slot rows P_i(x) of the tile and the psi(t) rows around it (3 x 3
+//                   rows per component) into the next free stage of a ring of shared-memory stages -- one
+//                   cp.async.bulk (TMA unit, UBLKCP; completion as transaction bytes on an mbarrier) per row, issued by
+//                   the lane that owns the row; at odd parity a population row comes from the neighbour row
+//                   (y - c_y, z - c_z) and is shifted by -c_x: the aligned segment plus the 16-byte piece left or right
+//                   of it (16-byte cp.async; also the one-cell halo of the psi rows).  For a PSI ticket: first the flags
+//                   of the up to 27 tiles around the tile (acquire), then the S*Q flow rows at the NEXT parity.
+//   step warps      (two teams of TX / cells-per-thread threads, alternating tickets) STEP ticket: steps a1, a3-a8 from
+//                   the stage -- moments, psi stencil, force, collide, store to the global slots the rows came from; in
+//                   fp32 every thread owns TWO cells and runs the packed f32x2 instantiation (V = F2) of the cell
+//                   arithmetic.  PSI ticket: step a2 for t + 1 -- rho^sigma in index order (Eq. 7 / 18), psi^sigma (Eq. 10
+//                   / 24 or psi = rho) to the second psi buffer, which the next launch reads.
+//   publisher warp  once all warps of a team have stored a STEP tile: one gpu-scope fence, then the tile's flag (launch
+//                   epoch) in global memory.
 //
-// Work distribution is static: block b owns the STEP tickets b, b + B, ... and psi worker w the PSI tickets w, w + W,
-// ... of the host-built lists (tile_schedule.h; one ticket = one tile).  Deadlock freedom: producer, step warps and
-// publisher wait only inside their block (free stage, landed copy, stored tile); only the psi warps wait for other
-// blocks, and nothing waits for a psi warp.  The host launches at most as many blocks as are co-resident.  Every
-// wait is bounded (clock64); a timeout sets *status and gives up instead of hanging the GPU.
+// Deadlock freedom: a ticket depends only on STEP tickets EARLIER in the list (a PSI ticket on the steps of the tiles
+// around its tile; a STEP ticket on nothing), every block takes its tickets in list order, and the host launches at
+// most as many blocks as are co-resident: the earliest unfinished ticket of the list can always proceed.  Every wait
+// is bounded (clock64); a timeout sets bits in *status and gives up instead of hanging the GPU.
 //
 // Requirements (else the two-launch path runs): periodic x, nx * sizeof(R) a multiple of 16 bytes, no solid mask,
 // Guo forcing.  Walls in y / z are uniform per row and handled here: rows beyond a wall are redirected to the
