@@ -24,7 +24,7 @@ namespace {
 #endif
 // rounds of the round-robin between a STEP ticket and the PSI tickets that depend on it (tile_schedule.h)
 #ifndef LBM_TILE_DELAY
-#define LBM_TILE_DELAY 3
+#define LBM_TILE_DELAY 6
 #endif
 
 thread_local std::string g_err;
@@ -317,7 +317,7 @@ int path_setup(lbm_ctx* c, int py) {
     if (py > nm) py = nm;
     const size_t n_tiles = (size_t)nm * ns * nxs;
     if ((double)n_tiles > 1.0e9) return fail(LBM_EINVAL, "resident-tile path: more than 1e9 tiles");
-    const int blocks = (long long)resident < (long long)(2 * n_tiles) ? resident : (int)(2 * n_tiles);
+    const int blocks = (long long)resident < (long long)n_tiles ? resident : (int)n_tiles;
     // a PSI ticket comes LBM_TILE_DELAY rounds of the round-robin after the last STEP ticket it depends on
     int delay_tiles = LBM_TILE_DELAY * blocks;
 #ifdef LBM_TUNING
@@ -325,16 +325,32 @@ int path_setup(lbm_ctx* c, int py) {
 #endif
     const int delay_rows = (delay_tiles + nxs - 1) / nxs;
     const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, delay_rows, nullptr);
-    std::vector<lbm::TileItem> items;
-    items.reserve(2 * n_tiles);
+    // One ticket = the next tile to step and the next tile whose psi(t + 1) is due (a PSI row becomes due where the
+    // schedule lists it: every step it depends on is an EARLIER ticket); the PSI tiles left over after the last step
+    // form the tail.  A PSI part is never paired with a step listed before it is due.
+    struct Pos { int xs, y, z; size_t due; };
+    std::vector<Pos> steps, psis;
+    steps.reserve(n_tiles); psis.reserve(n_tiles);
     for (const lbm::TileRow& r : rows) {
-        lbm::TileItem it;
-        it.y = sh.d == 3 ? r.m : r.s;
-        it.z = sh.d == 3 ? r.s : 0;
-        it.kind = r.kind;
-        for (int xs = 0; xs < nxs; ++xs) { it.xs = xs; items.push_back(it); }
+        Pos q;
+        q.y = sh.d == 3 ? r.m : r.s;
+        q.z = sh.d == 3 ? r.s : 0;
+        q.due = steps.size();                 // PSI: may ride on the step ticket with this index or a later one
+        for (int xs = 0; xs < nxs; ++xs) { q.xs = xs; (r.kind == lbm::TILE_STEP ? steps : psis).push_back(q); }
     }
-    if (items.size() != 2 * n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
+    if (steps.size() != n_tiles || psis.size() != n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
+    std::vector<lbm::TileItem> items;
+    items.reserve(n_tiles + n_tiles / 8);
+    size_t jp = 0;
+    for (size_t k = 0; k < n_tiles || jp < n_tiles; ++k) {
+        lbm::TileItem it = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (k < n_tiles) { it.sx = steps[k].xs; it.sy = steps[k].y; it.sz = steps[k].z; it.sv = 1; }
+        if (jp < n_tiles && (psis[jp].due <= k || k >= n_tiles)) {
+            it.px = psis[jp].xs; it.py = psis[jp].y; it.pz = psis[jp].z; it.pv = 1;
+            ++jp;
+        }
+        items.push_back(it);
+    }
     c->tile_py = py;
     c->tile_blocks = blocks;
     c->tile_n_items = (long long)items.size();

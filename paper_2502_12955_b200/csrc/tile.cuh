@@ -39,16 +39,22 @@
 namespace lbm {
 
 constexpr int TILE_ROW_BYTES = 1024;  // bytes of one row segment of a tile: 256 fp32 / 128 fp64 cells (one bulk copy)
-constexpr int TILE_PROD_WARPS = 4;    // producer warps per block (each issues the bulk copies of a quarter of the rows)
+#ifndef LBM_TILE_PRODW
+#define LBM_TILE_PRODW 4
+#endif
+constexpr int TILE_PROD_WARPS = LBM_TILE_PRODW;    // producer warps per block (each issues the bulk copies of its share of the rows)
 
 struct TileItem {
-    int xs, y, z;                     // x-segment, row
-    int kind;                         // TILE_STEP / TILE_PSI (tile_schedule.h)
+    int sx, sy, sz, sv;               // STEP part: x-segment, row of the tile to step; sv != 0: present
+    int px, py, pz, pv;               // PSI part: the tile whose psi(t + 1) is formed; pv != 0: present
+};
+struct TilePos {
+    int xs, y, z;
 };
 
 struct TileArgs {
-    const TileItem* items;            // the tickets of one time step (device), STEP and PSI tickets in schedule order
-    unsigned n_items;                 // 2 * tiles
+    const TileItem* items;            // the tickets of one time step (device): a tile to step and / or a tile whose psi is due
+    unsigned n_items;                 // tickets (tiles + the tail of PSI-only tickets)
     int nxs;                          // tiles per row
     int* flags;                       // one per tile (z, y, xs): launch epoch of the last completed step
     int epoch;                        // > 0, differs from every earlier launch since the flags were cleared
@@ -214,15 +220,16 @@ struct TileCfg {
     static constexpr int TEAMS = HEAVY ? 1 : 2;
     static constexpr int AUX_WARPS = 1 + TILE_PROD_WARPS;                  // publisher, producers
     static constexpr int THREADS = 32 * AUX_WARPS + TEAMS * STEP_THREADS;
-    static constexpr size_t STAGE_BYTES = (size_t)NROWS * RS * B;
-    // one ring of NS stages for the STEP and the PSI tickets alike (two rings -- NS stages of each kind -- were measured
-    // and are slower: only two STEP stages fit beside two PSI stages)
-    static constexpr int NS = (215 * 1024) / STAGE_BYTES >= 6 ? 6 : (int)((215 * 1024) / STAGE_BYTES);   // stages
-    static constexpr size_t ROWPTR_BYTES = (size_t)NS * 64 * sizeof(unsigned long long);    // pointers of the (up to 64) rows of a stage
-    static constexpr size_t ROWSX_BYTES = ((size_t)NS * NPOPS * sizeof(int) + 15) / 16 * 16;
+    static constexpr int SROWS = NROWS + NF;                     // a stage: the STEP part's rows, then the flow rows of the PSI part
+    static constexpr size_t STAGE_BYTES = (size_t)SROWS * RS * B;
+    // a ring of NS stages; a ticket brings a tile to step AND a tile whose psi(t + 1) is due, so that the fixed costs of
+    // a stage (issue of the copies, HBM latency, hand-over) are paid once for both
+    static constexpr int NS = (215 * 1024) / STAGE_BYTES >= 4 ? 4 : (int)((215 * 1024) / STAGE_BYTES);   // stages
+    static constexpr size_t ROWPTR_BYTES = (size_t)NS * 128 * sizeof(unsigned long long);   // pointers of the (up to 128) rows of a stage
+    static constexpr size_t ROWSX_BYTES = (size_t)NS * 128 * sizeof(int);
     static constexpr int NBAR = 2 * NS;
     static constexpr size_t SMEM = NS * STAGE_BYTES + ROWPTR_BYTES + ROWSX_BYTES + NBAR * 8 + 32;
-    static_assert(NROWS <= 16 * TILE_PROD_WARPS, "one row per producer lane (16 lanes per warp issue)");
+    static_assert(SROWS <= 32 * TILE_PROD_WARPS, "one row per producer lane");
     static_assert(TEAMS * STEP_WARPS <= 8, "done counters");
     static_assert(NS >= 2 && SMEM <= 227 * 1024, "shared memory");
     __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return NPOPS + t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
@@ -235,13 +242,13 @@ struct Tile {
     using LS = typename C::LS;
     using V = typename C::V;
     static constexpr int S = C::S, Q = C::Q, D = C::D, B = C::B, H = C::H, RS = C::RS, NF = C::NF, NPOPS = C::NPOPS, CPT = C::CPT;
-    static constexpr int NROWS = C::NROWS, NS = C::NS, TILE_TX = C::TX;
+    static constexpr int NROWS = C::NROWS, SROWS = C::SROWS, NS = C::NS, TILE_TX = C::TX;
 
     const KP<R>& p;
     const TileArgs& w;
-    R* stages;                          // [NS][NROWS][RS]
-    unsigned long long* rowptr;         // [NS][64]: global address of element x = 0 of the row staged there (0: none)
-    int* rowsx;                         // [NS][NPOPS]: its x-shift (-1, 0, +1): cell x reads position H + (x - x0) + shift
+    R* stages;                          // [NS][SROWS][RS]
+    unsigned long long* rowptr;         // [NS][128]: global address of element x = 0 of the row staged there (0: none)
+    int* rowsx;                         // [NS][128]: its x-shift (-1, 0, +1): cell x reads position H + (x - x0) + shift
     unsigned long long *full, *empty;
     unsigned* done;                     // [TEAMS * STEP_WARPS]: tickets of its team that step warp k has stored
 
@@ -254,7 +261,7 @@ struct Tile {
         done = (unsigned*)(empty + NS);
     }
     __device__ __forceinline__ R* slot_base(int stage) const {
-        return stages + (size_t)stage * NROWS * RS;
+        return stages + (size_t)stage * SROWS * RS;
     }
     static __device__ __forceinline__ int wrap(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
     __device__ __forceinline__ bool wall_y() const { return WALLYZ && p.bc[1]; }
@@ -268,8 +275,8 @@ struct Tile {
         return WALLYZ && ((wall_y() && (y == 0 || y == p.ny - 1)) || (wall_z() && (z == 0 || z == p.nz - 1)));
     }
     static __device__ __forceinline__ TileItem item_of(const TileItem* items, unsigned ticket) {
-        const int4 v = __ldg((const int4*)(items + ticket));
-        return TileItem{v.x, v.y, v.z, v.w};
+        const int4 a = __ldg((const int4*)(items + ticket)), b = __ldg((const int4*)(items + ticket) + 1);
+        return TileItem{a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
     }
     __device__ __forceinline__ int* flag_of(int xs, int y, int z) const {
         const int nm = D == 3 ? p.ny : 1;
@@ -280,7 +287,7 @@ struct Tile {
     // ---------------- producer ----------------
     // The flag this lane looks at for a PSI ticket at (xs, y, z): lane l < 27 has one of the (up to) 27 tiles around it
     // (nullptr: no such tile beyond a wall, or lane >= 27)
-    __device__ __forceinline__ const int* flag_around(const TileItem& it) const {
+    __device__ __forceinline__ const int* flag_around(const TilePos& it) const {
         const int l = (int)(threadIdx.x & 31);
         const int nm = D == 3 ? p.ny : 1, ns = D == 3 ? p.nz : p.ny;
         const int m = D == 3 ? it.y : 0, s = D == 3 ? it.z : it.y;
@@ -348,15 +355,17 @@ struct Tile {
         }
         return d;
     }
-    // producer warp `pwid` looks after the rows r = pwid + TILE_PROD_WARPS * lane (lane < 16) of every stage
+    // producer warp `pwid` looks after the rows r = pwid + TILE_PROD_WARPS * lane of every stage: rows 0 .. NROWS-1 belong to
+    // the STEP part of a ticket, rows NROWS .. SROWS-1 to its PSI part
     __device__ __forceinline__ void produce(int pwid, unsigned n_mine, unsigned b0, unsigned stride) const {
         const int lane = (int)(threadIdx.x & 31);
-        const int r = lane < 16 ? pwid + TILE_PROD_WARPS * lane : NROWS;
-        const RowDesc d_step = row_desc(r, PARITY, false), d_psi = row_desc(r, 1 - PARITY, true);
+        const int r = pwid + TILE_PROD_WARPS * lane;           // (>= SROWS: no row)
+        const bool psi_row = r >= NROWS;
+        const RowDesc d = psi_row ? row_desc(r - NROWS, 1 - PARITY, true) : row_desc(r, PARITY, false);
         const unsigned long long pol = l2_evict_first();
-        // the ticket after the current one and (PSI tickets) the flag value are loaded one ticket ahead
-        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : TileItem{0, 0, 0, TILE_STEP};
-        const int* nfl = nxt.kind == TILE_PSI ? flag_around(nxt) : nullptr;
+        // the ticket after the current one and the flag value of its PSI part are loaded one ticket ahead
+        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : TileItem{0, 0, 0, 0, 0, 0, 0, 0};
+        const int* nfl = nxt.pv ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
         int nseen = nfl ? ld_relaxed(nfl) : 0;
         for (unsigned n = 0; n < n_mine; ++n) {
             const TileItem it = nxt;
@@ -364,49 +373,51 @@ struct Tile {
             const int seen = nseen;
             if (n + 1 < n_mine) {
                 nxt = item_of(w.items, b0 + (n + 1) * stride);
-                nfl = nxt.kind == TILE_PSI ? flag_around(nxt) : nullptr;
+                nfl = nxt.pv ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
                 nseen = nfl ? ld_relaxed(nfl) : 0;
             }
-            const bool ps = it.kind == TILE_PSI;
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
-            const RowDesc d{ps ? d_psi.nbr : d_step.nbr, ps ? d_psi.own : d_step.own, ps ? d_psi.dy : d_step.dy,
-                            ps ? d_psi.dz : d_step.dz, ps ? d_psi.sx : d_step.sx};
-            // a PSI ticket reads what the step of the tiles around it has written: listed well after them (tile_schedule.h),
-            // so this wait is a formality -- but it is what makes the read correct
-            if (ps && !wait_flags(fl, seen)) return;
+            // the PSI part reads what the step of the tiles around its tile has written: it is listed well after them
+            // (tile_schedule.h), so this wait is a formality -- but it is what makes the read correct
+            if (it.pv && !wait_flags(fl, seen)) return;
             if (!mbar_wait(&empty[stage], ph ^ 1u, w.status, 2)) return;
             if (pwid == 0) TILE_TRACE(7, n);
-            const int x0 = it.xs * TILE_TX;
+            const bool have = psi_row ? it.pv != 0 : it.sv != 0;
+            const int xs = psi_row ? it.px : it.sx, y = psi_row ? it.py : it.sy, z = psi_row ? it.pz : it.sz;
+            const int x0 = xs * TILE_TX;
             const int len = min(TILE_TX, p.nx - x0);
             const R* src = nullptr;
             int sx = 0;
-            if (r < NROWS) {
-                if (crosses(it.y, it.z, d.dy, d.dz)) {
-                    if (d.own) src = d.own + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx;
-                } else if (d.nbr) {
-                    const int yy = wrap(it.y + d.dy, p.ny), zz = D == 3 ? wrap(it.z + d.dz, p.nz) : 0;
-                    src = d.nbr + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
-                    sx = d.sx;
+            if (r < SROWS) {
+                if (have) {
+                    if (crosses(y, z, d.dy, d.dz)) {
+                        if (d.own) src = d.own + ((size_t)z * p.ny + y) * (size_t)p.nx;
+                    } else if (d.nbr) {
+                        const int yy = wrap(y + d.dy, p.ny), zz = D == 3 ? wrap(z + d.dz, p.nz) : 0;
+                        src = d.nbr + ((size_t)zz * p.ny + yy) * (size_t)p.nx;
+                        sx = d.sx;
+                    }
                 }
-                rowptr[stage * 64 + r] = (unsigned long long)src;
-                if (r < NPOPS) rowsx[stage * NPOPS + r] = sx;
+                rowptr[stage * 128 + r] = (unsigned long long)src;
+                rowsx[stage * 128 + r] = sx;
             }
             // One cp.async.bulk (TMA unit, UBLKCP: no load/store-unit slots) per row for the segment, issued by the lane
             // that owns the row; completion: transaction bytes on the stage's barrier.  The 16-byte pieces beside the
             // segment (periodic wrap in x) are 16-byte cp.async; the barrier also counts one arrival per lane for them.
-            const unsigned dst = smem_u32(slot_base(stage) + (size_t)(r < NROWS ? r : 0) * RS);
+            const bool halo_row = r >= NPOPS && r < NROWS;     // a psi(t) row of the STEP part: one-cell halo on both sides
+            const unsigned dst = smem_u32(slot_base(stage) + (size_t)(r < SROWS ? r : 0) * RS);
             const unsigned bytes = __reduce_add_sync(0xffffffffu, src ? (unsigned)(len * B) : 0u);
             if (lane == 0) mbar_arrive_expect_tx(&full[stage], bytes);
             __syncwarp();
             if (src) {
 #ifndef LBM_TILE_NOHINT
-                if (r < NPOPS) bulk_g2s_hint(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage], pol);
+                if (!halo_row) bulk_g2s_hint(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage], pol);
                 else
 #endif
                 bulk_g2s(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage]);
-                if (sx < 0 || r >= NPOPS) cp_async16(dst, src + (x0 == 0 ? p.nx - H : x0 - H));
-                if (sx > 0 || r >= NPOPS) cp_async16(dst + (unsigned)((H + len) * B), src + (x0 + len == p.nx ? 0 : x0 + len));
+                if (sx < 0 || halo_row) cp_async16(dst, src + (x0 == 0 ? p.nx - H : x0 - H));
+                if (sx > 0 || halo_row) cp_async16(dst + (unsigned)((H + len) * B), src + (x0 + len == p.nx ? 0 : x0 + len));
             }
             cp_async_arrive(&full[stage]);
             if (pwid == 0) TILE_TRACE(0, n);
@@ -424,7 +435,7 @@ struct Tile {
             else return *q;
         } else {
             int sh = -LL::c(I, 0);
-            if constexpr (EDGE) sh = rowsx[stage * NPOPS + R0 + I];
+            if constexpr (EDGE) sh = rowsx[stage * 128 + R0 + I];
             if constexpr (C::PACK) return pack2(q[sh], q[sh + 1]);
             else return q[sh];
         }
@@ -442,12 +453,12 @@ struct Tile {
     // col[0..3] = x - 1, x, x + 1, x + 2 with wrap (x + 1 only for the second cell of a packed pair)
     template <class LL, int R0, int I, bool EDGE>
     __device__ __forceinline__ void write_pop(int stage, const int* col, V val) const {
-        R* g0 = (R*)rowptr[stage * 64 + R0 + I];
+        R* g0 = (R*)rowptr[stage * 128 + R0 + I];
         if constexpr (PARITY == 0 || I == 0 || LL::c(I, 0) == 0) {
             st_global(g0 + col[1], val);
         } else {
             int sh = -LL::c(I, 0);
-            if constexpr (EDGE) sh = rowsx[stage * NPOPS + R0 + I];
+            if constexpr (EDGE) sh = rowsx[stage * 128 + R0 + I];
             if constexpr (C::PACK) {
                 if (EDGE && sh == 0) {
                     st_global(g0 + col[1], val);
@@ -481,7 +492,7 @@ struct Tile {
         }
     }
     template <bool EDGE>
-    __device__ __forceinline__ void step_cells(int stage, const TileItem& it, int t) const {
+    __device__ __forceinline__ void step_cells(int stage, const TilePos& it, int t) const {
         const int x = it.xs * TILE_TX + t;
         const R* sb = slot_base(stage) + H + t;
         // The populations are read from the stage twice -- for the moments here, for the collision below -- instead of
@@ -539,57 +550,57 @@ struct Tile {
             write_pops<LS, NF, EDGE>(stage, col, hl);
         }
     }
-    // step a2 for time level t + 1 (a PSI ticket): rho^sigma in index order (Eq. 7 / 18) from the flow populations the
-    // stage holds at the NEXT parity, psi^sigma (Eq. 10 / 24 or psi = rho) to the second psi buffer
+    // step a2 for time level t + 1 (the PSI part of a ticket): rho^sigma in index order (Eq. 7 / 18) from the flow
+    // populations the stage holds at the NEXT parity (rows NROWS ...), psi^sigma (Eq. 10 / 24 or psi = rho) to the second
+    // psi buffer
     template <bool EDGE>
-    __device__ __forceinline__ void psi_cells(int stage, const TileItem& it, int t) const {
+    __device__ __forceinline__ void psi_cells(int stage, const TilePos& it, int t) const {
         const R* sb = slot_base(stage) + H + t;
         R* out = (R*)w.psi_out + ((size_t)it.z * p.ny + it.y) * (size_t)p.nx + (it.xs * TILE_TX + t);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
             V fl[Q];
-            read_pops<L, s * Q, EDGE, 1 - PARITY>(sb, stage, fl);
+            read_pops<L, NROWS + s * Q, EDGE, 1 - PARITY>(sb, stage, fl);
             V rho = fl[0];
             static_for<1, Q>([&](auto ic) { rho = rho + fl[decltype(ic)::value]; });
             st_global(out + (size_t)s * (size_t)p.N, psi_of(rho, p.psi_kind, p.rho0_psi));
         });
     }
-    // team `team` takes the tickets n = team, team + TEAMS, ... of the block
+    // Every ticket is worked on by all teams at once: team n % TEAMS steps its STEP part, the next team forms the psi of
+    // its PSI part (with one team: both, one after the other)
     __device__ __forceinline__ void step_role(int team, unsigned n_mine, unsigned b0, unsigned stride) const {
         const int t = ((int)threadIdx.x - team * C::STEP_THREADS) * CPT;
         const int lane = (int)(threadIdx.x & 31), wid = (int)(threadIdx.x >> 5);
         unsigned cnt = 0;
-        TileItem nxt = (unsigned)team < n_mine ? item_of(w.items, b0 + (unsigned)team * stride) : TileItem{0, 0, 0, TILE_STEP};
+        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : TileItem{0, 0, 0, 0, 0, 0, 0, 0};
         for (unsigned n = 0; n < n_mine; ++n) {
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
-            // every team consumes every phase of every stage in order -- a parity wait must never be asked about a phase
-            // two ahead of the last one seen, so a stage is refilled only after ALL step warps have let go of it -- and
-            // works on its own tickets
+            const TileItem it = nxt;                       // (loaded one ticket ahead)
+            if (n + 1 < n_mine) nxt = item_of(w.items, b0 + (n + 1) * stride);
             if (!mbar_wait(&full[stage], ph, w.status, 1)) return;
-            if (n % C::TEAMS != (unsigned)team) {
-                if (lane == 0) mbar_arrive(&empty[stage]);
-                continue;
-            }
-            const TileItem it = nxt;                       // (loaded one own ticket ahead)
-            if (n + C::TEAMS < n_mine) nxt = item_of(w.items, b0 + (n + C::TEAMS) * stride);
-            const bool ps = it.kind == TILE_PSI;
+            const bool do_step = n % C::TEAMS == (unsigned)team;
+            const bool do_psi = C::TEAMS == 1 || (n + 1) % C::TEAMS == (unsigned)team;
             if (threadIdx.x == 0) TILE_TRACE(5, n);
-            const int len = min(TILE_TX, p.nx - it.xs * TILE_TX);
 #ifndef LBM_TILE_NOSTEP
-            if (t < len) {
-                const bool edge = edge_row(it.y, it.z);
-                if (ps) {
-                    if (edge) psi_cells<WALLYZ>(stage, it, t); else psi_cells<false>(stage, it, t);
-                } else {
-                    if (edge) step_cells<WALLYZ>(stage, it, t); else step_cells<false>(stage, it, t);
+            if (do_step && it.sv) {
+                const TilePos sp{it.sx, it.sy, it.sz};
+                if (t < min(TILE_TX, p.nx - sp.xs * TILE_TX)) {
+                    if (edge_row(sp.y, sp.z)) step_cells<WALLYZ>(stage, sp, t); else step_cells<false>(stage, sp, t);
+                }
+            }
+            if (do_psi && it.pv) {
+                const TilePos pp{it.px, it.py, it.pz};
+                if (t < min(TILE_TX, p.nx - pp.xs * TILE_TX)) {
+                    if (edge_row(pp.y, pp.z)) psi_cells<WALLYZ>(stage, pp, t); else psi_cells<false>(stage, pp, t);
                 }
             }
 #endif
             __syncwarp();
             if (threadIdx.x == 0) TILE_TRACE(6, n);
             if (lane == 0) {
-                st_release_cta_shared(&done[wid], ++cnt);      // after the stores of the whole warp (syncwarp above)
+                // (the counter the publisher reads: STEP parts of this team's tickets, after the stores of the whole warp)
+                if (do_step) st_release_cta_shared(&done[wid], ++cnt);
                 mbar_arrive(&empty[stage]);
             }
         }
@@ -618,7 +629,7 @@ struct Tile {
                     fence_acq_rel_gpu();
                     for (unsigned j = k[tm] + lane; j < m; j += 32) {
                         const TileItem it = item_of(w.items, b0 + (j * C::TEAMS + tm) * stride);
-                        if (it.kind == TILE_STEP) st_relaxed(flag_of(it.xs, it.y, it.z), w.epoch);
+                        if (it.sv) st_relaxed(flag_of(it.sx, it.sy, it.sz), w.epoch);
                     }
                     TILE_TRACE(2, (m - 1) * C::TEAMS + tm);
                     left -= m - k[tm];
