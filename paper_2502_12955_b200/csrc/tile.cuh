@@ -6,26 +6,26 @@
 // launches per time step (k_psi, k_step) read the flow populations twice from HBM.  Here the psi pass of time level
 // t + 1 TRAILS the step of time level t inside the same launch, so that it reads the populations the step has just
 // written while they are still in L2 (126 MB).  One block per SM works through the tickets b, b + B, ... of a
-// host-built list (tile_schedule.h) of STEP and PSI tickets, one ticket = one tile of 1 KB rows (256 fp32 / 128 fp64
-// cells of an x-row):
+// host-built list (tile_schedule.h, path_setup); a ticket names a tile to step (its STEP part) and a tile whose
+// psi(t + 1) is due (its PSI part), one tile = 1 KB rows (256 fp32 / 128 fp64 cells of an x-row):
 //
-//   producer warps  (4) For a STEP ticket: the S*Q + Q_s slot rows P_i(x) of the tile and the psi(t) rows around it (3 x 3
-//                   rows per component) into the next free stage of a ring of shared-memory stages -- one
+//   producer warps  (4) The rows of both parts into the next free stage of a ring of shared-memory stages -- one
 //                   cp.async.bulk (TMA unit, UBLKCP; completion as transaction bytes on an mbarrier) per row, issued by
-//                   the lane that owns the row; at odd parity a population row comes from the neighbour row
-//                   (y - c_y, z - c_z) and is shifted by -c_x: the aligned segment plus the 16-byte piece left or right
-//                   of it (16-byte cp.async; also the one-cell halo of the psi rows).  For a PSI ticket: first the flags
-//                   of the up to 27 tiles around the tile (acquire), then the S*Q flow rows at the NEXT parity.
-//   step warps      (two teams of TX / cells-per-thread threads, alternating tickets) STEP ticket: steps a1, a3-a8 from
-//                   the stage -- moments, psi stencil, force, collide, store to the global slots the rows came from; in
-//                   fp32 every thread owns TWO cells and runs the packed f32x2 instantiation (V = F2) of the cell
-//                   arithmetic.  PSI ticket: step a2 for t + 1 -- rho^sigma in index order (Eq. 7 / 18), psi^sigma (Eq. 10
-//                   / 24 or psi = rho) to the second psi buffer, which the next launch reads.
+//                   the lane that owns the row.  STEP part: the S*Q + Q_s slot rows P_i(x) of the tile and the psi(t)
+//                   rows around it (3 x 3 rows per component); at odd parity a population row comes from the neighbour
+//                   row (y - c_y, z - c_z) and is shifted by -c_x: the aligned segment plus the 16-byte piece left or
+//                   right of it (16-byte cp.async; also the one-cell halo of the psi rows).  PSI part: first the flags
+//                   of the up to 27 tiles around the tile (acquire), then its S*Q flow rows at the NEXT parity.
+//   step warps      (two teams of TX / cells-per-thread threads, both on every ticket, swapping parts) STEP part: steps
+//                   a1, a3-a8 from the stage -- moments, psi stencil, force, collide, store to the global slots the rows
+//                   came from; in fp32 every thread owns TWO cells and runs the packed f32x2 instantiation (V = F2) of
+//                   the cell arithmetic.  PSI part: step a2 for t + 1 -- rho^sigma in index order (Eq. 7 / 18), psi^sigma
+//                   (Eq. 10 / 24 or psi = rho) to the second psi buffer, which the next launch reads.
 //   publisher warp  once all warps of a team have stored a STEP tile: one gpu-scope fence, then the tile's flag (launch
 //                   epoch) in global memory.
 //
-// Deadlock freedom: a ticket depends only on STEP tickets EARLIER in the list (a PSI ticket on the steps of the tiles
-// around its tile; a STEP ticket on nothing), every block takes its tickets in list order, and the host launches at
+// Deadlock freedom: a ticket depends only on the STEP parts of EARLIER tickets (its PSI part on the steps of the tiles
+// around that tile; its STEP part on nothing), every block takes its tickets in list order, and the host launches at
 // most as many blocks as are co-resident: the earliest unfinished ticket of the list can always proceed.  Every wait
 // is bounded (clock64); a timeout sets bits in *status and gives up instead of hanging the GPU.
 //
