@@ -24,7 +24,7 @@ namespace {
 #endif
 // rounds of the round-robin between a STEP ticket and the PSI tickets that depend on it (tile_schedule.h)
 #ifndef LBM_TILE_DELAY
-#define LBM_TILE_DELAY 8
+#define LBM_TILE_DELAY 7
 #endif
 
 thread_local std::string g_err;
