@@ -336,6 +336,50 @@ def time_oracle(cfg, steps, warmup, seconds):
     return n * steps / dt / 1e6, desc, dt
 
 
+_ORACLE_WORKER = """
+import json, sys, time
+sys.path.insert(0, sys.argv[1])
+from oracle.ref_lbm import RefLBM
+a = json.loads(sys.argv[2])
+ref = RefLBM(*a["grid"], a["lattice"], a["model"], **a["params"])
+ref.init_from_seed(1)
+ref.step(1)
+t0 = time.perf_counter()
+ref.step(a["steps"])
+print(ref.N * a["steps"], time.perf_counter() - t0)
+"""
+
+
+def time_oracle_all_cores(cfg, steps, budget_cells, timeout=150.0):
+    """The oracle is single-threaded and stays so; this is the optional second figure of SURVEY 8(d): one independent
+    oracle instance per host core (separate processes, the same sample grid each, bounded by `timeout`), aggregate
+    MLUPS = all updates / the slowest instance's time.  Labelled as such; not a tuned program."""
+    import subprocess
+    cores = min(os.cpu_count() or 1, 32)                   # bounded: every instance holds two copies of its populations
+    over = dict(rmin=4.0, rmax=8.0, vol_frac=0.05) if cfg["params"].get("init_kind") == "RANDOM_DROPLETS" else {}
+    grid = oracle_sample_grid(cfg, budget_cells)
+    params = dict(cfg["params"], **over)
+    params = {k: (list(v) if isinstance(v, tuple) else v) for k, v in params.items() if k != "wall_u"}
+    arg = json.dumps(dict(grid=list(grid), lattice=cfg["lattice"], model=cfg["model"], params=params, steps=steps))
+    procs = [subprocess.Popen([sys.executable, "-c", _ORACLE_WORKER, ROOT, arg], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                              text=True) for _ in range(cores)]
+    updates, dt = 0, 0.0
+    t_end = time.time() + timeout
+    try:
+        for pr in procs:
+            out, _ = pr.communicate(timeout=max(1.0, t_end - time.time()))
+            u, d = out.split()
+            updates += int(u)
+            dt = max(dt, float(d))
+    finally:
+        for pr in procs:
+            if pr.poll() is None:
+                pr.kill()
+    desc = "%d independent single-thread oracle processes, each %s %s grid %dx%dx%d, %d steps" % (
+        cores, cfg["lattice"], cfg["model"], grid[0], grid[1], grid[2], steps)
+    return updates / dt / 1e6, cores, desc
+
+
 def workload_name(key, cfg):
     s = shape_of(cfg)
     return "%s: %s %s %s %dx%dx%d" % (key, cfg["lattice"], cfg["model"], "fp64" if s["B"] == 8 else "fp32",
@@ -517,6 +561,11 @@ def main():
         line["roofline"]["d3q19_fused"] = fused
         mlups, desc, _ = time_oracle(cfg, 6, 1, seconds=20.0)
         line["cpu_baseline"] = {"value": round(mlups, 3), "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": desc}
+        try:
+            am, cores, adesc = time_oracle_all_cores(cfg, 6, 1 << 19)
+            line["cpu_baseline"]["all_cores"] = {"value": round(am, 3), "unit": "MLUPS", "cores": cores, "sample": adesc}
+        except Exception as exc:                               # the single-thread figure above is the baseline
+            line["cpu_baseline"]["all_cores"] = {"unavailable": repr(exc)[:200]}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
