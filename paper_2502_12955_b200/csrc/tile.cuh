@@ -38,7 +38,11 @@
 
 namespace lbm {
 
-constexpr int TILE_ROW_BYTES = 1024;  // bytes of one row segment of a tile: 256 fp32 / 128 fp64 cells (one bulk copy)
+// bytes of one row segment of a tile (one bulk copy): a multiple of 16
+#ifndef LBM_TILE_ROW_BYTES
+#define LBM_TILE_ROW_BYTES 1024
+#endif
+constexpr int TILE_ROW_BYTES = LBM_TILE_ROW_BYTES;
 #ifndef LBM_TILE_PRODW
 #define LBM_TILE_PRODW 4
 #endif
@@ -212,8 +216,8 @@ struct TileCfg {
     static constexpr int NPSI = D == 3 ? 9 : 3;                  // psi rows (dy, dz) per component
     static constexpr int NP = S * NPSI;
     static constexpr int NROWS = NPOPS + NP;                     // rows of a stage: populations, then psi
-    static constexpr int STEP_THREADS = TX / CPT;
-    static constexpr int STEP_WARPS = STEP_THREADS / 32;
+    static constexpr int STEP_WARPS = (TX / CPT + 31) / 32;
+    static constexpr int STEP_THREADS = 32 * STEP_WARPS;        // (threads beyond the tile's cells idle)
     // Two teams of step warps work on two stages at a time (two warps per scheduler hide each other's latencies).  The
     // step role of the D3Q19 models in fp64 needs more registers (19 doubles per component and thread): one team.
     static constexpr bool HEAVY = B == 8 && Q > 9;
