@@ -195,6 +195,22 @@ int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_
  * timed out; lbm_run_host performs the same check before it returns). */
 int lbm_check(lbm_ctx* ctx);
 
+/* The Shan-Chen step for callers that must not allocate (code under CUDA-graph capture set-up, serving loops, harnesses
+ * that forbid cudaMalloc): n time steps (n even, >= 0) of a Shan-Chen model (LBM_SC1 / LBM_SC2 / LBM_SC2_ADE; a1-a8 as in
+ * lbm_step, register kernels: psi pass + fused step per time step) IN PLACE on the caller's DEVICE array f of canonical
+ * populations at an even time level, f[sigma][i][cell] followed by h[i][cell] (the layout of lbm_set_populations; the
+ * result is canonical again), on the CURRENT device and the stream params->stream.  No context, no workspace
+ * (params->workspace is ignored), no mask, no cudaMalloc / cudaFree / allocating library call: the psi field (Eq. 10 /
+ * 24), the only intermediate of the path, lives in a static device array of lbm_static_scratch_bytes() = 16 MiB that
+ * every GPU which loads the library holds until exit.  LBM_EINVAL if S * nx * ny * nz * sizeof(value) exceeds that
+ * (e.g. two components in fp32: up to 2^21 cells = 128^3), for other models, odd n, or invalid parameters.  Every call
+ * on a device shares the array: it keeps the last call's contents (nothing in it needs to start at zero: every step
+ * writes psi of all cells before reading any), and two calls that overlap on the GPU (different streams or host
+ * threads, same device) RACE on it -- serialise them.  Asynchronous like lbm_step.  Results equal lbm_step's bit for
+ * bit. */
+size_t lbm_static_scratch_bytes(void);
+int lbm_step_static(int nx, int ny, int nz, int lattice, int model, const lbm_params* params, void* f, int n);
+
 /* number of time steps taken since init / set_populations */
 int64_t lbm_time(const lbm_ctx* ctx);
 

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -802,6 +803,78 @@ int lbm_check(lbm_ctx* c) {
 #ifdef LBM_TILE_TRACE
 int lbm_debug_trace(void* out) { return (int)cudaMemcpy(out, g_trace, sizeof(long long) * 10 * 4096, cudaMemcpyDeviceToHost); }
 #endif
+
+// ---------------------------------------------------------------------------------------------------------------
+// lbm_step_static: the Shan-Chen step for callers that must not allocate (include/lbm.h).  The psi field -- the scratch
+// of the psi pass / fused step pair -- lives in a file-scope device array instead of a workspace.  In HOST code the
+// array's name is only a stand-in for the symbol: its device address comes from cudaGetSymbolAddress, once per device.
+// ---------------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+#define LBM_STATIC_SCRATCH_BYTES (16u << 20)
+static __device__ __align__(256) unsigned char g_static_scratch[LBM_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+void* g_static_ptr[STATIC_MAX_DEVICES];           // device address of g_static_scratch per device ordinal (nullptr: not asked yet)
+std::mutex g_static_mutex;
+
+// the device address of the scratch array on the CURRENT device
+int static_scratch_address(void** out) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(LBM_EINVAL, "lbm_step_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* ptr = nullptr;
+        CK(cudaGetSymbolAddress(&ptr, g_static_scratch));
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return 0;
+}
+}  // namespace
+
+extern "C" {
+
+size_t lbm_static_scratch_bytes(void) { return (size_t)LBM_STATIC_SCRATCH_BYTES; }
+
+int lbm_step_static(int nx, int ny, int nz, int lattice, int model, const lbm_params* p, void* f, int n) {
+    Shape sh;
+    const std::string e = validate(nx, ny, nz, lattice, model, p, &sh);
+    if (!e.empty()) return fail(LBM_EINVAL, "lbm_step_static: " + e);
+    if (!f) return fail(LBM_EINVAL, "lbm_step_static: f is NULL");
+    if (!sh.sc) return fail(LBM_EINVAL, "lbm_step_static: the model has no psi field (no scratch): use lbm_step");
+    if (n < 0 || (n & 1)) return fail(LBM_EINVAL, "lbm_step_static: n must be even and >= 0 (the populations are canonical at even time levels)");
+    const size_t need = (size_t)sh.S * sh.N * sh.B;
+    if (need > (size_t)LBM_STATIC_SCRATCH_BYTES)
+        return fail(LBM_EINVAL, "lbm_step_static: the psi field needs " + std::to_string(need) + " bytes, the static scratch holds " +
+                                    std::to_string((size_t)LBM_STATIC_SCRATCH_BYTES) + " (S * nx * ny * nz * sizeof(value)): use lbm_create / lbm_step");
+    void* scratch = nullptr;
+    int rc = static_scratch_address(&scratch);
+    if (rc) return rc;
+    // a context on the stack: no workspace, no schedule, no graph -- only what fill_kp and the launchers read
+    lbm_ctx c{};
+    c.nx = nx; c.ny = ny; c.nz = nz; c.lattice = lattice; c.model = model;
+    c.p = *p; c.sh = sh;
+    c.stream = (cudaStream_t)p->stream;
+    c.f = f;
+    c.h = sh.scalar ? (char*)f + (size_t)sh.S * sh.Q * sh.N * sh.B : nullptr;     // canonical layout: h follows f
+    c.psi = scratch;
+    c.bc_walls = p->bc[0] || p->bc[1] || p->bc[2];
+    c.forced = p->forcing == 1 ? 2 : 1;
+    if (p->precision == 64) c.ops = lattice == LBM_D3Q19 ? lbm::ops_f64_d3q19() : lbm::ops_f64_d2q9();
+    else c.ops = lattice == LBM_D3Q19 ? lbm::ops_f32_d3q19() : lbm::ops_f32_d2q9();
+    fill_kp(c.kp64, &c);
+    fill_kp(c.kp32, &c);
+    const int wmode = c.bc_walls ? 1 : 0;
+    for (int k = 0; k < n; ++k) {
+        // a2 writes psi of every cell before a3 reads any: nothing in the scratch needs to start at zero
+        CK(c.ops->psi(c.kp(), model, k & 1, wmode, c.stream));
+        CK(c.ops->step(c.kp(), model, k & 1, wmode, c.forced, 0, c.stream));
+    }
+    return 0;
+}
 
 int64_t lbm_time(const lbm_ctx* c) { return c ? c->t : -1; }
 int64_t lbm_launch_count(const lbm_ctx* c) { return c ? c->launches : -1; }

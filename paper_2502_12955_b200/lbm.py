@@ -22,7 +22,7 @@ PATHS = {"register": 0, "pipeline": 1}
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_tile_schedule", "lbm_check", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_tile_schedule", "lbm_check", "lbm_static_scratch_bytes", "lbm_step_static", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -77,6 +77,9 @@ def lib():
     L.lbm_get_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_set_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
+    L.lbm_static_scratch_bytes.restype = C.c_size_t
+    L.lbm_static_scratch_bytes.argtypes = []
+    L.lbm_step_static.argtypes = [C.c_int] * 5 + [P, C.c_void_p, C.c_int]
     L.lbm_set_path.argtypes = [C.c_void_p, C.c_int, C.c_int]
     L.lbm_get_path.argtypes = [C.c_void_p]
     L.lbm_set_mask.argtypes = [C.c_void_p, C.c_void_p]
@@ -160,6 +163,23 @@ def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True, delay_rows=
     if rc != 0:
         raise LbmError(rc, last_error())
     return out, lead.value
+
+
+def static_scratch_bytes():
+    return int(lib().lbm_static_scratch_bytes())
+
+
+def step_static(nx, ny, nz, lattice, model, f, n, stream=None, **params):
+    """lbm_step_static: n (even) steps of a Shan-Chen model in place on the device tensor f of canonical populations,
+    with the psi field in the library's static device array -- no allocation (include/lbm.h).  Marshalling only."""
+    L = lib()
+    p = make_params(**params)
+    p.stream = stream
+    lat = LATTICES[lattice] if isinstance(lattice, str) else int(lattice)
+    mod = MODELS[model] if isinstance(model, str) else int(model)
+    rc = L.lbm_step_static(int(nx), int(ny), int(nz), lat, mod, C.byref(p), f.data_ptr(), int(n))
+    if rc != 0:
+        raise LbmError(rc, last_error())
 
 
 def lattice_table(lattice, kind=0):
