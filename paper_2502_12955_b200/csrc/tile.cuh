@@ -9,9 +9,9 @@
 // host-built list (tile_schedule.h, path_setup); a ticket names a tile to step (its STEP part) and a tile whose
 // psi(t + 1) is due (its PSI part), one tile = 1 KB rows (256 fp32 / 128 fp64 cells of an x-row):
 //
-//   producer warps  (4) The rows of both parts into the next free stage of a ring of shared-memory stages -- one
-//                   cp.async.bulk (TMA unit, UBLKCP; completion as transaction bytes on an mbarrier) per row, issued by
-//                   the lane that owns the row.  STEP part: the S*Q + Q_s slot rows P_i(x) of the tile and the psi(t)
+//   producer warps  (4 for the STEP parts, 2 for the PSI parts, one 'landed' barrier per part and stage) The rows of a part
+//                   into the next free stage of a ring of shared-memory stages -- one cp.async.bulk (TMA unit, UBLKCP;
+//                   completion as transaction bytes on an mbarrier) per row, issued by the lane that owns the row.  STEP part: the S*Q + Q_s slot rows P_i(x) of the tile and the psi(t)
 //                   rows around it (3 x 3 rows per component); at odd parity a population row comes from the neighbour
 //                   row (y - c_y, z - c_z) and is shifted by -c_x: the aligned segment plus the 16-byte piece left or
 //                   right of it (16-byte cp.async; also the one-cell halo of the psi rows).  PSI part: first the flags
@@ -43,10 +43,14 @@ namespace lbm {
 #define LBM_TILE_ROW_BYTES 1024
 #endif
 constexpr int TILE_ROW_BYTES = LBM_TILE_ROW_BYTES;
-#ifndef LBM_TILE_PRODW
-#define LBM_TILE_PRODW 4
+// producer warps per block: for the STEP parts (they never wait for another block) and for the PSI parts (they wait for
+// the flags of the tiles around the PSI tile); each lane looks after one row
+#ifndef LBM_TILE_PRODS
+#define LBM_TILE_PRODS 4
 #endif
-constexpr int TILE_PROD_WARPS = LBM_TILE_PRODW;    // producer warps per block (each issues the bulk copies of its share of the rows)
+#ifndef LBM_TILE_PRODP
+#define LBM_TILE_PRODP 2
+#endif
 
 struct TileItem {
     int sx, sy, sz, sv;               // STEP part: x-segment, row of the tile to step; sv != 0: present
@@ -222,7 +226,8 @@ struct TileCfg {
     // step role of the D3Q19 models in fp64 needs more registers (19 doubles per component and thread): one team.
     static constexpr bool HEAVY = B == 8 && Q > 9;
     static constexpr int TEAMS = HEAVY ? 1 : 2;
-    static constexpr int AUX_WARPS = 1 + TILE_PROD_WARPS;                  // publisher, producers
+    static constexpr int PROD_S = HEAVY ? 2 : LBM_TILE_PRODS, PROD_P = LBM_TILE_PRODP;
+    static constexpr int AUX_WARPS = 1 + PROD_S + PROD_P;                 // publisher, producers
     static constexpr int THREADS = 32 * AUX_WARPS + TEAMS * STEP_THREADS;
     static constexpr int SROWS = NROWS + NF;                     // a stage: the STEP part's rows, then the flow rows of the PSI part
     static constexpr size_t STAGE_BYTES = (size_t)SROWS * RS * B;
@@ -231,9 +236,9 @@ struct TileCfg {
     static constexpr int NS = (215 * 1024) / STAGE_BYTES >= 4 ? 4 : (int)((215 * 1024) / STAGE_BYTES);   // stages
     static constexpr size_t ROWPTR_BYTES = (size_t)NS * 128 * sizeof(unsigned long long);   // pointers of the (up to 128) rows of a stage
     static constexpr size_t ROWSX_BYTES = (size_t)NS * 128 * sizeof(int);
-    static constexpr int NBAR = 2 * NS;
+    static constexpr int NBAR = 3 * NS;                          // per stage: STEP part landed, PSI part landed, stage free
     static constexpr size_t SMEM = NS * STAGE_BYTES + ROWPTR_BYTES + ROWSX_BYTES + NBAR * 8 + 32;
-    static_assert(SROWS <= 32 * TILE_PROD_WARPS, "one row per producer lane");
+    static_assert(NROWS <= 32 * PROD_S && NF <= 32 * PROD_P, "one row per producer lane");
     static_assert(TEAMS * STEP_WARPS <= 8, "done counters");
     static_assert(NS >= 2 && SMEM <= 227 * 1024, "shared memory");
     __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return NPOPS + t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
@@ -261,7 +266,7 @@ struct Tile {
         rowptr = (unsigned long long*)(smem + NS * C::STAGE_BYTES);
         rowsx = (int*)((unsigned char*)rowptr + C::ROWPTR_BYTES);
         full = (unsigned long long*)((unsigned char*)rowsx + C::ROWSX_BYTES);
-        empty = full + NS;
+        empty = full + 2 * NS;                              // full[2 * stage + part] (part 0: STEP rows, 1: PSI rows), empty[stage]
         done = (unsigned*)(empty + NS);
     }
     __device__ __forceinline__ R* slot_base(int stage) const {
@@ -359,17 +364,20 @@ struct Tile {
         }
         return d;
     }
-    // producer warp `pwid` looks after the rows r = pwid + TILE_PROD_WARPS * lane of every stage: rows 0 .. NROWS-1 belong to
-    // the STEP part of a ticket, rows NROWS .. SROWS-1 to its PSI part
-    __device__ __forceinline__ void produce(int pwid, unsigned n_mine, unsigned b0, unsigned stride) const {
+    // Producer warp `pw` of the `nw` warps of part PART (0: the STEP part of every ticket, rows 0 .. NROWS-1 of a stage; 1: the
+    // PSI part, rows NROWS .. SROWS-1) looks after the rows pw + nw * lane of its part.  The STEP producers never wait
+    // for another block; the PSI producers wait for the flags of the tiles around the PSI tile first.
+    template <int PART>
+    __device__ __forceinline__ void produce(int pw, int nw, unsigned n_mine, unsigned b0, unsigned stride) const {
         const int lane = (int)(threadIdx.x & 31);
-        const int r = pwid + TILE_PROD_WARPS * lane;           // (>= SROWS: no row)
-        const bool psi_row = r >= NROWS;
-        const RowDesc d = psi_row ? row_desc(r - NROWS, 1 - PARITY, true) : row_desc(r, PARITY, false);
+        const int q = pw + nw * lane;                          // row within the part
+        const int r = PART == 0 ? (q < NROWS ? q : SROWS) : (q < NF ? NROWS + q : SROWS);      // row of the stage (SROWS: none)
+        const RowDesc d = PART == 1 ? row_desc(q, 1 - PARITY, true) : row_desc(q, PARITY, false);
         const unsigned long long pol = l2_evict_first();
         // the ticket after the current one and the flag value of its PSI part are loaded one ticket ahead
-        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : TileItem{0, 0, 0, 0, 0, 0, 0, 0};
-        const int* nfl = nxt.pv ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
+        const TileItem none{0, 0, 0, 0, 0, 0, 0, 0};
+        TileItem nxt = n_mine > 0 ? item_of(w.items, b0) : none;
+        const int* nfl = (PART == 1 && nxt.pv) ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
         int nseen = nfl ? ld_relaxed(nfl) : 0;
         for (unsigned n = 0; n < n_mine; ++n) {
             const TileItem it = nxt;
@@ -377,18 +385,19 @@ struct Tile {
             const int seen = nseen;
             if (n + 1 < n_mine) {
                 nxt = item_of(w.items, b0 + (n + 1) * stride);
-                nfl = nxt.pv ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
+                nfl = (PART == 1 && nxt.pv) ? flag_around(TilePos{nxt.px, nxt.py, nxt.pz}) : nullptr;
                 nseen = nfl ? ld_relaxed(nfl) : 0;
             }
             const int stage = (int)(n % NS);
             const unsigned ph = (n / NS) & 1u;
+            unsigned long long* fb = &full[2 * stage + PART];
             // the PSI part reads what the step of the tiles around its tile has written: it is listed well after them
-            // (tile_schedule.h), so this wait is a formality -- but it is what makes the read correct
-            if (it.pv && !wait_flags(fl, seen)) return;
+            // (tile_schedule.h), so this wait is mostly a formality -- but it is what makes the read correct
+            if (PART == 1 && it.pv && !wait_flags(fl, seen)) return;
             if (!mbar_wait(&empty[stage], ph ^ 1u, w.status, 2)) return;
-            if (pwid == 0) TILE_TRACE(7, n);
-            const bool have = psi_row ? it.pv != 0 : it.sv != 0;
-            const int xs = psi_row ? it.px : it.sx, y = psi_row ? it.py : it.sy, z = psi_row ? it.pz : it.sz;
+            if (PART == 0 && pw == 0) TILE_TRACE(7, n);
+            const bool have = PART == 1 ? it.pv != 0 : it.sv != 0;
+            const int xs = PART == 1 ? it.px : it.sx, y = PART == 1 ? it.py : it.sy, z = PART == 1 ? it.pz : it.sz;
             const int x0 = xs * TILE_TX;
             const int len = min(TILE_TX, p.nx - x0);
             const R* src = nullptr;
@@ -407,24 +416,24 @@ struct Tile {
                 rowsx[stage * 128 + r] = sx;
             }
             // One cp.async.bulk (TMA unit, UBLKCP: no load/store-unit slots) per row for the segment, issued by the lane
-            // that owns the row; completion: transaction bytes on the stage's barrier.  The 16-byte pieces beside the
+            // that owns the row; completion: transaction bytes on the part's barrier.  The 16-byte pieces beside the
             // segment (periodic wrap in x) are 16-byte cp.async; the barrier also counts one arrival per lane for them.
-            const bool halo_row = r >= NPOPS && r < NROWS;     // a psi(t) row of the STEP part: one-cell halo on both sides
+            const bool halo_row = PART == 0 && r >= NPOPS && r < NROWS;     // a psi(t) row: one-cell halo on both sides
             const unsigned dst = smem_u32(slot_base(stage) + (size_t)(r < SROWS ? r : 0) * RS);
             const unsigned bytes = __reduce_add_sync(0xffffffffu, src ? (unsigned)(len * B) : 0u);
-            if (lane == 0) mbar_arrive_expect_tx(&full[stage], bytes);
+            if (lane == 0) mbar_arrive_expect_tx(fb, bytes);
             __syncwarp();
             if (src) {
 #ifndef LBM_TILE_NOHINT
-                if (!halo_row) bulk_g2s_hint(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage], pol);
+                if (!halo_row) bulk_g2s_hint(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), fb, pol);
                 else
 #endif
-                bulk_g2s(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), &full[stage]);
+                bulk_g2s(dst + (unsigned)(H * B), src + x0, (unsigned)(len * B), fb);
                 if (sx < 0 || halo_row) cp_async16(dst, src + (x0 == 0 ? p.nx - H : x0 - H));
                 if (sx > 0 || halo_row) cp_async16(dst + (unsigned)((H + len) * B), src + (x0 + len == p.nx ? 0 : x0 + len));
             }
-            cp_async_arrive(&full[stage]);
-            if (pwid == 0) TILE_TRACE(0, n);
+            cp_async_arrive(fb);
+            if (PART == 0 && pw == 0) TILE_TRACE(0, n);
         }
     }
 
@@ -582,9 +591,12 @@ struct Tile {
             const unsigned ph = (n / NS) & 1u;
             const TileItem it = nxt;                       // (loaded one ticket ahead)
             if (n + 1 < n_mine) nxt = item_of(w.items, b0 + (n + 1) * stride);
-            if (!mbar_wait(&full[stage], ph, w.status, 1)) return;
             const bool do_step = n % C::TEAMS == (unsigned)team;
             const bool do_psi = C::TEAMS == 1 || (n + 1) % C::TEAMS == (unsigned)team;
+            // the team that steps waits for the STEP rows, the team that forms psi for the PSI rows; every step warp sees
+            // every phase of both barriers before it lets go of the stage (a parity wait must never be asked about a phase
+            // two ahead of the last one seen, and a stage is refilled only after all of its rows have landed)
+            if (do_step && !mbar_wait(&full[2 * stage], ph, w.status, 1)) return;
             if (threadIdx.x == 0) TILE_TRACE(5, n);
 #ifndef LBM_TILE_NOSTEP
             if (do_step && it.sv) {
@@ -593,6 +605,7 @@ struct Tile {
                     if (edge_row(sp.y, sp.z)) step_cells<WALLYZ>(stage, sp, t); else step_cells<false>(stage, sp, t);
                 }
             }
+            if (!mbar_wait(&full[2 * stage + 1], ph, w.status, 1)) return;
             if (do_psi && it.pv) {
                 const TilePos pp{it.px, it.py, it.pz};
                 if (t < min(TILE_TX, p.nx - pp.xs * TILE_TX)) {
@@ -600,6 +613,7 @@ struct Tile {
                 }
             }
 #endif
+            if (!do_step && !mbar_wait(&full[2 * stage], ph, w.status, 1)) return;
             __syncwarp();
             if (threadIdx.x == 0) TILE_TRACE(6, n);
             if (lane == 0) {
@@ -661,7 +675,8 @@ k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
     const int wid = (int)(threadIdx.x >> 5);
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::NS; ++s) {
-            mbar_init(&tl.full[s], 33 * TILE_PROD_WARPS);     // per producer warp: one expect_tx arrival, 32 cp.async arrivals
+            mbar_init(&tl.full[2 * s], 33 * C::PROD_S);       // per producer warp: one expect_tx arrival, 32 cp.async arrivals
+            mbar_init(&tl.full[2 * s + 1], 33 * C::PROD_P);
             mbar_init(&tl.empty[s], C::TEAMS * C::STEP_WARPS);
         }
         for (int k = 0; k < 8; ++k) tl.done[k] = 0u;
@@ -676,7 +691,8 @@ k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
     constexpr int SW = C::TEAMS * C::STEP_WARPS;
     if (wid < SW) tl.step_role(wid / C::STEP_WARPS, n_mine, b0, stride);
     else if (wid == SW) tl.publish_role(n_mine, b0, stride);
-    else tl.produce(wid - (SW + 1), n_mine, b0, stride);
+    else if (wid <= SW + C::PROD_P) tl.template produce<1>(wid - (SW + 1), C::PROD_P, n_mine, b0, stride);
+    else tl.template produce<0>(wid - (SW + 1 + C::PROD_P), C::PROD_S, n_mine, b0, stride);
 }
 
 }  // namespace lbm
