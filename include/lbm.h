@@ -169,7 +169,7 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *                       neighbours at one time level: PAPER.md:128, 136; R9) is formed in the same launch -- every
  *                       ticket also brings a tile whose surrounding tiles have been stepped -- from populations still in L2,
  *                       into a second psi buffer (allocated by the library, S * N values): every population crosses
- *                       HBM once per step in each direction (ncu: 1.04 x the algorithmic bytes on config 5).  Needs
+ *                       HBM once per step in each direction (ncu: 1.05 x the algorithmic bytes on config 5).  Needs
  *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing, no solid-node mask (LBM_EINVAL
  *                       otherwise) and the GPU to itself (all blocks co-resident); walls in y / z are handled.
  * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a
