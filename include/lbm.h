@@ -191,6 +191,14 @@ int lbm_get_path(const lbm_ctx* ctx);
 int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_s, int delay_rows, int32_t* items,
                       size_t capacity, size_t* count, int* deferred_rows);
 
+/* The tickets LBM_PATH_PIPELINE deals out round-robin to its blocks, built from that row schedule with nxs tiles per
+ * row: *count tickets of 8 int32 (sx, sy, sz, step-part present, px, py, pz, psi-part present): ticket k carries the
+ * k-th tile to step and the next tile whose psi is due; a psi part depends only on step parts of EARLIER tickets (the
+ * property that makes the kernel's waits deadlock-free; tests/test_abi.py checks it).  three_d: rows are (y, z), else
+ * (y, 0).  Host-only, needs no GPU. */
+int lbm_tile_tickets(int nm, int ns, int nxs, int rows_per_pencil, int wrap_m, int wrap_s, int delay_rows, int three_d,
+                     int32_t* tickets, size_t capacity, size_t* count);
+
 /* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a bounded wait of LBM_PATH_PIPELINE
  * timed out; lbm_run_host performs the same check before it returns). */
 int lbm_check(lbm_ctx* ctx);

@@ -326,32 +326,8 @@ int path_setup(lbm_ctx* c, int py) {
 #endif
     const int delay_rows = (delay_tiles + nxs - 1) / nxs;
     const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, py, wrap_m, wrap_s, delay_rows, nullptr);
-    // One ticket = the next tile to step and the next tile whose psi(t + 1) is due (a PSI row becomes due where the
-    // schedule lists it: every step it depends on is an EARLIER ticket); the PSI tiles left over after the last step
-    // form the tail.  A PSI part is never paired with a step listed before it is due.
-    struct Pos { int xs, y, z; size_t due; };
-    std::vector<Pos> steps, psis;
-    steps.reserve(n_tiles); psis.reserve(n_tiles);
-    for (const lbm::TileRow& r : rows) {
-        Pos q;
-        q.y = sh.d == 3 ? r.m : r.s;
-        q.z = sh.d == 3 ? r.s : 0;
-        q.due = steps.size();                 // PSI: may ride on the step ticket with this index or a later one
-        for (int xs = 0; xs < nxs; ++xs) { q.xs = xs; (r.kind == lbm::TILE_STEP ? steps : psis).push_back(q); }
-    }
-    if (steps.size() != n_tiles || psis.size() != n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
-    std::vector<lbm::TileItem> items;
-    items.reserve(n_tiles + n_tiles / 8);
-    size_t jp = 0;
-    for (size_t k = 0; k < n_tiles || jp < n_tiles; ++k) {
-        lbm::TileItem it = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (k < n_tiles) { it.sx = steps[k].xs; it.sy = steps[k].y; it.sz = steps[k].z; it.sv = 1; }
-        if (jp < n_tiles && (psis[jp].due <= k || k >= n_tiles)) {
-            it.px = psis[jp].xs; it.py = psis[jp].y; it.pz = psis[jp].z; it.pv = 1;
-            ++jp;
-        }
-        items.push_back(it);
-    }
+    const std::vector<lbm::TileItem> items = lbm::tile_tickets(rows, nxs, sh.d == 3);
+    if (items.size() < n_tiles) return fail(LBM_ECUDA, "resident-tile path: inconsistent schedule");
     c->tile_py = py;
     c->tile_blocks = blocks;
     c->tile_n_items = (long long)items.size();
@@ -789,6 +765,21 @@ int lbm_tile_schedule(int nm, int ns, int rows_per_pencil, int wrap_m, int wrap_
             items[3 * k + 1] = v[k].m;
             items[3 * k + 2] = v[k].s;
         }
+    }
+    return 0;
+}
+
+int lbm_tile_tickets(int nm, int ns, int nxs, int rows_per_pencil, int wrap_m, int wrap_s, int delay_rows, int three_d,
+                     int32_t* tickets, size_t capacity, size_t* count) {
+    if (!count) return fail(LBM_EINVAL, "count is NULL");
+    if (nm < 1 || ns < 1 || nxs < 1) return fail(LBM_EINVAL, "nm, ns and nxs must be >= 1");
+    const std::vector<lbm::TileRow> rows = lbm::tile_schedule(nm, ns, rows_per_pencil, wrap_m != 0, wrap_s != 0, delay_rows, nullptr);
+    const std::vector<lbm::TileItem> v = lbm::tile_tickets(rows, nxs, three_d != 0);
+    *count = v.size();
+    if (tickets) {
+        if (capacity < v.size()) return fail(LBM_EINVAL, "capacity too small");
+        static_assert(sizeof(lbm::TileItem) == 8 * sizeof(int32_t), "ticket layout");
+        std::memcpy(tickets, v.data(), v.size() * sizeof(lbm::TileItem));
     }
     return 0;
 }

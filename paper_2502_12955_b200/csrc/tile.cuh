@@ -52,10 +52,7 @@ constexpr int TILE_ROW_BYTES = LBM_TILE_ROW_BYTES;
 #define LBM_TILE_PRODP 2
 #endif
 
-struct TileItem {
-    int sx, sy, sz, sv;               // STEP part: x-segment, row of the tile to step; sv != 0: present
-    int px, py, pz, pv;               // PSI part: the tile whose psi(t + 1) is formed; pv != 0: present
-};
+// (struct TileItem, one ticket: tile_schedule.h)
 struct TilePos {
     int xs, y, z;
 };

@@ -101,4 +101,41 @@ inline std::vector<TileRow> tile_schedule(int nm, int ns, int py, bool wrap_m, b
     return items;
 }
 
+// One ticket of the resident-tile kernel: a tile to step and / or a tile whose psi(t + 1) is due
+struct TileItem {
+    int sx, sy, sz, sv;               // STEP part: x-segment, row of the tile to step; sv != 0: present
+    int px, py, pz, pv;               // PSI part: the tile whose psi(t + 1) is formed; pv != 0: present
+};
+
+// The tickets of one time step from the row schedule: ticket k carries the k-th tile to step (rows in schedule order,
+// nxs tiles per row, x fastest) and the next tile whose psi is due.  A PSI row is due where the schedule lists it --
+// every step it depends on is the STEP part of an EARLIER ticket, which is what makes the kernel's waits deadlock-free
+// -- so a PSI tile rides on the first ticket whose index is at least the number of tiles stepped before its row was
+// listed; the PSI tiles left over after the last step form a tail of PSI-only tickets.  three_d: rows are (y, z) = (m, s),
+// else (y, z) = (s, 0).
+inline std::vector<TileItem> tile_tickets(const std::vector<TileRow>& rows, int nxs, bool three_d) {
+    struct Pos { int xs, y, z; size_t due; };
+    std::vector<Pos> steps, psis;
+    for (const TileRow& r : rows) {
+        Pos q;
+        q.y = three_d ? r.m : r.s;
+        q.z = three_d ? r.s : 0;
+        q.due = steps.size();                 // PSI: may ride on the step ticket with this index or a later one
+        for (int xs = 0; xs < nxs; ++xs) { q.xs = xs; (r.kind == TILE_STEP ? steps : psis).push_back(q); }
+    }
+    std::vector<TileItem> items;
+    items.reserve(steps.size() + steps.size() / 8 + 16);
+    size_t jp = 0;
+    for (size_t k = 0; k < steps.size() || jp < psis.size(); ++k) {
+        TileItem it = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (k < steps.size()) { it.sx = steps[k].xs; it.sy = steps[k].y; it.sz = steps[k].z; it.sv = 1; }
+        if (jp < psis.size() && (psis[jp].due <= k || k >= steps.size())) {
+            it.px = psis[jp].xs; it.py = psis[jp].y; it.pz = psis[jp].z; it.pv = 1;
+            ++jp;
+        }
+        items.push_back(it);
+    }
+    return items;
+}
+
 }  // namespace lbm

@@ -22,7 +22,7 @@ PATHS = {"register": 0, "pipeline": 1}
 # every symbol include/lbm.h declares (tests check that the library exports each one)
 SYMBOLS = ("lbm_workspace_bytes", "lbm_create", "lbm_init_from_seed", "lbm_step", "lbm_get_macros",
            "lbm_get_force", "lbm_population_count", "lbm_get_populations", "lbm_set_populations",
-           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_tile_schedule", "lbm_check", "lbm_static_scratch_bytes", "lbm_step_static", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
+           "lbm_run_host", "lbm_set_path", "lbm_get_path", "lbm_set_mask", "lbm_tile_schedule", "lbm_tile_tickets", "lbm_check", "lbm_static_scratch_bytes", "lbm_step_static", "lbm_time", "lbm_launch_count", "lbm_kernel_timing", "lbm_kernel_time_ms", "lbm_lattice_table", "lbm_destroy",
            "lbm_last_error")
 
 
@@ -77,6 +77,7 @@ def lib():
     L.lbm_get_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_set_populations.argtypes = [C.c_void_p, C.c_void_p]
     L.lbm_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
+    L.lbm_tile_tickets.argtypes = [C.c_int] * 8 + [C.c_void_p, C.c_size_t, C.POINTER(C.c_size_t)]
     L.lbm_static_scratch_bytes.restype = C.c_size_t
     L.lbm_static_scratch_bytes.argtypes = []
     L.lbm_step_static.argtypes = [C.c_int] * 5 + [P, C.c_void_p, C.c_int]
@@ -163,6 +164,22 @@ def tile_schedule(nm, ns, rows_per_pencil, wrap_m=True, wrap_s=True, delay_rows=
     if rc != 0:
         raise LbmError(rc, last_error())
     return out, lead.value
+
+
+def tile_tickets(nm, ns, nxs, rows_per_pencil, wrap_m=True, wrap_s=True, delay_rows=0, three_d=True):
+    """The resident-tile kernel's tickets as an (n, 8) int32 array (sx, sy, sz, sv, px, py, pz, pv); host-only call."""
+    import numpy as np
+    L = lib()
+    n = C.c_size_t(0)
+    args = (int(nm), int(ns), int(nxs), int(rows_per_pencil), int(wrap_m), int(wrap_s), int(delay_rows), int(three_d))
+    rc = L.lbm_tile_tickets(*args, None, 0, C.byref(n))
+    if rc != 0:
+        raise LbmError(rc, last_error())
+    out = np.zeros((n.value, 8), np.int32)
+    rc = L.lbm_tile_tickets(*args, out.ctypes.data, n.value, C.byref(n))
+    if rc != 0:
+        raise LbmError(rc, last_error())
+    return out
 
 
 def static_scratch_bytes():

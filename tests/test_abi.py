@@ -197,3 +197,46 @@ def test_tile_schedule_is_valid(nm, ns, py, wrap_m, wrap_s, delay):
     assert deferred <= pencils * (2 * ns + 2 * (p + 2)) + 2
 
 
+
+
+@pytest.mark.parametrize("nm,ns,nxs,py,delay,three_d", [(1, 9, 3, 1, 0, False), (1, 40, 2, 1, 5, False), (6, 5, 2, 2, 0, True),
+                                                        (8, 7, 3, 3, 4, True), (5, 4, 1, 8, 2, True), (1, 1, 1, 1, 0, True),
+                                                        (12, 10, 2, 4, 30, True)])
+@pytest.mark.parametrize("wrap_m,wrap_s", [(True, True), (False, True), (True, False), (False, False)])
+def test_tile_tickets_depend_only_on_earlier_tickets(nm, ns, nxs, py, delay, three_d, wrap_m, wrap_s):
+    """The tickets the resident-tile kernel deals out round-robin (tile_schedule.h tile_tickets, used by lbm_set_path):
+    every tile is stepped by exactly one ticket and has its psi formed by exactly one ticket; the psi part of ticket k
+    reads what the steps of the (up to 27) tiles around its tile have written, and each of those steps is the step part
+    of a ticket with a SMALLER index -- with blocks that take their tickets in order and are all resident, the earliest
+    unfinished ticket can therefore always proceed; the tail of psi-only tickets stays short."""
+    import paper_2502_12955_b200 as pkg
+    tk = pkg.lbm.tile_tickets(nm, ns, nxs, py, wrap_m, wrap_s, delay, three_d).tolist()
+    n_tiles = nm * ns * nxs
+    step_at, psi_at = {}, {}
+    for k, (sx, sy, sz, sv, px, py_, pz, pv) in enumerate(tk):
+        assert sv or pv
+        if sv:
+            assert (sx, sy, sz) not in step_at and 0 <= sx < nxs
+            step_at[(sx, sy, sz)] = k
+        if pv:
+            assert (px, py_, pz) not in psi_at and 0 <= px < nxs
+            psi_at[(px, py_, pz)] = k
+    assert len(step_at) == n_tiles and len(psi_at) == n_tiles
+    assert all(tk[k][3] for k in range(n_tiles))                 # the first n_tiles tickets all step
+    def rows_around(y, z):
+        m, s = (y, z) if three_d else (0, y)
+        for dm in (-1, 0, 1):
+            for ds in (-1, 0, 1):
+                mm, ss = m + dm, s + ds
+                if (not wrap_m and not 0 <= mm < nm) or (not wrap_s and not 0 <= ss < ns):
+                    continue
+                mm, ss = mm % nm, ss % ns
+                yield (mm, ss) if three_d else (ss, 0)
+    for (px, y, z), k in psi_at.items():
+        for (yy, zz) in rows_around(y, z):
+            for dx in (-1, 0, 1):
+                assert step_at[((px + dx) % nxs, yy, zz)] < k
+    p = max(1, min(py, nm))
+    # tail: the rows that only the LAST pencil completes (its own last planes, the wrapped plane, the columns of rows
+    # beside it) and the delay -- a vanishing fraction of a large grid
+    assert len(tk) - n_tiles <= (2 * ns + 3 * (p + 2) + delay) * nxs + 1
