@@ -200,7 +200,9 @@ int lbm_tile_tickets(int nm, int ns, int nxs, int rows_per_pencil, int wrap_m, i
                      int32_t* tickets, size_t capacity, size_t* count);
 
 /* Synchronise the stream and report deferred device-side errors (LBM_ECUDA if a bounded wait of LBM_PATH_PIPELINE
- * timed out; lbm_run_host performs the same check before it returns). */
+ * timed out; lbm_run_host performs the same check before it returns).  Without a synchronisation, lbm_step,
+ * lbm_get_macros and lbm_get_populations report such an error of an earlier, completed lbm_step (a pinned host copy
+ * of the status word is refreshed at the end of every lbm_step on that path). */
 int lbm_check(lbm_ctx* ctx);
 
 /* The Shan-Chen step for callers that must not allocate (code under CUDA-graph capture set-up, serving loops, harnesses

@@ -164,6 +164,7 @@ struct lbm_ctx {
     size_t tile_n_tiles;
     int tile_epoch;
     bool path_user_set;               // the caller chose the path (lbm_set_path): no automatic switch
+    int* tile_status_host;            // pinned host mirror of the device status word, refreshed after every lbm_step on the tile path
 
     const void* kp() const { return p.precision == 64 ? (const void*)&kp64 : (const void*)&kp32; }
     // kernel variant: 0 fully periodic, 1 bounce-back walls (bc), 2 with a solid-node mask
@@ -282,7 +283,8 @@ void tile_free(lbm_ctx* c) {
         if (c->psi != c->psi_ws) { set_psi(c, c->psi_ws); c->psi_t = -1; }
         cudaFree(extra);
     }
-    c->tile_items = nullptr; c->tile_flags = nullptr; c->psi_alt = nullptr;
+    if (c->tile_status_host) cudaFreeHost(c->tile_status_host);
+    c->tile_items = nullptr; c->tile_flags = nullptr; c->psi_alt = nullptr; c->tile_status_host = nullptr;
     c->path = LBM_PATH_REGISTER;
 }
 
@@ -336,6 +338,8 @@ int path_setup(lbm_ctx* c, int py) {
     cudaError_t e = cudaMalloc((void**)&c->tile_items, items.size() * sizeof(lbm::TileItem));
     if (e == cudaSuccess) e = cudaMalloc((void**)&c->tile_flags, (c->tile_n_tiles + 1) * sizeof(int));    // flags, status word
     if (e == cudaSuccess) e = cudaMalloc(&c->psi_alt, sh.psi_bytes);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->tile_status_host, sizeof(int), cudaHostAllocDefault);
+    if (e == cudaSuccess) *c->tile_status_host = 0;
     if (e != cudaSuccess) { cudaGetLastError(); tile_free(c); return fail(LBM_ENOMEM, "cudaMalloc of the schedule failed"); }
     CK(cudaMemcpyAsync(c->tile_items, items.data(), items.size() * sizeof(lbm::TileItem), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemsetAsync(c->tile_flags, 0, (c->tile_n_tiles + 1) * sizeof(int), c->stream));
@@ -377,6 +381,16 @@ int run_tile(lbm_ctx* c) {
     c->psi_alt = cur;
     c->psi_t = c->t + 1;
     return mark(c, 0);
+}
+
+// The status word as of the last lbm_step that has COMPLETED on the tile path (its copy into the pinned mirror is the
+// last thing that call enqueues): a timed-out wait is reported by the next API call at the latest, without a
+// synchronisation; lbm_check / lbm_run_host report it exactly
+int tile_status_seen(lbm_ctx* c) {
+    if (c->tile_status_host && *(volatile int*)c->tile_status_host != 0)
+        return fail(LBM_ECUDA, "resident-tile kernel: a bounded wait timed out in an earlier lbm_step (status " +
+                                   std::to_string(*(volatile int*)c->tile_status_host) + "); the state is invalid");
+    return 0;
 }
 
 // deferred device-side error of the resident-tile path (a bounded wait gave up); the stream must be idle
@@ -434,7 +448,7 @@ lbm_ctx* lbm_create(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     c->timing = false;
     c->graph_exec = nullptr; c->graph_capture_stream = nullptr; c->graph_failed = false;
     c->path = LBM_PATH_REGISTER; c->tile_items = nullptr; c->tile_flags = nullptr;
-    c->tile_py = 0; c->tile_blocks = 0; c->tile_epoch = 0; c->path_user_set = false;
+    c->tile_py = 0; c->tile_blocks = 0; c->tile_epoch = 0; c->path_user_set = false; c->tile_status_host = nullptr;
     if (cudaGetDevice(&c->device) != cudaSuccess) { g_err = "lbm_create: cudaGetDevice failed"; delete c; return nullptr; }
     if (p->workspace) {
         if (((uintptr_t)p->workspace & 255u) != 0) { g_err = "lbm_create: workspace must be 256-byte aligned"; delete c; return nullptr; }
@@ -560,6 +574,7 @@ int lbm_step(lbm_ctx* c, int n) {
     if (!c->inited) return fail(LBM_ESTATE, "lbm_step before lbm_init_from_seed / lbm_set_populations");
     if (n < 0) return fail(LBM_EINVAL, "n < 0");
     DeviceGuard g(c->device);
+    { int rs = tile_status_seen(c); if (rs) return rs; }
     if ((c->t & 1) == 0) choose_default_path(c);
     int done = 0;
     if (c->path == LBM_PATH_REGISTER && !c->timing && !c->graph_failed && c->sh.N <= GRAPH_MAX_CELLS) {
@@ -595,6 +610,8 @@ int lbm_step(lbm_ctx* c, int n) {
         if ((rc = mark(c, 0))) return rc;
         c->t++;
     }
+    if (c->path != LBM_PATH_REGISTER && n > done)
+        CK(cudaMemcpyAsync(c->tile_status_host, c->tile_flags + c->tile_n_tiles, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     return 0;
 }
 
@@ -603,6 +620,7 @@ int lbm_get_macros(lbm_ctx* c, void* rho, void* u, void* phi, void* C) {
     if (!c->inited) return fail(LBM_ESTATE, "lbm_get_macros before init");
     if (C && !c->sh.scalar) return fail(LBM_EINVAL, "model has no scalar lattice");
     DeviceGuard g(c->device);
+    { int rs = tile_status_seen(c); if (rs) return rs; }
     if (c->sh.sc && c->psi_t != c->t) { int rc = run_psi(c); if (rc) return rc; }
     CK(c->ops->macros(c->kp(), c->model, (int)(c->t & 1), c->wmode(), rho, u, phi, C, nullptr, c->stream));
     c->launches++;
@@ -629,6 +647,7 @@ int lbm_get_populations(lbm_ctx* c, void* f) {
     if (!c || !f) return fail(LBM_EINVAL, "NULL argument");
     if (!c->inited) return fail(LBM_ESTATE, "lbm_get_populations before init");
     DeviceGuard g(c->device);
+    { int rs = tile_status_seen(c); if (rs) return rs; }
     const size_t nf = (size_t)c->sh.S * c->sh.Q * c->sh.N * c->sh.B, nh = (size_t)c->sh.Qs * c->sh.N * c->sh.B;
     if ((c->t & 1) == 0) {
         CK(cudaMemcpyAsync(f, c->f, nf, cudaMemcpyDeviceToDevice, c->stream));
