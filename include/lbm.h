@@ -72,7 +72,7 @@ typedef struct lbm_params {
     double   G[2][2];       /* Shan-Chen coupling G_{sigma sigma~}; SC1 uses G[0][0]; Eq. 11/13 */
     int32_t  psi_kind;      /* 0: psi = rho0 (1 - exp(-rho/rho0)), Eq. 10/24 ; 1: psi = rho (R3) */
     int32_t  forcing;       /* 0: Guo, Eq. 20-23; 1: Shan-Chen velocity shift, Eq. 16-19
-                               (PAPER.md:154-174): u_eq = u' + tau F / rho, no F_i term; LBM_PATH_REGISTER only */
+                               (PAPER.md:154-174): u_eq = u' + tau F / rho, no F_i term; both launch paths */
     double   rho0_psi;      /* rho0 of Eq. 10 */
     double   force[3];      /* constant body-force density; S = 2: split by mass fraction (R5) */
     int32_t  bc[3];         /* per axis: 0 periodic, 1 halfway bounce-back walls on both faces.
@@ -170,7 +170,7 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *                       ticket also brings a tile whose surrounding tiles have been stepped -- from populations still in L2,
  *                       into a second psi buffer (allocated by the library, S * N values): every population crosses
  *                       HBM once per step in each direction (ncu: 1.05 x the algorithmic bytes on config 5).  Needs
- *                       nx * sizeof(value) % 16 == 0, periodic x, Guo forcing, no solid-node mask (LBM_EINVAL
+ *                       nx * sizeof(value) % 16 == 0, periodic x, no solid-node mask (LBM_EINVAL
  *                       otherwise) and the GPU to itself (all blocks co-resident); walls in y / z are handled.
  * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a
  * two-component D3Q19 fp32 context with more than 2^21 cells to LBM_PATH_PIPELINE where it applies -- the one case

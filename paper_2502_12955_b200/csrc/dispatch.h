@@ -20,8 +20,8 @@ struct Ops {
                            cudaStream_t st);
     cudaError_t (*init)(const void* kp, int model, const InitArgs* ia, cudaStream_t st);
     // resident-tile persistent kernel of the Shan-Chen models (tile.cuh); walls: bounce-back walls in y and / or z
-    cudaError_t (*tile)(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st);
-    int (*tile_blocks)(int model, int parity, int walls);     // co-resident blocks on the current device
+    cudaError_t (*tile)(const void* kp, int model, int parity, int walls, int vshift, const TileArgs* wa, int blocks, cudaStream_t st);
+    int (*tile_blocks)(int model, int parity, int walls, int vshift);     // co-resident blocks on the current device
     int (*tile_tx)();                                         // cells per tile
 };
 

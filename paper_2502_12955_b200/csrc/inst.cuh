@@ -180,12 +180,12 @@ struct Launch {
     }
 
     // resident-tile kernel (tile.cuh): wa == nullptr -> only return the number of co-resident blocks through *out_blocks
-    template <int MODEL, bool WALLYZ>
+    template <int MODEL, bool WALLYZ, bool VSHIFT>
     static cudaError_t tile3(const KP<R>& p, int parity, const TileArgs* wa, int blocks, cudaStream_t st, int* out_blocks) {
         using C = TileCfg<R, L, MODEL>;
         constexpr size_t smem = C::SMEM;
-        auto k0 = k_tile<R, L, MODEL, 0, WALLYZ>;
-        auto k1 = k_tile<R, L, MODEL, 1, WALLYZ>;
+        auto k0 = k_tile<R, L, MODEL, 0, WALLYZ, VSHIFT>;
+        auto k1 = k_tile<R, L, MODEL, 1, WALLYZ, VSHIFT>;
         auto k = parity ? k1 : k0;
         // per device and context, cheap: set on every call
         cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -210,23 +210,25 @@ struct Launch {
         k<<<blocks, C::THREADS, smem, st>>>(p, *wa);
         return cudaGetLastError();
     }
-    static cudaError_t tile_any(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st,
+    static cudaError_t tile_any(const void* kp, int model, int parity, int walls, int vshift, const TileArgs* wa, int blocks, cudaStream_t st,
                                 int* out_blocks) {
         const KP<R>& p = *(const KP<R>*)kp;
         cudaError_t e = cudaErrorInvalidValue;
         with_sc_model(model, [&](auto M) {
-            if (walls) e = tile3<decltype(M)::value, true>(p, parity, wa, blocks, st, out_blocks);
-            else e = tile3<decltype(M)::value, false>(p, parity, wa, blocks, st, out_blocks);
+            constexpr int m = decltype(M)::value;
+            if (walls) e = vshift ? tile3<m, true, true>(p, parity, wa, blocks, st, out_blocks) : tile3<m, true, false>(p, parity, wa, blocks, st, out_blocks);
+            else e = vshift ? tile3<m, false, true>(p, parity, wa, blocks, st, out_blocks) : tile3<m, false, false>(p, parity, wa, blocks, st, out_blocks);
         });
         return e;
     }
-    static cudaError_t tile(const void* kp, int model, int parity, int walls, const TileArgs* wa, int blocks, cudaStream_t st) {
-        return tile_any(kp, model, parity, walls, wa, blocks, st, nullptr);
+    // vshift: the velocity-shift forcing scheme (Eq. 16-19) instead of Guo forcing
+    static cudaError_t tile(const void* kp, int model, int parity, int walls, int vshift, const TileArgs* wa, int blocks, cudaStream_t st) {
+        return tile_any(kp, model, parity, walls, vshift, wa, blocks, st, nullptr);
     }
-    static int tile_blocks(int model, int parity, int walls) {
+    static int tile_blocks(int model, int parity, int walls, int vshift) {
         int b = 0;
         KP<R> dummy{};
-        if (tile_any(&dummy, model, parity, walls, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
+        if (tile_any(&dummy, model, parity, walls, vshift, nullptr, 0, nullptr, &b) != cudaSuccess) { cudaGetLastError(); return 0; }
         return b;
     }
     static int tile_tx() { return TILE_ROW_BYTES / (int)sizeof(R); }

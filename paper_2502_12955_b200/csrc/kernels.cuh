@@ -370,6 +370,28 @@ __device__ __forceinline__ void cell_macros_core(const KP<T>& p, const V (*fl)[L
     cell_force_velocity<V, L, MODEL, FORCED, ADH>(p, acc, psi_own, m, adh);
 }
 
+// Shan-Chen (velocity-shift) forcing scheme, DESIGN.md section 5 row a5': common velocity u' = sum_s (j^s / tau^s) /
+// sum_s (rho^s / tau^s), Eq. 17; u^eq,s = u' + tau^s F^s / rho^s, Eq. 16
+template <class V, class L, int MODEL, class T>
+__device__ __forceinline__ void shift_velocities(const KP<T>& p, const CellMacro<V, L, MODEL>& m, V (*ueq)[3]) {
+    constexpr int S = ModelTraits<MODEL>::S;
+    V den = m.rho[0] * vbcast<V>(p.omega[0]);
+    if constexpr (S == 2) den = vfma(m.rho[1], vbcast<V>(p.omega[1]), den);
+    const V inv_den = vrecip(den);
+    V inv_rs[S];
+    static_for<0, S>([&](auto sc) { inv_rs[decltype(sc)::value] = vrecip(m.rho[decltype(sc)::value]); });
+    static_for<0, L::D>([&](auto ac) {
+        constexpr int a = decltype(ac)::value;
+        V num = m.j[0][a] * vbcast<V>(p.omega[0]);
+        if constexpr (S == 2) num = vfma(m.j[1][a], vbcast<V>(p.omega[1]), num);
+        const V up = num * inv_den;
+        static_for<0, S>([&](auto sc) {
+            constexpr int s = decltype(sc)::value;
+            ueq[s][a] = vfma(vbcast<V>(p.tau[s]) * m.F[s][a], inv_rs[s], up);
+        });
+    });
+}
+
 // steps a1-a4 given the populations of the cell (fl[s][i]) and the psi field in global memory
 template <class R, class L, int MODEL, bool FORCED, bool COH = false, class NB>
 __device__ __forceinline__ void cell_macros(const KP<R>& p, const NB& nb, const R (*fl)[L::Q], CellMacro<R, L, MODEL>& m) {
@@ -571,23 +593,7 @@ __device__ __forceinline__ void step_cell(const KP<R>& p, int x, int y, int z) {
     // Shan-Chen (velocity-shift) forcing scheme: common velocity u' = sum_s (j^s / tau^s) / sum_s (rho^s / tau^s),
     // Eq. 17; u^eq,s = u' + tau^s F^s / rho^s, Eq. 16; no forcing term F_i
     R ueq[S][3];
-    if constexpr (VSHIFT) {
-        R den = m.rho[0] * p.omega[0];
-        if constexpr (S == 2) den = vfma(m.rho[1], p.omega[1], den);
-        const R inv_den = vrecip(den);
-        R inv_rs[S];
-        static_for<0, S>([&](auto sc) { inv_rs[decltype(sc)::value] = vrecip(m.rho[decltype(sc)::value]); });
-        static_for<0, L::D>([&](auto ac) {
-            constexpr int a = decltype(ac)::value;
-            R num = m.j[0][a] * p.omega[0];
-            if constexpr (S == 2) num = vfma(m.j[1][a], p.omega[1], num);
-            const R up = num * inv_den;
-            static_for<0, S>([&](auto sc) {
-                constexpr int s = decltype(sc)::value;
-                ueq[s][a] = vfma(p.tau[s] * m.F[s][a], inv_rs[s], up);
-            });
-        });
-    }
+    if constexpr (VSHIFT) shift_velocities<R, L, MODEL>(p, m, ueq);
 
     Nbr<L::D, WALLS> ns = nb;
     asm volatile("" : "+r"(ns.xx[0]), "+r"(ns.xx[1]), "+r"(ns.xx[2]));

@@ -288,11 +288,10 @@ void tile_free(lbm_ctx* c) {
     c->path = LBM_PATH_REGISTER;
 }
 
-// what the resident-tile kernel handles (tile.cuh): Shan-Chen models with Guo forcing, periodic x, 16-byte aligned
+// what the resident-tile kernel handles (tile.cuh): Shan-Chen models with either forcing scheme, periodic x, 16-byte aligned
 // rows, walls in y / z at rest, no solid-node mask
 const char* tile_ineligible(const lbm_ctx* c) {
     if (!c->sh.sc) return "LBM_PATH_PIPELINE exists for the Shan-Chen models (BGK already moves the algorithmic bytes)";
-    if (c->forced == 2) return "velocity-shift forcing runs on LBM_PATH_REGISTER only";
     if (c->kp64.mask) return "a solid-node mask runs on LBM_PATH_REGISTER only";
     if (c->p.bc[0] != 0) return "LBM_PATH_PIPELINE needs periodic x";
     if (((size_t)c->nx * c->sh.B) % 16 != 0) return "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes";
@@ -310,8 +309,9 @@ int path_setup(lbm_ctx* c, int py) {
     const int tx = c->ops->tile_tx();
     const int nxs = (c->nx + tx - 1) / tx;
     const int walls = c->bc_walls ? 1 : 0;
-    int resident = c->ops->tile_blocks(c->model, 0, walls);
-    const int r1 = c->ops->tile_blocks(c->model, 1, walls);
+    const int vshift = c->forced == 2 ? 1 : 0;
+    int resident = c->ops->tile_blocks(c->model, 0, walls, vshift);
+    const int r1 = c->ops->tile_blocks(c->model, 1, walls, vshift);
     if (r1 < resident) resident = r1;
     if (resident < 1) return fail(LBM_ECUDA, "resident-tile kernel: occupancy query failed");
     // default pencil: one plane of the pencil (what the psi pass trails the step by) stays far below the L2 capacity
@@ -373,7 +373,7 @@ int run_tile(lbm_ctx* c) {
 #endif
     int rc = mark(c, 0);
     if (rc) return rc;
-    CK(c->ops->tile(c->kp(), c->model, parity, c->bc_walls ? 1 : 0, &wa, c->tile_blocks, c->stream));
+    CK(c->ops->tile(c->kp(), c->model, parity, c->bc_walls ? 1 : 0, c->forced == 2 ? 1 : 0, &wa, c->tile_blocks, c->stream));
     c->launches++;
     // the launch has written psi(t + 1) to psi_alt: it is the current buffer from now on
     void* cur = c->psi;

@@ -29,8 +29,8 @@
 // most as many blocks as are co-resident: the earliest unfinished ticket of the list can always proceed.  Every wait
 // is bounded (clock64); a timeout sets bits in *status and gives up instead of hanging the GPU.
 //
-// Requirements (else the two-launch path runs): periodic x, nx * sizeof(R) a multiple of 16 bytes, no solid mask,
-// Guo forcing.  Walls in y / z are uniform per row and handled here: rows beyond a wall are redirected to the
+// Requirements (else the two-launch path runs): periodic x, nx * sizeof(R) a multiple of 16 bytes, no solid mask;
+// either forcing scheme.  Walls in y / z are uniform per row and handled here: rows beyond a wall are redirected to the
 // cell's own slot (halfway bounce-back) and left out of the psi stencil (Eq. 11-12), adhesion Eq. 14 included.
 #pragma once
 #include "kernels.cuh"
@@ -241,7 +241,7 @@ struct TileCfg {
     __host__ __device__ static constexpr int psi_row(int t, int cy, int cz) { return NPOPS + t * NPSI + (cy + 1) + (D == 3 ? 3 * (cz + 1) : 0); }
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLYZ>
+template <class R, class L, int MODEL, int PARITY, bool WALLYZ, bool VSHIFT = false>
 struct Tile {
     using C = TileCfg<R, L, MODEL>;
     using MT = typename C::MT;
@@ -546,11 +546,14 @@ struct Tile {
         });
         cell_force_velocity<V, L, MODEL, true, WALLYZ>(p, acc, psi_own, m, adh);
         const int col[4] = {x == 0 ? p.nx - 1 : x - 1, x, x + 1 == p.nx ? 0 : x + 1, x + 2 >= p.nx ? x + 2 - p.nx : x + 2};
+        V ueq[S][3];                                       // velocity-shift forcing scheme (Eq. 16-19): no forcing term F_i
+        if constexpr (VSHIFT) shift_velocities<V, L, MODEL>(p, m, ueq);
         static_for<0, S>([&](auto sc) {
             constexpr int s = decltype(sc)::value;
             V fl[Q];
             read_pops<L, s * Q, EDGE>(sb, stage, fl);
-            collide_component<V, L, true, s>(p, fl, m.rho[s], m.u, m.F[s]);
+            if constexpr (VSHIFT) collide_component<V, L, false, s>(p, fl, m.rho[s], ueq[s], m.F[s]);
+            else collide_component<V, L, true, s>(p, fl, m.rho[s], m.u, m.F[s]);
             write_pops<L, s * Q, EDGE>(stage, col, fl);
         });
         if constexpr (MT::SCALAR) {
@@ -662,10 +665,10 @@ struct Tile {
     }
 };
 
-template <class R, class L, int MODEL, int PARITY, bool WALLYZ>
+template <class R, class L, int MODEL, int PARITY, bool WALLYZ, bool VSHIFT>
 __global__ void __launch_bounds__(TileCfg<R, L, MODEL>::THREADS, 1)
 k_tile(const __grid_constant__ KP<R> p, const __grid_constant__ TileArgs w) {
-    using T = Tile<R, L, MODEL, PARITY, WALLYZ>;
+    using T = Tile<R, L, MODEL, PARITY, WALLYZ, VSHIFT>;
     using C = typename T::C;
     extern __shared__ __align__(128) unsigned char tile_smem[];
     const T tl(p, w, tile_smem);

@@ -432,6 +432,12 @@ PATH_CASES = [
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 0, 1), G_ads=(-0.3, 0.3))),
     ("cfg5", (132, 6, 5), dict(rmin=1.0, rmax=2.0, vol_frac=0.2, bc=(0, 1, 1), G_ads=(0.1, -0.2))),
     ("cfg5", (8, 6, 5), dict(rmin=1.0, rmax=2.0, vol_frac=0.2, bc=(0, 1, 1), G_ads=(0.1, -0.2), precision=64, tau=(0.9, 1.1))),
+    # velocity-shift forcing scheme (forcing = 1, Eq. 16-19) with unequal relaxation times
+    ("cfg5", (264, 12, 10), dict(forcing=1, rmin=2.0, rmax=4.0, vol_frac=0.1, tau=(0.9, 1.2))),
+    ("cfg5", (12, 9, 7), dict(forcing=1, rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7, bc=(0, 1, 0), G_ads=(0.2, -0.1))),
+    ("cfg3", (260, 37, 1), dict(forcing=1, force=(1e-5, 2e-5, 0.0), tau=(0.8, 1.3))),
+    ("cfg3", (132, 5, 1), dict(forcing=1, precision=32, bc=(0, 1, 0), G_ads=(0.25, -0.25))),
+    ("cfg2", (256, 40, 1), dict(forcing=1, radius=9.0)),
 ]
 PATHS = [("register", 0), ("pipeline", 0), ("pipeline", 1), ("pipeline", 3), ("pipeline", 1000)]
 
@@ -474,8 +480,8 @@ def test_pipeline_path_rejects_what_it_does_not_handle(gpu):
         dev.set_path("pipeline")                     # walls in x
     cfg = workloads.config("cfg3", grid=(8, 4, 1), forcing=1)
     dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
-    with pytest.raises(gpu.LbmError):
-        dev.set_path("pipeline")                     # velocity-shift forcing
+    dev.set_path("pipeline")                         # velocity-shift forcing: handled
+    assert dev.get_path() == "pipeline"
     cfg = workloads.config("cfg4", grid=(8, 4, 4))
     dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
     with pytest.raises(gpu.LbmError):
@@ -510,6 +516,7 @@ def test_default_path_of_large_shan_chen_grids(gpu):
 @pytest.mark.parametrize("name,grid,over", [
     ("cfg5", (520, 72, 48), dict(rmin=4.0, rmax=8.0, bc=(0, 1, 1), G_ads=(-0.2, 0.3))),       # ragged x tiles, walls in y and z
     ("cfg5", (1024, 40, 36), dict(rmin=4.0, rmax=8.0, force=(1e-6, -2e-6, 3e-6))),             # four tiles per row
+    ("cfg5", (512, 64, 40), dict(rmin=4.0, rmax=8.0, forcing=1, tau=(0.9, 1.2))),                # velocity-shift forcing
     ("cfg3", (4096, 300, 1), dict(bc=(0, 1, 0), G_ads=(0.1, -0.1))),                           # D2Q9 fp64, walls in y
     ("cfg2", (2048, 260, 1), dict(radius=60.0)),                                                # D2Q9 SC1 fp64 (psi with exp)
 ], ids=lambda v: str(v).replace(" ", ""))
