@@ -877,6 +877,32 @@ def test_couette_linear_profile(lattice, grid, axis):
     assert np.abs(m["rho"] - 1.0).max() < 1e-10
 
 
+@pytest.mark.parametrize("model,kw", [
+    ("SC2", dict(psi_kind=1, G=((0.0, 0.0), (0.0, 0.0)), rho_init=(0.7, 1.6), tau=(0.8, 0.8))),          # two components, no interaction
+    ("SC2_ADE", dict(psi_kind=1, G=((0.0, 0.0), (0.0, 0.0)), rho_init=(1.2, 0.4), tau=(0.8, 0.8), tau_c=0.9, c_init=0.3)),
+    ("SC1", dict(psi_kind=1, G=((0.0, 0.0), (0.0, 0.0)), rho_init=(1.3, 1.0), tau=(0.8, 0.8))),
+    ("BGK_T", dict(rho_init=(1.1, 1.0), tau=(0.8, 0.8), tau_c=0.7, c_init=0.6)),
+])
+def test_couette_with_a_moving_wall_for_every_model(model, kw):
+    """The moving-wall bounce-back (R24) acts on every flow lattice with its own density: without
+    interaction (G = 0) each component of a multi-component model, and the flow lattice of the thermal model, is a plain
+    LBGK fluid, so the steady state is the exact linear Couette profile of Eq. 41 for the barycentric velocity, uniform
+    densities, and an untouched scalar / internal energy (the wall is adiabatic and impermeable: plain reflection)."""
+    U, H, tau = 2e-2, 11, 0.8
+    r = RefLBM(4, H, 1, "D2Q9", model, precision=64, bc=(0, 1, 0), wall_u={(1, 1): (U, 0.0, 0.0)}, **kw)
+    r.init_from_seed(0)
+    r.step(int(12 * H * H / ((tau - 0.5) / 3)))
+    m = r.get_macros()
+    ux = m["u"][0].reshape(H, 4)
+    exact = U * (np.arange(H) + 0.5) / H
+    assert np.abs(ux - exact[:, None]).max() < 1e-10 * U
+    assert np.abs(m["u"][1]).max() < 1e-14
+    for s_ in range(r.S):
+        assert np.abs(m["rho"][s_] - kw["rho_init"][s_]).max() < 1e-10
+    if m["C"] is not None:
+        assert np.abs(m["C"] - kw["c_init"]).max() < 1e-10
+
+
 def test_walls_moving_together_drag_the_fluid_to_plug_flow():
     """Both walls moving with the same velocity: the only steady state is rigid motion u = U everywhere."""
     U = (1.5e-2, -0.5e-2, 0.0)
