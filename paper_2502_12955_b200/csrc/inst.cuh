@@ -59,17 +59,24 @@ struct Launch {
         else k_step<R, L, MODEL, 0, WALLS, FORCED, VSHIFT, MOVING><<<grid_for(p), block_for(p), 0, st>>>(p);
     }
     // forced: 0 no force, 1 Guo forcing (Eq. 20-23), 2 Shan-Chen velocity-shift forcing (Eq. 16-19);
-    // moving: some wall has a velocity (LBM_BGK with Guo forcing only)
+    // moving: some wall has a velocity (Guo forcing only)
     static cudaError_t step(const void* kp, int model, int parity, int wmode, int forced, int moving, cudaStream_t st) {
         const KP<R>& p = *(const KP<R>*)kp;
         bool ok = false;
         if (moving) {
-            if (model != M_BGK || forced == 2 || wmode == 0) return cudaErrorInvalidValue;
+            if (forced == 2 || wmode == 0) return cudaErrorInvalidValue;
             ok = with_int<3>(wmode, [&](auto W) {
                 constexpr int w = decltype(W)::value;
                 if constexpr (w != 0) {
-                    if (forced) step3<M_BGK, w, true, false, true>(p, parity, st);
-                    else step3<M_BGK, w, false, false, true>(p, parity, st);
+                    if (model == M_BGK) {
+                        if (forced) step3<M_BGK, w, true, false, true>(p, parity, st);
+                        else step3<M_BGK, w, false, false, true>(p, parity, st);
+                    } else if (model == M_BGK_T) {
+                        if (forced) step3<M_BGK_T, w, true, false, true>(p, parity, st);
+                        else step3<M_BGK_T, w, false, false, true>(p, parity, st);
+                    } else {
+                        with_sc_model(model, [&](auto M) { step3<decltype(M)::value, w, true, false, true>(p, parity, st); });
+                    }
                 }
             });
         } else if (model == M_BGK) {

@@ -89,8 +89,8 @@ std::string validate(int nx, int ny, int nz, int lattice, int model, const lbm_p
     for (int a = 0; a < 3; ++a)
         for (int sd = 0; sd < 2; ++sd)
             for (int b = 0; b < 3; ++b)
-                if (p->bc[a] == 1 && p->wall_u[a][sd][b] != 0.0 && (model != LBM_BGK || p->forcing != 0))
-                    return "moving walls (wall_u) are implemented for LBM_BGK with Guo forcing only";
+                if (p->bc[a] == 1 && p->wall_u[a][sd][b] != 0.0 && p->forcing != 0)
+                    return "moving walls (wall_u) are implemented for Guo forcing (forcing = 0) only";
     if (sh) {
         sh->S = S;
         sh->d = lattice == LBM_D3Q19 ? 3 : 2;
@@ -293,6 +293,7 @@ void tile_free(lbm_ctx* c) {
 const char* tile_ineligible(const lbm_ctx* c) {
     if (!c->sh.sc) return "LBM_PATH_PIPELINE exists for the Shan-Chen models (BGK already moves the algorithmic bytes)";
     if (c->kp64.mask) return "a solid-node mask runs on LBM_PATH_REGISTER only";
+    if (c->moving) return "moving walls run on LBM_PATH_REGISTER only";
     if (c->p.bc[0] != 0) return "LBM_PATH_PIPELINE needs periodic x";
     if (((size_t)c->nx * c->sh.B) % 16 != 0) return "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes";
     return nullptr;
@@ -878,10 +879,15 @@ int lbm_step_static(int nx, int ny, int nz, int lattice, int model, const lbm_pa
     fill_kp(c.kp64, &c);
     fill_kp(c.kp32, &c);
     const int wmode = c.bc_walls ? 1 : 0;
+    int moving = 0;
+    for (int a = 0; a < 3; ++a)
+        for (int sd = 0; sd < 2; ++sd)
+            for (int b = 0; b < 3; ++b)
+                if (p->bc[a] == 1 && p->wall_u[a][sd][b] != 0.0) moving = 1;
     for (int k = 0; k < n; ++k) {
         // a2 writes psi of every cell before a3 reads any: nothing in the scratch needs to start at zero
         CK(c.ops->psi(c.kp(), model, k & 1, wmode, c.stream));
-        CK(c.ops->step(c.kp(), model, k & 1, wmode, c.forced, 0, c.stream));
+        CK(c.ops->step(c.kp(), model, k & 1, wmode, c.forced, moving, c.stream));
     }
     return 0;
 }

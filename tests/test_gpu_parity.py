@@ -98,6 +98,12 @@ SMALL = [
     ("cfg4", (5, 4, 7), dict(bc=(0, 0, 1), force=(0.0, 0.0, 0.0), wall_u={(2, 1): (0.02, -0.01, 0.0)})),
     ("cfg4", (6, 5, 4), dict(bc=(1, 1, 1), wall_u={(0, 0): (0.0, 0.01, 0.02), (1, 1): (0.01, 0.0, -0.01), (2, 0): (0.02, 0.01, 0.0)}, precision=32)),
     ("cfg1", (9, 6, 1), dict(bc=(0, 1, 0), wall_u={(1, 0): (-0.01, 0.0, 0.0), (1, 1): (0.03, 0.0, 0.0)})),
+    # ... for the other models too (every flow lattice with its own density; scalar / energy lattices plainly reflected)
+    ("cfgT", (9, 6, 7), dict(wall_u={(2, 0): (0.0, 0.02, 0.0), (2, 1): (0.03, 0.0, 0.0)})),
+    ("cfgT2", (8, 9, 1), dict(bc=(1, 1, 0), force=(0.0, 0.0, 0.0), wall_u={(1, 1): (0.02, 0.0, 0.0), (0, 0): (0.0, -0.01, 0.0)}, precision=32)),
+    ("cfg2", (17, 12, 1), dict(radius=4.0, bc=(0, 1, 0), G_ads=(-0.3, 0.0), wall_u={(1, 1): (0.02, 0.0, 0.0)})),
+    ("cfg3", (16, 9, 1), dict(bc=(1, 1, 0), G_ads=(-0.2, 0.3), wall_u={(1, 0): (0.01, 0.0, 0.0), (0, 1): (0.0, 0.02, 0.0)})),
+    ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 0, 1), G_ads=(-0.3, 0.3), wall_u={(2, 1): (0.02, -0.01, 0.0)})),
     # Shan-Chen models between bounce-back walls: fluid-only stencil + adhesion force (Eq. 11-12, 14)
     ("cfg2", (33, 17, 1), dict(radius=5.0, bc=(0, 1, 0), G_ads=(-0.4, 0.0))),
     ("cfg2", (17, 12, 1), dict(radius=4.0, bc=(1, 1, 0), rho_wall=1.2)),
@@ -486,6 +492,12 @@ def test_pipeline_path_rejects_what_it_does_not_handle(gpu):
     dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
     with pytest.raises(gpu.LbmError):
         dev.set_path("pipeline")                     # BGK: the register path already moves the algorithmic bytes
+    cfg = workloads.config("cfg3", grid=(8, 4, 1), bc=(0, 1, 0), wall_u={(1, 1): (0.01, 0.0, 0.0)})
+    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
+    with pytest.raises(gpu.LbmError):
+        dev.set_path("pipeline")                     # moving walls
+    with pytest.raises(gpu.LbmError):
+        gpu.LBM(8, 4, 1, "D2Q9", "SC2", bc=(0, 1, 0), forcing=1, wall_u={(1, 1): (0.01, 0.0, 0.0)})   # moving walls need Guo forcing
 
 
 def test_default_path_of_large_shan_chen_grids(gpu):
