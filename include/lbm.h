@@ -95,8 +95,7 @@ typedef struct lbm_params {
     double   wall_u[3][2][3];  /* [axis][0 low face, 1 high face][component]: velocity of that wall (used where
                                bc[axis] == 1).  A population reflected by a moving wall loses
                                2 w_i rho^sigma (c_i . u_w) / c_s^2 (Couette flow Eq. 41), every
-                               model (scalar / energy lattices are reflected without a term); forcing 0,
-                               LBM_PATH_REGISTER only */
+                               model (scalar / energy lattices are reflected without a term); forcing 0 only */
     double   tau_s;         /* LBM_BGK_T with a solid-node mask: relaxation time tau_{e,s} = 3 alpha_s + 1/2 of the
                                solid-phase internal-energy lattice g_{s,i} on the solid nodes, Eq. 31-33
                                (PAPER.md:316-327): g^eq_s = w_i rho_s eps_s, pure diffusion among solid nodes, the

@@ -293,7 +293,6 @@ void tile_free(lbm_ctx* c) {
 const char* tile_ineligible(const lbm_ctx* c) {
     if (!c->sh.sc) return "LBM_PATH_PIPELINE exists for the Shan-Chen models (BGK already moves the algorithmic bytes)";
     if (c->kp64.mask) return "a solid-node mask runs on LBM_PATH_REGISTER only";
-    if (c->moving) return "moving walls run on LBM_PATH_REGISTER only";
     if (c->p.bc[0] != 0) return "LBM_PATH_PIPELINE needs periodic x";
     if (((size_t)c->nx * c->sh.B) % 16 != 0) return "LBM_PATH_PIPELINE needs nx * sizeof(value) to be a multiple of 16 bytes";
     return nullptr;
@@ -368,6 +367,7 @@ int run_tile(lbm_ctx* c) {
     wa.epoch = ++c->tile_epoch;
     wa.status = c->tile_flags + c->tile_n_tiles;
     wa.psi_out = c->psi_alt;
+    wa.moving = c->moving ? 1 : 0;
 #ifdef LBM_TILE_TRACE
     if (!g_trace) { cudaMalloc((void**)&g_trace, sizeof(long long) * 10 * 4096); cudaMemset(g_trace, 0, sizeof(long long) * 10 * 4096); }
     wa.trace = g_trace;

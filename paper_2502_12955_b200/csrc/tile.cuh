@@ -65,6 +65,7 @@ struct TileArgs {
     int epoch;                        // > 0, differs from every earlier launch since the flags were cleared
     int* status;                      // bits set when a bounded wait timed out
     void* psi_out;                    // psi(t + 1): S * N values, not the buffer KP::psi points at
+    int moving;                       // some wall in y / z has a velocity (KP::wall_u): moving-wall bounce-back on the edge rows
 #ifdef LBM_TILE_TRACE
     long long* trace;
 #endif
@@ -501,6 +502,25 @@ struct Tile {
             return *q;
         }
     }
+    // Moving-wall halfway bounce-back on a row next to a wall in y / z (DESIGN R24; moving_wall_correction
+    // of kernels.cuh with the row-uniform wall test): a post-collision population f*_k that leaves through a wall comes
+    // back minus 2 w_k rho^s (c_k . u_w) / c_s^2; a direction crossing two walls takes the y wall
+    __device__ __forceinline__ void moving_wall_rows(const TilePos& it, V rho_s, V* fl) const {
+        static_for<1, Q>([&](auto kc) {
+            constexpr int k = decltype(kc)::value;
+            constexpr int CY = L::c(k, 1), CZ = L::c(k, 2);
+            if constexpr (CY != 0 || CZ != 0) {
+                if (crosses(it.y, it.z, CY, CZ)) {
+                    const R* uw = nullptr;
+                    if constexpr (CY != 0) { if (wall_y() && (CY < 0 ? it.y == 0 : it.y == p.ny - 1)) uw = p.wall_u[1][CY < 0 ? 0 : 1]; }
+                    if constexpr (CZ != 0) { if (!uw && wall_z() && (CZ < 0 ? it.z == 0 : it.z == p.nz - 1)) uw = p.wall_u[2][CZ < 0 ? 0 : 1]; }
+                    const R u3[3] = {uw[0], uw[1], uw[2]};
+                    const R cuw = dotc<L, k>(u3);
+                    fl[k] = vfma(-(vconst<V>(6.0 * L::w(k)) * rho_s), vbcast<V>(cuw), fl[k]);
+                }
+            }
+        });
+    }
     template <bool EDGE>
     __device__ __forceinline__ void step_cells(int stage, const TilePos& it, int t) const {
         const int x = it.xs * TILE_TX + t;
@@ -554,6 +574,9 @@ struct Tile {
             read_pops<L, s * Q, EDGE>(sb, stage, fl);
             if constexpr (VSHIFT) collide_component<V, L, false, s>(p, fl, m.rho[s], ueq[s], m.F[s]);
             else collide_component<V, L, true, s>(p, fl, m.rho[s], m.u, m.F[s]);
+            if constexpr (EDGE) {
+                if (w.moving) moving_wall_rows(it, m.rho[s], fl);
+            }
             write_pops<L, s * Q, EDGE>(stage, col, fl);
         });
         if constexpr (MT::SCALAR) {

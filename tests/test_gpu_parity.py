@@ -438,6 +438,11 @@ PATH_CASES = [
     ("cfg5", (12, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 0, 1), G_ads=(-0.3, 0.3))),
     ("cfg5", (132, 6, 5), dict(rmin=1.0, rmax=2.0, vol_frac=0.2, bc=(0, 1, 1), G_ads=(0.1, -0.2))),
     ("cfg5", (8, 6, 5), dict(rmin=1.0, rmax=2.0, vol_frac=0.2, bc=(0, 1, 1), G_ads=(0.1, -0.2), precision=64, tau=(0.9, 1.1))),
+    # moving walls in y / z (sheared two-component flow)
+    ("cfg5", (264, 9, 7), dict(rmin=2.0, rmax=3.0, vol_frac=0.2, bc=(0, 1, 1), G_ads=(-0.3, 0.3), tau=(0.9, 1.2),
+                              wall_u={(2, 1): (0.02, -0.01, 0.0), (2, 0): (-0.02, 0.0, 0.0), (1, 0): (0.01, 0.0, 0.02)})),
+    ("cfg3", (132, 9, 1), dict(bc=(0, 1, 0), G_ads=(-0.2, 0.3), wall_u={(1, 0): (0.01, 0.0, 0.0), (1, 1): (-0.02, 0.0, 0.0)})),
+    ("cfg2", (136, 12, 1), dict(radius=4.0, bc=(0, 1, 0), G_ads=(-0.3, 0.0), wall_u={(1, 1): (0.02, 0.0, 0.0)})),
     # velocity-shift forcing scheme (forcing = 1, Eq. 16-19) with unequal relaxation times
     ("cfg5", (264, 12, 10), dict(forcing=1, rmin=2.0, rmax=4.0, vol_frac=0.1, tau=(0.9, 1.2))),
     ("cfg5", (12, 9, 7), dict(forcing=1, rmin=2.0, rmax=3.0, vol_frac=0.2, precision=64, tau=(0.9, 1.1), tau_c=0.7, bc=(0, 1, 0), G_ads=(0.2, -0.1))),
@@ -492,10 +497,6 @@ def test_pipeline_path_rejects_what_it_does_not_handle(gpu):
     dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
     with pytest.raises(gpu.LbmError):
         dev.set_path("pipeline")                     # BGK: the register path already moves the algorithmic bytes
-    cfg = workloads.config("cfg3", grid=(8, 4, 1), bc=(0, 1, 0), wall_u={(1, 1): (0.01, 0.0, 0.0)})
-    dev = gpu.LBM(*cfg["grid"], cfg["lattice"], cfg["model"], **cfg["params"])
-    with pytest.raises(gpu.LbmError):
-        dev.set_path("pipeline")                     # moving walls
     with pytest.raises(gpu.LbmError):
         gpu.LBM(8, 4, 1, "D2Q9", "SC2", bc=(0, 1, 0), forcing=1, wall_u={(1, 1): (0.01, 0.0, 0.0)})   # moving walls need Guo forcing
 
@@ -529,6 +530,7 @@ def test_default_path_of_large_shan_chen_grids(gpu):
     ("cfg5", (520, 72, 48), dict(rmin=4.0, rmax=8.0, bc=(0, 1, 1), G_ads=(-0.2, 0.3))),       # ragged x tiles, walls in y and z
     ("cfg5", (1024, 40, 36), dict(rmin=4.0, rmax=8.0, force=(1e-6, -2e-6, 3e-6))),             # four tiles per row
     ("cfg5", (512, 64, 40), dict(rmin=4.0, rmax=8.0, forcing=1, tau=(0.9, 1.2))),                # velocity-shift forcing
+    ("cfg5", (512, 48, 40), dict(rmin=4.0, rmax=8.0, bc=(0, 0, 1), wall_u={(2, 0): (-0.02, 0.0, 0.0), (2, 1): (0.02, 0.01, 0.0)})),   # shear
     ("cfg3", (4096, 300, 1), dict(bc=(0, 1, 0), G_ads=(0.1, -0.1))),                           # D2Q9 fp64, walls in y
     ("cfg2", (2048, 260, 1), dict(radius=60.0)),                                                # D2Q9 SC1 fp64 (psi with exp)
 ], ids=lambda v: str(v).replace(" ", ""))
