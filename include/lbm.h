@@ -171,7 +171,8 @@ int lbm_run_host(lbm_ctx* ctx, const void* f_in_host, int n,
  *                       into a second psi buffer (allocated by the library, S * N values): every population crosses
  *                       HBM once per step in each direction (ncu: 1.05 x the algorithmic bytes on config 5).  Needs
  *                       nx * sizeof(value) % 16 == 0, periodic x, no solid-node mask (LBM_EINVAL
- *                       otherwise) and the GPU to itself (all blocks co-resident); walls in y / z are handled.
+ *                       otherwise) and the GPU to itself (all blocks co-resident); walls in y / z, at rest or moving, and both
+ *                       forcing schemes are handled.
  * lbm_create starts on LBM_PATH_REGISTER; unless lbm_set_path was called, the first lbm_step switches a
  * two-component D3Q19 fp32 context with more than 2^21 cells to LBM_PATH_PIPELINE where it applies -- the one case
  * in which it is the faster path; smaller grids replay a CUDA graph of the register kernels.

@@ -31,7 +31,8 @@
 //
 // Requirements (else the two-launch path runs): periodic x, nx * sizeof(R) a multiple of 16 bytes, no solid mask;
 // either forcing scheme.  Walls in y / z are uniform per row and handled here: rows beyond a wall are redirected to the
-// cell's own slot (halfway bounce-back) and left out of the psi stencil (Eq. 11-12), adhesion Eq. 14 included.
+// cell's own slot (halfway bounce-back) and left out of the psi stencil (Eq. 11-12), adhesion Eq. 14 and moving walls
+// (moving_wall_rows) included.
 #pragma once
 #include "kernels.cuh"
 #include "tile_schedule.h"
